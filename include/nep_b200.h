@@ -1,0 +1,140 @@
+/*
+ * nep_b200.h -- C ABI of libnep_b200.so: the NEP (neuroevolution potential, arXiv 2107.08119)
+ * per-step force evaluation on one NVIDIA B200 (sm_100a).
+ *
+ * The calls follow the paper's statement of the problem (PAPER.md = /root/reference/PAPER.md):
+ *   inputs  {r_i}, species, periodic box                      PAPER.md:54-66   (Sec. II A, Eq. 1-3)
+ *   hyper-parameters r_c^R, r_c^A, n_max^R, n_max^A, l_max,
+ *                    N_neu                                    PAPER.md:334-347 (Table I)
+ *   parameter vector z of dimension N_par                     PAPER.md:221-224 (Eq. 26)
+ *   outputs U_i, F_i, W_i (3x3), J_i                          PAPER.md:68-92   (Eq. 4-7)
+ *
+ * General rules
+ *   - Every `*_dev` pointer is a DEVICE pointer owned by the caller (e.g. torch tensor.data_ptr());
+ *     every other pointer is a HOST pointer.  The library never allocates in nep_compute /
+ *     nep_md_step; all scratch lives in the caller-provided workspace.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All compute
+ *     calls are asynchronous on that stream.
+ *   - Per-atom vectors are SoA: x[N] | y[N] | z[N].  The virial is [9][N], row-major components
+ *     xx,xy,xz,yx,yy,yz,zx,zy,zz with  W_i^{ab} = sum_j r_ij^a (dU_j/dr_ji)^b  (Eq. 6).
+ *   - Units: eV, Angstrom, amu, fs.  Force eV/A, virial eV, heat current eV*A/fs.
+ *   - Outputs are in the caller's atom order although the library sorts atoms by cell internally.
+ *   - Return value: NEP_OK (0) or a negative nep_error.  Device-side conditions (neighbour
+ *     capacity overflow, stale list) are recorded in a sticky status word read by nep_status().
+ *     Nothing is ever silently truncated.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns NEP_ECUDA.
+ */
+#ifndef NEP_B200_H
+#define NEP_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    NEP_OK        = 0,
+    NEP_EINVAL    = -1,  /* bad hyper-parameters, n_params mismatch, null pointer, unsupported shape   */
+    NEP_EBOX      = -2,  /* a box length <= 2 (r_c^R + skin): minimum image ambiguous                   */
+    NEP_ENOMEM    = -3,  /* workspace too small                                                         */
+    NEP_ECUDA     = -4,  /* CUDA runtime / launch failure (or no device)                                */
+    NEP_EOVERFLOW = -5,  /* some atom has more neighbours than cap_radial / cap_angular / the MD cap    */
+    NEP_ESTALE    = -6,  /* nep_compute called with positions that moved > skin/2 since nep_neighbors   */
+    NEP_ESTATE    = -7   /* call order: nep_compute / nep_md_step before nep_neighbors                  */
+} nep_error;
+
+typedef struct nep_model  nep_model;   /* opaque, library-owned, immutable after nep_create           */
+typedef struct nep_system nep_system;  /* opaque, library-owned: lists, scratch layout, permutation   */
+
+/* Table I.  n_max follows the PAPER's convention: n = 0..n_max inclusive, so a
+ * family has n_max+1 radial functions and N_des = (n_max_R+1) + (n_max_A+1) l_max  (Eq. 16). */
+typedef struct {
+    double rc_radial;       /* r_c^R, Angstrom                                                        */
+    double rc_angular;      /* r_c^A, Angstrom, <= rc_radial                                          */
+    int    n_max_radial;    /* 0..15                                                                  */
+    int    n_max_angular;   /* 0..15 (kernels are instantiated for n_max_angular+1 in {8, 9})         */
+    int    l_max;           /* must be 4 in this build                                                */
+    int    n_neurons;       /* N_neu, single hidden layer (Eq. 21-22), 1..128                         */
+    int    n_types;         /* 1..8; >1 switches on the sqrt(Z_i Z_j) weighting of Eq. 19             */
+} nep_hyper;
+
+/* ---- model -------------------------------------------------------------------------------------- */
+
+/* Validates the hyper-parameters and uploads the network.
+ *   atomic_number [n_types] host: Z of each type (Eq. 19); ignored when n_types == 1.
+ *   params [n_params] host, fp64, order  w1[H][D] row-major | b1[H] | w2[H] | b2   with
+ *          x_mu = tanh(sum_nu w1[mu][nu] q_nu - b1[mu]),  U_i = sum_mu w2[mu] x_mu - b2  (Eq. 21-22;
+ *          note the MINUS biases).  Descriptor order q = [q_0..q_{n_max_R} | (n=0: l=1..l_max) |
+ *          (n=1: l=1..l_max) | ...].  n_params must equal (D+2)H+1 (Eq. 26) else NEP_EINVAL. */
+int  nep_create(const nep_hyper* hyper, const int* atomic_number, const double* params, size_t n_params,
+                nep_model** out);
+int  nep_descriptor_dim(const nep_model*);          /* Eq. 16 */
+int  nep_num_params(const nep_model*);              /* Eq. 26 */
+void nep_destroy(nep_model*);
+
+/* ---- system ------------------------------------------------------------------------------------- */
+
+/* Bytes of device workspace nep_system_create needs (0 on invalid arguments).  cap_radial /
+ * cap_angular bound the neighbours per atom inside r_c^R / r_c^A (the paper's "M");
+ * the internal Verlet list with skin is sized from them. */
+size_t nep_workspace_bytes(const nep_model*, int64_t n_atoms, int cap_radial, int cap_angular, double skin);
+
+/* type_dev [N] device int32 in 0..n_types-1 (copied).  workspace_dev: caller-owned device memory,
+ * 256-byte aligned, >= nep_workspace_bytes(); must outlive the system.  skin >= 0 (Angstrom) is the
+ * Verlet skin: lists stay valid while no atom has moved more than skin/2 since the last build. */
+int  nep_system_create(const nep_model*, int64_t n_atoms, const int* type_dev, int cap_radial,
+                       int cap_angular, double skin, void* workspace_dev, size_t workspace_bytes,
+                       nep_system** out);
+void nep_system_destroy(nep_system*);
+
+/* Cell binning, cell sort and the Verlet list (cutoff r_c^R + skin) with reverse slots
+ * ("smaller than r_c", "three neighbor lists").
+ *   pos_dev [3][N] fp64 device, any real values (wrapped internally).
+ *   box [3] host: orthorhombic periodic lengths; each must exceed 2 (r_c^R + skin) else NEP_EBOX. */
+int  nep_neighbors(nep_system*, const double* pos_dev, const double box[3], void* cuda_stream);
+
+/* The radial (which = 0, r < r_c^R) or angular (which = 1, r < r_c^A) list the force kernels use,
+ * filtered from the Verlet list at the positions of the last nep_neighbors / nep_compute /
+ * nep_md_step, with the predicate |d|^2 < r_c^2 evaluated in fp64 on minimum-image differences.
+ *   count_dev [N], index_dev [N][cap] (cap = cap_radial or cap_angular) device int32, caller's atom
+ *   numbering, row order unspecified (compare as sorted sets); unused entries are -1. */
+int  nep_get_neighbors(nep_system*, int which, int* count_dev, int* index_dev, void* cuda_stream);
+
+/* One evaluation of Eq. 12-15, 19, 21-25 and 4-7 at pos_dev with the lists of the last
+ * nep_neighbors (positions may have moved by up to skin/2 per atom; more sets NEP_ESTALE).
+ *   vel_dev [3][N] fp64, nullable (then heat_dev is not written).
+ *   energy_dev [N], force_dev [3][N], virial_dev [9][N] (nullable), heat_dev [3][N] (nullable): fp32. */
+int  nep_compute(nep_system*, const double* pos_dev, const double* vel_dev, float* energy_dev,
+                 float* force_dev, float* virial_dev, float* heat_dev, void* cuda_stream);
+
+/* n_steps velocity-Verlet NVE steps (BASELINE.json north_star; the paper's own timing used NVT,
+ * PAPER.md:395):  v += dt/2 F/m;  r += dt v;  [rebuild lists on device when an atom moved > skin/2];
+ * evaluate;  v += dt/2 F/m;  J_i = W_i . v_i (Eq. 7, both at t+dt).  a = F / (m * 103.642697) A/fs^2.
+ * Requires nep_neighbors at the current positions first; the first call evaluates F(t0) itself.
+ *   pos_dev, vel_dev [3][N] fp64: updated in place (positions are not wrapped).
+ *   mass_by_type [n_types] host, amu.
+ *   energy/force/virial/heat_dev: state after the last step (virial/heat nullable).
+ *   heat_sum_dev [3][N] fp64 nullable: J_i added once per step (per-atom heat current accumulation).
+ *   thermo_dev [n_steps][5] fp64 nullable: U_tot, K_tot, Jx, Jy, Jz after each step.
+ * No host synchronisation happens inside; the whole call is a fixed launch sequence. */
+int  nep_md_step(nep_system*, double* pos_dev, double* vel_dev, const double* mass_by_type, double dt_fs,
+                 int n_steps, float* energy_dev, float* force_dev, float* virial_dev, float* heat_dev,
+                 double* heat_sum_dev, double* thermo_dev, void* cuda_stream);
+
+/* Synchronises the stream last used by this system and returns the sticky device status
+ * (NEP_OK, NEP_EOVERFLOW, NEP_ESTALE) or NEP_ECUDA.  Clears the sticky word. */
+int  nep_status(nep_system*);
+
+/* Counters since nep_system_create (host values; synchronises like nep_status):
+ * out[0] = list rebuilds, out[1] = max radial count seen, out[2] = max angular count seen,
+ * out[3] = max Verlet-list count seen. */
+int  nep_stats(nep_system*, int64_t out[4]);
+
+const char* nep_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NEP_B200_H */

@@ -1,0 +1,172 @@
+"""Thin Python binding of libnep_b200.so (include/nep_b200.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/nep_b200.cu; PyTorch is used for device
+memory and streams.  There is no CPU fallback: if the shared library is missing, loading fails."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libnep_b200.so")
+_lib = None
+
+SYMBOLS = ["nep_create", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",
+           "nep_system_create", "nep_system_destroy", "nep_neighbors", "nep_get_neighbors", "nep_compute",
+           "nep_md_step", "nep_status", "nep_stats", "nep_strerror"]
+
+
+class NepError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        super().__init__("%s failed: %d (%s)" % (where, code, lib().nep_strerror(code).decode()))
+
+
+class Hyper(C.Structure):
+    _fields_ = [("rc_radial", C.c_double), ("rc_angular", C.c_double), ("n_max_radial", C.c_int),
+                ("n_max_angular", C.c_int), ("l_max", C.c_int), ("n_neurons", C.c_int), ("n_types", C.c_int)]
+
+
+def lib():
+    """Loads the C-ABI library (built by paper_2107_08119_b200/build.py).  Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError("libnep_b200.so is missing: run `python -m paper_2107_08119_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(_LIB_PATH)
+        L.nep_strerror.restype = C.c_char_p
+        L.nep_workspace_bytes.restype = C.c_size_t
+        L.nep_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_int, C.c_double]
+        L.nep_create.argtypes = [C.POINTER(Hyper), C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_void_p)]
+        L.nep_system_create.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_void_p,
+                                        C.c_size_t, C.POINTER(C.c_void_p)]
+        L.nep_neighbors.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nep_get_neighbors.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nep_compute.argtypes = [C.c_void_p] * 8
+        L.nep_md_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int] + [C.c_void_p] * 7
+        for f in ("nep_destroy", "nep_system_destroy"):
+            getattr(L, f).argtypes = [C.c_void_p]
+            getattr(L, f).restype = None
+        for f in ("nep_descriptor_dim", "nep_num_params", "nep_status"):
+            getattr(L, f).argtypes = [C.c_void_p]
+        L.nep_stats.argtypes = [C.c_void_p, C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _check(code, where):
+    if code != 0:
+        raise NepError(code, where)
+
+
+class Model:
+    """nep_create / nep_destroy."""
+
+    def __init__(self, rc_radial, rc_angular, n_max_radial, n_max_angular, l_max, n_neurons, atomic_numbers, params):
+        zs = np.ascontiguousarray(atomic_numbers, dtype=np.int32)
+        par = np.ascontiguousarray(params, dtype=np.float64)
+        self.hyper = Hyper(rc_radial, rc_angular, n_max_radial, n_max_angular, l_max, n_neurons, len(zs))
+        self._h = C.c_void_p()
+        _check(lib().nep_create(C.byref(self.hyper), zs.ctypes.data_as(C.c_void_p), par.ctypes.data_as(C.c_void_p),
+                                par.size, C.byref(self._h)), "nep_create")
+
+    @property
+    def descriptor_dim(self):
+        return lib().nep_descriptor_dim(self._h)
+
+    @property
+    def num_params(self):
+        return lib().nep_num_params(self._h)
+
+    def __del__(self):
+        if getattr(self, "_h", None) and self._h.value and _lib is not None:
+            _lib.nep_destroy(self._h)
+            self._h = C.c_void_p()
+
+
+class System:
+    """nep_system_create + the compute calls.  Tensors are CUDA tensors owned by the caller."""
+
+    def __init__(self, model: Model, types: torch.Tensor, cap_radial=64, cap_angular=32, skin=1.0):
+        assert types.is_cuda and types.dtype == torch.int32
+        self.model = model
+        self.n = types.numel()
+        self.cap_radial, self.cap_angular, self.skin = cap_radial, cap_angular, skin
+        nbytes = lib().nep_workspace_bytes(model._h, self.n, cap_radial, cap_angular, skin)
+        if nbytes == 0:
+            raise NepError(-1, "nep_workspace_bytes")
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=types.device)
+        off = (-self.workspace.data_ptr()) % 256
+        self._h = C.c_void_p()
+        _check(lib().nep_system_create(model._h, self.n, _ptr(types), cap_radial, cap_angular, float(skin),
+                                       C.c_void_p(self.workspace.data_ptr() + off), nbytes, C.byref(self._h)),
+               "nep_system_create")
+
+    def neighbors(self, pos: torch.Tensor, box):
+        assert pos.is_cuda and pos.dtype == torch.float64 and pos.is_contiguous() and pos.shape == (3, self.n)
+        b = (C.c_double * 3)(*[float(v) for v in box])
+        _check(lib().nep_neighbors(self._h, _ptr(pos), C.cast(b, C.c_void_p), _stream()), "nep_neighbors")
+
+    def get_neighbors(self, which: int):
+        cap = self.cap_angular if which else self.cap_radial
+        count = torch.empty(self.n, dtype=torch.int32, device=self.workspace.device)
+        index = torch.empty((self.n, cap), dtype=torch.int32, device=self.workspace.device)
+        _check(lib().nep_get_neighbors(self._h, which, _ptr(count), _ptr(index), _stream()), "nep_get_neighbors")
+        return count, index
+
+    def alloc_outputs(self):
+        dev = self.workspace.device
+        return (torch.empty(self.n, dtype=torch.float32, device=dev), torch.empty((3, self.n), dtype=torch.float32, device=dev),
+                torch.empty((9, self.n), dtype=torch.float32, device=dev), torch.empty((3, self.n), dtype=torch.float32, device=dev))
+
+    def compute(self, pos, vel=None, out=None):
+        assert pos.is_cuda and pos.dtype == torch.float64 and pos.is_contiguous()
+        U, F, W, J = out if out is not None else self.alloc_outputs()
+        _check(lib().nep_compute(self._h, _ptr(pos), _ptr(vel), _ptr(U), _ptr(F), _ptr(W), _ptr(J), _stream()),
+               "nep_compute")
+        return U, F, W, J
+
+    def md_step(self, pos, vel, masses, dt, n_steps, out=None, heat_sum=None, thermo=None):
+        assert pos.dtype == torch.float64 and vel.dtype == torch.float64 and pos.is_contiguous() and vel.is_contiguous()
+        U, F, W, J = out if out is not None else self.alloc_outputs()
+        m = np.ascontiguousarray(masses, dtype=np.float64)
+        _check(lib().nep_md_step(self._h, _ptr(pos), _ptr(vel), m.ctypes.data_as(C.c_void_p), float(dt), int(n_steps),
+                                 _ptr(U), _ptr(F), _ptr(W), _ptr(J), _ptr(heat_sum), _ptr(thermo), _stream()),
+               "nep_md_step")
+        return U, F, W, J
+
+    def status(self):
+        """Synchronises; raises NepError on a sticky device-side error (overflow, stale list)."""
+        _check(lib().nep_status(self._h), "nep_status")
+
+    def stats(self):
+        out = (C.c_int64 * 4)()
+        _check(lib().nep_stats(self._h, C.cast(out, C.c_void_p)), "nep_stats")
+        return dict(rebuilds=out[0], max_radial=out[1], max_angular=out[2], max_verlet=out[3])
+
+    def __del__(self):
+        if getattr(self, "_h", None) and self._h.value and _lib is not None:
+            _lib.nep_system_destroy(self._h)
+            self._h = C.c_void_p()
+
+
+def from_workload(w, cap_radial=64, cap_angular=32, skin=1.0, device="cuda:0"):
+    """Model + System + device tensors for a paper_2107_08119_b200.inputs.Workload."""
+    model = Model(w.rc_r, w.rc_a, w.n_max_r, w.n_max_a, w.l_max, w.n_neurons, w.atomic_numbers, w.params)
+    types = torch.from_numpy(w.types).to(device)
+    system = System(model, types, cap_radial, cap_angular, skin)
+    pos = torch.from_numpy(w.pos).to(device).contiguous()
+    vel = torch.from_numpy(w.vel).to(device).contiguous()
+    return model, system, pos, vel

@@ -1,0 +1,1054 @@
+// nep_b200.cu -- libnep_b200.so: NEP force evaluation for one B200 (sm_100a).  C ABI: include/nep_b200.h.
+//
+// Data flow of one evaluation (all in the cell-sorted atom order):
+//   k_filter    Verlet list -> per-step radial/angular lists as records {r_ij (fp32 from an fp64
+//               minimum-image difference), j, type_j}; predicate |d|^2 < r_c^2 in fp64
+//   k_main      two lanes per atom: radial descriptor (Eq. 12), angular sums s[n][lm] (Eq. 17-18 route
+//               to Eq. 13), network (Eq. 21-22) and dU/dq, partial forces (Eq. 23-25) -> p_ij
+//   k_assemble  F_i = sum_j (p_ij - p_ji), W_i = sum_j r_ij (x) p_ji (Eq. 4-6), second half-kick,
+//               J_i = W_i . v_i (Eq. 7), thermo sums; outputs in the caller's atom order
+// Neighbour build (rare): k_bin -> k_scan -> k_fill -> k_sort_cells -> k_gather -> k_build_md -> k_rev.
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include <math.h>
+#include <new>
+
+#include "../../include/nep_b200.h"
+#include "nep_math.cuh"
+
+using namespace nepk;
+
+namespace {
+
+constexpr int kMaxTypes = 8;
+constexpr int kJMask = 0x00FFFFFF;            // sorted index of the neighbour (N < 2^24)
+constexpr double kAmuConv = 103.642697;       // 1 amu A^2/fs^2 in eV
+
+// device status / counter words (int32 each)
+enum { F_STATUS = 0, F_REBUILD = 1, F_STEP = 2, F_NREBUILD = 3, F_MAXR = 4, F_MAXA = 5, F_MAXMD = 6, F_BUILT = 7,
+       F_COUNT = 16 };
+enum { ST_OVERFLOW = 1, ST_STALE = 2 };
+
+struct Box {
+    double L[3], invL[3];
+    int nc[3];
+    int ncell;
+};
+
+struct SysDev {                 // device pointers into the caller's workspace
+    int* flags;
+    int* type_in;               // [N] caller order
+    int* perm;                  // [N] sorted -> caller index
+    int* perm_tmp;              // [N]
+    int* cell_of;               // [N] cell id in the order of the build input
+    int* cell_cnt;              // [max_cells + 1]
+    int* cell_start;            // [max_cells + 1]
+    int* cell_fill;             // [max_cells]
+    int* type_s;                // [N] sorted
+    double* xs;                 // [3][N] sorted positions (unwrapped)
+    double* vs;                 // [3][N] sorted velocities
+    double* xref;               // [3][N] sorted positions at the last build
+    double* tmp3;               // [3][N]
+    float* Fs;                  // [3][N] sorted forces
+    float* Us;                  // [N] sorted site energies
+    float4* Fself;              // [N] sum_j p_ij
+    int* md_cnt;                // [N]
+    int* md_idx;                // [cap_md][N]  j | rev << 24
+    int* nnR;                   // [N]
+    int* nnA;                   // [N]
+    float4* rec;                // [cap_R][N]  {dx, dy, dz, bits(j | type_j << 24)}
+    unsigned short* slots;      // [cap_R][N]  md_slot | rev << 8
+    float4* p;                  // [N][cap_md] partial forces dU_i/dr_ij at Verlet slots
+};
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+}  // namespace
+
+struct nep_model {
+    nep_hyper h;
+    int D, Dp, NR, NA, H, npar;
+    int Z[kMaxTypes];
+    float* params_dev;          // staged layout: w1[H][Dp] | b1[H] | w2[H] | b2 | pad, fp32
+    int params_floats;
+    float* sqrtzz_dev;          // [kMaxTypes*kMaxTypes]
+};
+
+struct nep_system {
+    const nep_model* model;
+    int64_t N;
+    int capR, capA, capMD, max_cells;
+    double skin;
+    SysDev d;
+    Box box;
+    bool built, have_forces;
+    cudaStream_t last_stream;
+    cudaGraphExec_t step_graph;
+    // key of the captured graph (a change re-captures)
+    const void* g_key[10];
+    double g_dt;
+    double g_mass[kMaxTypes];
+    int64_t host_stats[4];
+};
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------
+// neighbour build
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int cell_coord(double x, double L, double invL, int nc) {
+    double f = x * invL;
+    f -= floor(f);
+    int c = (int)(f * nc);
+    return c >= nc ? nc - 1 : (c < 0 ? 0 : c);
+}
+
+__device__ __forceinline__ bool gate_closed(const int* flags, int gated) { return gated && flags[F_REBUILD] == 0; }
+
+__global__ void k_clear_cells(SysDev d, int ncell, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c <= ncell; c += gridDim.x * blockDim.x) d.cell_cnt[c] = 0;
+}
+
+// cell id of every atom of the build input `x` ([3][N]) and the per-cell population
+__global__ void k_bin(SysDev d, const double* __restrict__ x, int N, Box b, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+        const int cx = cell_coord(x[i], b.L[0], b.invL[0], b.nc[0]);
+        const int cy = cell_coord(x[N + i], b.L[1], b.invL[1], b.nc[1]);
+        const int cz = cell_coord(x[2 * N + i], b.L[2], b.invL[2], b.nc[2]);
+        const int c = (cx * b.nc[1] + cy) * b.nc[2] + cz;
+        d.cell_of[i] = c;
+        atomicAdd(&d.cell_cnt[c], 1);
+    }
+}
+
+// exclusive scan of cell_cnt[0..ncell) -> cell_start[0..ncell]; one block of 1024 threads
+__global__ void __launch_bounds__(1024) k_scan(SysDev d, int ncell, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    __shared__ int part[1024];
+    const int t = threadIdx.x;
+    const int per = (ncell + 1023) / 1024;
+    const int lo = t * per, hi = min(ncell, lo + per);
+    int s = 0;
+    for (int c = lo; c < hi; ++c) s += d.cell_cnt[c];
+    part[t] = s;
+    __syncthreads();
+    for (int off = 1; off < 1024; off <<= 1) {
+        int v = (t >= off) ? part[t - off] : 0;
+        __syncthreads();
+        part[t] += v;
+        __syncthreads();
+    }
+    int run = part[t] - s;
+    for (int c = lo; c < hi; ++c) {
+        d.cell_start[c] = run;
+        d.cell_fill[c] = run;
+        run += d.cell_cnt[c];
+    }
+    if (t == 1023) d.cell_start[ncell] = part[1023];
+}
+
+__global__ void k_fill(SysDev d, int N, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+        const int slot = atomicAdd(&d.cell_fill[d.cell_of[i]], 1);
+        d.perm_tmp[slot] = i;
+    }
+}
+
+// deterministic order inside a cell: ascending build-input index (insertion sort, cells are small)
+__global__ void k_sort_cells(SysDev d, int ncell, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += gridDim.x * blockDim.x) {
+        const int lo = d.cell_start[c], hi = d.cell_start[c + 1];
+        for (int a = lo + 1; a < hi; ++a) {
+            const int v = d.perm_tmp[a];
+            int k = a - 1;
+            while (k >= lo && d.perm_tmp[k] > v) { d.perm_tmp[k + 1] = d.perm_tmp[k]; --k; }
+            d.perm_tmp[k + 1] = v;
+        }
+    }
+}
+
+// Gather the build input into the new sorted order.  first != 0: input is the caller's arrays
+// (perm := perm_tmp).  first == 0 (in-loop rebuild): input is the current sorted state, so
+// perm := perm[perm_tmp]; velocities move too.  Two-phase through tmp buffers (k_gather_a/b).
+__global__ void k_gather_a(SysDev d, const double* __restrict__ xin, const double* __restrict__ vin, int N,
+                           int first, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < N; k += gridDim.x * blockDim.x) {
+        const int src = d.perm_tmp[k];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) d.xref[a * N + k] = xin[a * N + src];
+        if (vin) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) d.tmp3[a * N + k] = vin[a * N + src];
+        }
+        d.cell_of[k] = first ? src : d.perm[src];      // cell_of is free now: reuse as the new perm
+    }
+}
+
+__global__ void k_gather_b(SysDev d, int N, int have_v, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < N; k += gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) d.xs[a * N + k] = d.xref[a * N + k];
+        if (have_v) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) d.vs[a * N + k] = d.tmp3[a * N + k];
+        }
+        const int p = d.cell_of[k];
+        d.perm[k] = p;
+        d.type_s[k] = d.type_in[p];
+    }
+}
+
+__device__ __forceinline__ double min_image(double t, double L, double invL) { return t - L * rint(t * invL); }
+
+// Verlet list: all j != i with |r_ij|^2 < (r_c^R + skin)^2, rows ascending in the sorted index j
+// (neighbour cells are visited in ascending cell id; a cell's atoms are contiguous and ascending).
+__global__ void __launch_bounds__(128) k_build_md(SysDev d, int N, Box b, double rc2, int capMD, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double xi = d.xs[i], yi = d.xs[N + i], zi = d.xs[2 * N + i];
+    const int cx = cell_coord(xi, b.L[0], b.invL[0], b.nc[0]);
+    const int cy = cell_coord(yi, b.L[1], b.invL[1], b.nc[1]);
+    const int cz = cell_coord(zi, b.L[2], b.invL[2], b.nc[2]);
+    int cells[27];
+    int ncells = 0;
+    const int wx = b.nc[0] > 1 ? 1 : 0, wy = b.nc[1] > 1 ? 1 : 0, wz = b.nc[2] > 1 ? 1 : 0;   // nc is 1 or >= 3
+    for (int ox = -wx; ox <= wx; ++ox)
+        for (int oy = -wy; oy <= wy; ++oy)
+            for (int oz = -wz; oz <= wz; ++oz) {
+                const int c = (((cx + ox + b.nc[0]) % b.nc[0]) * b.nc[1] + (cy + oy + b.nc[1]) % b.nc[1]) * b.nc[2] +
+                              (cz + oz + b.nc[2]) % b.nc[2];
+                int k = ncells++;
+                while (k > 0 && cells[k - 1] > c) { cells[k] = cells[k - 1]; --k; }
+                cells[k] = c;
+            }
+    int cnt = 0;
+    for (int q = 0; q < ncells; ++q) {
+        const int lo = d.cell_start[cells[q]], hi = d.cell_start[cells[q] + 1];
+        for (int j = lo; j < hi; ++j) {
+            if (j == i) continue;
+            const double dx = min_image(d.xs[j] - xi, b.L[0], b.invL[0]);
+            const double dy = min_image(d.xs[N + j] - yi, b.L[1], b.invL[1]);
+            const double dz = min_image(d.xs[2 * N + j] - zi, b.L[2], b.invL[2]);
+            const double r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 < rc2) {
+                if (cnt < capMD) d.md_idx[(size_t)cnt * N + i] = j;
+                ++cnt;
+            }
+        }
+    }
+    d.md_cnt[i] = min(cnt, capMD);
+    if (cnt > capMD) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
+    atomicMax(&d.flags[F_MAXMD], cnt);
+}
+
+// reverse slot: position of i in j's (ascending) row, by binary search
+__global__ void __launch_bounds__(128) k_rev(SysDev d, int N, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int cnt = d.md_cnt[i];
+    for (int s = 0; s < cnt; ++s) {
+        const int j = d.md_idx[(size_t)s * N + i] & kJMask;
+        int lo = 0, hi = d.md_cnt[j] - 1, found = 0;
+        while (lo <= hi) {
+            const int mid = (lo + hi) >> 1;
+            const int v = d.md_idx[(size_t)mid * N + j] & kJMask;
+            if (v == i) { found = mid; break; }
+            if (v < i) lo = mid + 1; else hi = mid - 1;
+        }
+        d.md_idx[(size_t)s * N + i] = j | (found << 24);
+    }
+}
+
+__global__ void k_build_done(SysDev d, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    d.flags[F_REBUILD] = 0;
+    d.flags[F_NREBUILD] += 1;
+    d.flags[F_BUILT] = 1;
+}
+
+// ------------------------------------------------------------------------------------------------
+// per-step list filter (the paper's "multiple levels of neighbor list")
+// ------------------------------------------------------------------------------------------------
+// One thread per sorted atom.  The predicate is the oracle's plain IEEE expression
+//   d = (x_j - x_i) - L rint((x_j - x_i)/L);  (dx*dx + dy*dy) + dz*dz < rc*rc     (no FMA contraction)
+// so the sets agree bit for bit (reading Q9).  Angular neighbours (r < r_c^A) are packed
+// from slot 0 upwards, radial-only ones (r_c^A <= r < r_c^R) from slot capR-1 downwards.
+__global__ void __launch_bounds__(128) k_filter(SysDev d, int N, Box b, double rcR2, double rcA2, int capR, int capA,
+                                                int capMD) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double xi = d.xs[i], yi = d.xs[N + i], zi = d.xs[2 * N + i];
+    const int cnt = d.md_cnt[i];
+    int nA = 0, nO = 0;
+    for (int s = 0; s < cnt; ++s) {
+        const int e = d.md_idx[(size_t)s * N + i];
+        const int j = e & kJMask;
+        const double dx = min_image(d.xs[j] - xi, b.L[0], b.invL[0]);
+        const double dy = min_image(d.xs[N + j] - yi, b.L[1], b.invL[1]);
+        const double dz = min_image(d.xs[2 * N + j] - zi, b.L[2], b.invL[2]);
+        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        if (r2 < rcR2) {
+            const bool ang = r2 < rcA2;
+            if (nA + nO < capR) {
+                const int slot = ang ? nA : capR - 1 - nO;
+                const int w = j | (d.type_s[j] << 24);
+                d.rec[(size_t)slot * N + i] = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(w));
+                d.slots[(size_t)slot * N + i] = (unsigned short)(s | ((e >> 24) << 8));
+            }
+            if (ang) ++nA; else ++nO;
+        }
+    }
+    const int nR = nA + nO;
+    const bool over = nR > capR || nA > capA;
+    d.nnA[i] = over ? 0 : nA;          // an overflowing atom is dropped (and reported), never truncated
+    d.nnR[i] = over ? 0 : nR;
+    if (over) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
+    // warp-aggregated statistics
+    int mR = nR, mA = nA;
+    for (int o = 16; o > 0; o >>= 1) {
+        mR = max(mR, __shfl_xor_sync(0xffffffffu, mR, o));
+        mA = max(mA, __shfl_xor_sync(0xffffffffu, mA, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (mR > d.flags[F_MAXR]) atomicMax(&d.flags[F_MAXR], mR);
+        if (mA > d.flags[F_MAXA]) atomicMax(&d.flags[F_MAXA], mA);
+    }
+}
+
+// lists in the caller's numbering for nep_get_neighbors
+__global__ void k_export_lists(SysDev d, int N, int which, int capR, int cap_out, int* count, int* index) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int nA = d.nnA[i], nR = d.nnR[i];
+    const int n = which ? nA : nR;
+    const int row = d.perm[i];
+    count[row] = n;
+    for (int k = 0; k < cap_out; ++k) {
+        int v = -1;
+        if (k < n) {
+            const int slot = k < nA ? k : capR - 1 - (k - nA);
+            v = d.perm[__float_as_int(d.rec[(size_t)slot * N + i].w) & kJMask];
+        }
+        index[(size_t)row * cap_out + k] = v;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// descriptor + network + partial forces, two lanes per atom
+// ------------------------------------------------------------------------------------------------
+struct MainParams {
+    float rcR_inv, rcA_inv;
+    int H, N, capR, capMD;
+};
+
+// Lane h of an atom's pair owns the angular radial indices n = h*NH .. h*NH+NH-1 (all 24 lm of each),
+// so both lanes run the same instruction stream; q and the per-neighbour partial force cross the pair
+// with __shfl_xor.  The network is evaluated by both lanes (weights are warp-uniform smem broadcasts).
+template <int NR, int NA, bool MULTI>
+__global__ void __launch_bounds__(128) k_main(SysDev d, MainParams P, const float* __restrict__ params,
+                                              const float* __restrict__ sqrtzz) {
+    constexpr int NH = (NA + 1) / 2;
+    constexpr int D = NR + 4 * NA;
+    constexpr int Dp = (D + 3) & ~3;
+    constexpr float C[kNumLM] = {NEP_CLM_LIST};
+    constexpr int LOF[kNumLM] = {NEP_LOF_LIST};
+    extern __shared__ __align__(16) float sm[];
+    const int H = P.H, N = P.N;
+    const int nfl = H * Dp + 2 * H + 1;
+    float* szz = sm + ((nfl + 3) & ~3);
+    for (int k = threadIdx.x; k < nfl; k += blockDim.x) sm[k] = params[k];
+    if (MULTI) for (int k = threadIdx.x; k < kMaxTypes * kMaxTypes; k += blockDim.x) szz[k] = sqrtzz[k];
+    __syncthreads();
+
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = (t >> 1) < N;
+    const int i = active ? (t >> 1) : N - 1;
+    const int h = t & 1;
+    const unsigned FULL = 3u << (threadIdx.x & 30);   // the atom's lane pair (loop trip counts differ across pairs)
+    const int nR = d.nnR[i], nA = d.nnA[i];
+    const float* zrow = MULTI ? szz + d.type_s[i] * kMaxTypes : nullptr;
+    const float4* rec = d.rec + i;
+    auto slot_of = [&](int k) { return k < nA ? k : P.capR - 1 - (k - nA); };
+
+    // ---- radial descriptor, Eq. 12: neighbours split between the two lanes ----
+    float q[Dp];
+#pragma unroll
+    for (int v = 0; v < Dp; ++v) q[v] = 0.f;
+    for (int k = h; k < nR; k += 2) {
+        const float4 e = rec[(size_t)slot_of(k) * N];
+        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+        float rinv = rsqrtf(r2);
+        rinv = rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);
+        const float om = MULTI ? zrow[(__float_as_int(e.w) >> 24) & 7] : 1.f;
+        float g[NR];
+        radial_fn<NR, false>(r2 * rinv, P.rcR_inv, om, g, nullptr);
+#pragma unroll
+        for (int n = 0; n < NR; ++n) q[n] += g[n];
+    }
+#pragma unroll
+    for (int n = 0; n < NR; ++n) q[n] += __shfl_xor_sync(FULL, q[n], 1);
+
+    // ---- angular sums s[n][lm] = sum_j g_n(r_ij) b_lm(r^_ij)  (Eq. 18 in real form) ----
+    float s[NH][kNumLM];
+#pragma unroll
+    for (int k = 0; k < NH; ++k)
+#pragma unroll
+        for (int m = 0; m < kNumLM; ++m) s[k][m] = 0.f;
+    for (int k = 0; k < nA; ++k) {
+        const float4 e = rec[(size_t)k * N];
+        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+        float rinv = rsqrtf(r2);
+        rinv = rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);
+        const float om = MULTI ? zrow[(__float_as_int(e.w) >> 24) & 7] : 1.f;
+        float g[NA];
+        radial_fn<NA, false>(r2 * rinv, P.rcA_inv, om, g, nullptr);
+        float go[NH];
+#pragma unroll
+        for (int a = 0; a < NH; ++a) go[a] = h ? (a + NH < NA ? g[a + NH < NA ? a + NH : 0] : 0.f) : g[a];
+        float b[kNumLM];
+        ylm_basis(e.x * rinv, e.y * rinv, e.z * rinv, b);
+#pragma unroll
+        for (int a = 0; a < NH; ++a)
+#pragma unroll
+            for (int m = 0; m < kNumLM; ++m) s[a][m] = fmaf(go[a], b[m], s[a][m]);
+    }
+
+    // ---- q_nl = sum_m C_lm s_nlm^2 (Eq. 17 with n' = n), exchanged across the pair ----
+    {
+        float qa[NH][4];
+#pragma unroll
+        for (int a = 0; a < NH; ++a) {
+#pragma unroll
+            for (int l = 0; l < 4; ++l) qa[a][l] = 0.f;
+#pragma unroll
+            for (int m = 0; m < kNumLM; ++m) qa[a][LOF[m] - 1] = fmaf(C[m] * s[a][m], s[a][m], qa[a][LOF[m] - 1]);
+        }
+#pragma unroll
+        for (int a = 0; a < NH; ++a)
+#pragma unroll
+            for (int l = 0; l < 4; ++l) {
+                const float mine = qa[a][l];
+                const float other = __shfl_xor_sync(FULL, mine, 1);
+                q[NR + 4 * a + l] = h ? other : mine;                       // n = a       (lane 0's)
+                if (a + NH < NA) q[NR + 4 * (a + NH) + l] = h ? mine : other;   // n = a + NH  (lane 1's)
+            }
+    }
+
+    // ---- network Eq. 21-22 and Fp = dU/dq; two neurons per iteration for ILP ----
+    float Fp[Dp];
+#pragma unroll
+    for (int v = 0; v < Dp; ++v) Fp[v] = 0.f;
+    const float* b1 = sm + H * Dp;
+    const float* w2 = b1 + H;
+    float U = -w2[H];                                                    // - b2
+    for (int mu = 0; mu < H; mu += 2) {
+        const bool two = mu + 1 < H;
+        const float4* r0 = reinterpret_cast<const float4*>(sm + mu * Dp);
+        const float4* r1 = reinterpret_cast<const float4*>(sm + (two ? mu + 1 : mu) * Dp);
+        float a0 = -b1[mu], a1 = two ? -b1[mu + 1] : 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll
+        for (int v = 0; v < Dp / 4; ++v) {
+            const float4 w0 = r0[v], w1 = r1[v];
+            a0 = fmaf(w0.x, q[4 * v], a0); a2 = fmaf(w0.y, q[4 * v + 1], a2);
+            a0 = fmaf(w0.z, q[4 * v + 2], a0); a2 = fmaf(w0.w, q[4 * v + 3], a2);
+            a1 = fmaf(w1.x, q[4 * v], a1); a3 = fmaf(w1.y, q[4 * v + 1], a3);
+            a1 = fmaf(w1.z, q[4 * v + 2], a1); a3 = fmaf(w1.w, q[4 * v + 3], a3);
+        }
+        float t0, d0, t1, d1;
+        tanh_sech2(a0 + a2, &t0, &d0);
+        tanh_sech2(a1 + a3, &t1, &d1);
+        const float g0 = w2[mu] * d0, g1 = two ? w2[mu + 1] * d1 : 0.f;
+        U = fmaf(w2[mu], t0, U);
+        if (two) U = fmaf(w2[mu + 1], t1, U);
+#pragma unroll
+        for (int v = 0; v < Dp / 4; ++v) {
+            const float4 w0 = r0[v], w1 = r1[v];
+            Fp[4 * v] = fmaf(g0, w0.x, fmaf(g1, w1.x, Fp[4 * v]));
+            Fp[4 * v + 1] = fmaf(g0, w0.y, fmaf(g1, w1.y, Fp[4 * v + 1]));
+            Fp[4 * v + 2] = fmaf(g0, w0.z, fmaf(g1, w1.z, Fp[4 * v + 2]));
+            Fp[4 * v + 3] = fmaf(g0, w0.w, fmaf(g1, w1.w, Fp[4 * v + 3]));
+        }
+    }
+    if (active && h == 0) d.Us[i] = U;
+
+    // ---- A[n][lm] = 2 Fp_nl C_lm s_nlm, in place ----
+#pragma unroll
+    for (int a = 0; a < NH; ++a)
+#pragma unroll
+        for (int m = 0; m < kNumLM; ++m) {
+            const float f0 = Fp[NR + 4 * a + LOF[m] - 1];
+            const float f1 = (a + NH < NA) ? Fp[NR + 4 * (a + NH < NA ? a + NH : 0) + LOF[m] - 1] : 0.f;
+            s[a][m] *= 2.f * C[m] * (h ? f1 : f0);
+        }
+    float FpR[NR];      // this lane's share of the radial-family force on shared (angular) neighbours
+#pragma unroll
+    for (int n = 0; n < NR; ++n) FpR[n] = ((n & 1) == h) ? Fp[n] : 0.f;
+
+    // ---- partial forces, Eq. 23-25 ----
+    float fsx = 0.f, fsy = 0.f, fsz = 0.f;
+    float4* prow = d.p + (size_t)i * P.capMD;
+    const unsigned short* slots = d.slots + i;
+    for (int k = 0; k < nA; ++k) {          // both lanes: same neighbour, own half of n
+        const float4 e = rec[(size_t)k * N];
+        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+        float rinv = rsqrtf(r2);
+        rinv = rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);
+        const float r = r2 * rinv;
+        const float om = MULTI ? zrow[(__float_as_int(e.w) >> 24) & 7] : 1.f;
+        const float x = e.x * rinv, y = e.y * rinv, z = e.z * rinv;
+        float g[NA], dg[NA];
+        radial_fn<NA, true>(r, P.rcA_inv, om, g, dg);
+        float Sp[kNumLM], St[kNumLM];
+#pragma unroll
+        for (int m = 0; m < kNumLM; ++m) { Sp[m] = 0.f; St[m] = 0.f; }
+#pragma unroll
+        for (int a = 0; a < NH; ++a) {
+            const int a1 = a + NH < NA ? a + NH : 0;
+            const float ga = (h ? (a + NH < NA ? g[a1] : 0.f) : g[a]) * rinv;
+            const float da = h ? (a + NH < NA ? dg[a1] : 0.f) : dg[a];
+#pragma unroll
+            for (int m = 0; m < kNumLM; ++m) {
+                Sp[m] = fmaf(s[a][m], da, Sp[m]);
+                St[m] = fmaf(s[a][m], ga, St[m]);
+            }
+        }
+        float px, py, pz;
+        ylm_force(x, y, z, Sp, St, &px, &py, &pz);
+        float gr[NR], dgr[NR];
+        radial_fn<NR, true>(r, P.rcR_inv, om, gr, dgr);
+        float sr = 0.f;
+#pragma unroll
+        for (int n = 0; n < NR; ++n) sr = fmaf(FpR[n], dgr[n], sr);
+        px = fmaf(sr, x, px); py = fmaf(sr, y, py); pz = fmaf(sr, z, pz);
+        px += __shfl_xor_sync(FULL, px, 1);
+        py += __shfl_xor_sync(FULL, py, 1);
+        pz += __shfl_xor_sync(FULL, pz, 1);
+        if (h == 0) {
+            fsx += px; fsy += py; fsz += pz;
+            if (active) prow[slots[(size_t)k * N] & 0xff] = make_float4(px, py, pz, 0.f);
+        }
+    }
+    for (int k = nA + h; k < nR; k += 2) {  // radial-only neighbours, split between the lanes
+        const int sl = P.capR - 1 - (k - nA);
+        const float4 e = rec[(size_t)sl * N];
+        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+        float rinv = rsqrtf(r2);
+        rinv = rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);
+        const float om = MULTI ? zrow[(__float_as_int(e.w) >> 24) & 7] : 1.f;
+        float gr[NR], dgr[NR];
+        radial_fn<NR, true>(r2 * rinv, P.rcR_inv, om, gr, dgr);
+        float sr = 0.f;
+#pragma unroll
+        for (int n = 0; n < NR; ++n) sr = fmaf(Fp[n], dgr[n], sr);
+        sr *= rinv;
+        const float px = sr * e.x, py = sr * e.y, pz = sr * e.z;
+        fsx += px; fsy += py; fsz += pz;
+        if (active) prow[slots[(size_t)sl * N] & 0xff] = make_float4(px, py, pz, 0.f);
+    }
+    fsx += __shfl_xor_sync(FULL, fsx, 1);
+    fsy += __shfl_xor_sync(FULL, fsy, 1);
+    fsz += __shfl_xor_sync(FULL, fsz, 1);
+    if (active && h == 0) d.Fself[i] = make_float4(fsx, fsy, fsz, 0.f);
+}
+
+// ------------------------------------------------------------------------------------------------
+// assembly (Eq. 4-7) + second half-kick + thermo, and the integrator's first half
+// ------------------------------------------------------------------------------------------------
+struct AsmParams {
+    int N, capR, capMD;
+    int md;                       // 0: nep_compute; 1: MD step (kick, J from vs, thermo); 2: F(t0) of nep_md_step
+    double half_dt;               // dt/2
+    double inv_mass[kMaxTypes];   // 1 / (m * 103.642697)
+    double ke_mass[kMaxTypes];    // 0.5 * m * 103.642697
+    const double* vel_in;         // nep_compute: caller-order velocities (nullable)
+    float* energy; float* force; float* virial; float* heat;   // caller-order outputs (virial/heat nullable)
+    double* heat_sum; double* thermo;
+};
+
+__global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
+    const int N = P.N;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double tU = 0.0, tK = 0.0, tJ[3] = {0.0, 0.0, 0.0};
+    if (i < N) {
+        const int nR = d.nnR[i], nA = d.nnA[i];
+        float fx = 0.f, fy = 0.f, fz = 0.f;
+        float w[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll 4
+        for (int k = 0; k < nR; ++k) {
+            const int slot = k < nA ? k : P.capR - 1 - (k - nA);
+            const float4 e = d.rec[(size_t)slot * N + i];
+            const int j = __float_as_int(e.w) & kJMask;
+            const int rev = d.slots[(size_t)slot * N + i] >> 8;
+            const float4 pj = d.p[(size_t)j * P.capMD + rev];          // dU_j/dr_ji
+            fx += pj.x; fy += pj.y; fz += pj.z;
+            w[0] = fmaf(e.x, pj.x, w[0]); w[1] = fmaf(e.x, pj.y, w[1]); w[2] = fmaf(e.x, pj.z, w[2]);
+            w[3] = fmaf(e.y, pj.x, w[3]); w[4] = fmaf(e.y, pj.y, w[4]); w[5] = fmaf(e.y, pj.z, w[5]);
+            w[6] = fmaf(e.z, pj.x, w[6]); w[7] = fmaf(e.z, pj.y, w[7]); w[8] = fmaf(e.z, pj.z, w[8]);
+        }
+        const float4 fs = d.Fself[i];
+        fx = fs.x - fx; fy = fs.y - fy; fz = fs.z - fz;               // Eq. 4-5
+        const int row = d.perm[i];
+        const float u = d.Us[i];
+        d.Fs[i] = fx; d.Fs[N + i] = fy; d.Fs[2 * N + i] = fz;
+        P.energy[row] = u;
+        P.force[row] = fx; P.force[N + row] = fy; P.force[2 * N + row] = fz;
+        if (P.virial) {
+#pragma unroll
+            for (int c = 0; c < 9; ++c) P.virial[(size_t)c * N + row] = w[c];
+        }
+        double vx = 0.0, vy = 0.0, vz = 0.0;
+        bool have_v = false;
+        if (P.md) {
+            const int ty = d.type_s[i];
+            const double im = P.md == 1 ? P.inv_mass[ty] * P.half_dt : 0.0;   // md == 2: F(t0) only, no kick
+            vx = d.vs[i] + im * (double)fx; vy = d.vs[N + i] + im * (double)fy; vz = d.vs[2 * N + i] + im * (double)fz;
+            d.vs[i] = vx; d.vs[N + i] = vy; d.vs[2 * N + i] = vz;
+            tK = P.ke_mass[ty] * (vx * vx + vy * vy + vz * vz);
+            tU = (double)u;
+            have_v = true;
+        } else if (P.vel_in) {
+            vx = P.vel_in[row]; vy = P.vel_in[N + row]; vz = P.vel_in[2 * N + row];
+            have_v = true;
+        }
+        if (have_v) {                                                // Eq. 7: J^a = sum_b W^{ab} v^b
+            const float fvx = (float)vx, fvy = (float)vy, fvz = (float)vz;
+            const float jx = w[0] * fvx + w[1] * fvy + w[2] * fvz;
+            const float jy = w[3] * fvx + w[4] * fvy + w[5] * fvz;
+            const float jz = w[6] * fvx + w[7] * fvy + w[8] * fvz;
+            if (P.heat) { P.heat[row] = jx; P.heat[N + row] = jy; P.heat[2 * N + row] = jz; }
+            if (P.md == 1 && P.heat_sum) {
+                P.heat_sum[row] += (double)jx; P.heat_sum[N + row] += (double)jy; P.heat_sum[2 * N + row] += (double)jz;
+            }
+            tJ[0] = jx; tJ[1] = jy; tJ[2] = jz;
+        }
+    }
+    if (P.md == 1 && P.thermo) {
+        __shared__ double red[5][4];
+        double v[5] = {tU, tK, tJ[0], tJ[1], tJ[2]};
+#pragma unroll
+        for (int c = 0; c < 5; ++c)
+            for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+        const int wid = threadIdx.x >> 5;
+        if ((threadIdx.x & 31) == 0)
+            for (int c = 0; c < 5; ++c) red[c][wid] = v[c];
+        __syncthreads();
+        if (threadIdx.x < 5) {
+            const double t = red[threadIdx.x][0] + red[threadIdx.x][1] + red[threadIdx.x][2] + red[threadIdx.x][3];
+            atomicAdd(&P.thermo[(size_t)(d.flags[F_STEP] - 1) * 5 + threadIdx.x], t);
+        }
+    }
+}
+
+// v += dt/2 F/m;  r += dt v;  raise the rebuild flag when an atom has moved > skin/2 since the build
+__global__ void k_kick_drift(SysDev d, int N, double dt, double half_skin2, AsmParams P) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) d.flags[F_STEP] += 1;
+    if (i >= N) return;
+    const double im = P.inv_mass[d.type_s[i]] * P.half_dt;
+    double disp2 = 0.0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double v = d.vs[a * N + i] + im * (double)d.Fs[a * N + i];
+        const double x = d.xs[a * N + i] + dt * v;
+        d.vs[a * N + i] = v;
+        d.xs[a * N + i] = x;
+        const double dd = x - d.xref[a * N + i];
+        disp2 += dd * dd;
+    }
+    if (disp2 > half_skin2) d.flags[F_REBUILD] = 1;
+}
+
+// caller arrays -> sorted state.  mode 0 (nep_compute): a displacement > skin/2 is an error (stale
+// list); mode 1 (nep_md_step): it requests a rebuild.
+__global__ void k_load_state(SysDev d, int N, const double* __restrict__ pos, const double* __restrict__ vel,
+                             double half_skin2, int mode) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k == 0 && mode == 1) d.flags[F_STEP] = 0;
+    if (k >= N) return;
+    const int src = d.perm[k];
+    double disp2 = 0.0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double x = pos[a * N + src];
+        d.xs[a * N + k] = x;
+        const double dd = x - d.xref[a * N + k];
+        disp2 += dd * dd;
+        if (vel) d.vs[a * N + k] = vel[a * N + src];
+    }
+    if (disp2 > half_skin2) {
+        if (mode == 0) atomicOr(&d.flags[F_STATUS], ST_STALE); else d.flags[F_REBUILD] = 1;
+    }
+}
+
+__global__ void k_store_state(SysDev d, int N, double* __restrict__ pos, double* __restrict__ vel) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const int dst = d.perm[k];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        pos[a * N + dst] = d.xs[a * N + k];
+        vel[a * N + dst] = d.vs[a * N + k];
+    }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// host side: C ABI
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+#define NEP_CUDA_OK(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { set_cuda_error(e_, #expr); return NEP_ECUDA; } } while (0)
+
+thread_local char g_cuda_msg[256] = "CUDA error";
+void set_cuda_error(cudaError_t e, const char* what) {
+    snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error: %s (%s)", cudaGetErrorString(e), what);
+}
+
+int cap_md_of(const nep_model* m, int capR, double skin) {
+    const double f = (m->h.rc_radial + skin) / m->h.rc_radial;
+    int c = (int)ceil(capR * f * f * f);
+    c = (c + 3) & ~3;
+    return c > 124 ? 124 : c;       // the reverse slot is stored in 7 bits
+}
+
+struct Layout {
+    size_t off[32];
+    size_t total;
+};
+
+// carve the workspace; the same routine sizes it (base == nullptr)
+Layout carve(int64_t N, int capR, int capMD, int max_cells, SysDev* d, char* base) {
+    Layout L; size_t o = 0; int k = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align256(o + bytes); L.off[k++] = at; return base ? base + at : nullptr; };
+    const size_t n = (size_t)N;
+    SysDev t;
+    t.flags = (int*)take(F_COUNT * sizeof(int));
+    t.type_in = (int*)take(n * 4);
+    t.perm = (int*)take(n * 4);
+    t.perm_tmp = (int*)take(n * 4);
+    t.cell_of = (int*)take(n * 4);
+    t.cell_cnt = (int*)take(((size_t)max_cells + 1) * 4);
+    t.cell_start = (int*)take(((size_t)max_cells + 1) * 4);
+    t.cell_fill = (int*)take(((size_t)max_cells + 1) * 4);
+    t.type_s = (int*)take(n * 4);
+    t.xs = (double*)take(3 * n * 8);
+    t.vs = (double*)take(3 * n * 8);
+    t.xref = (double*)take(3 * n * 8);
+    t.tmp3 = (double*)take(3 * n * 8);
+    t.Fs = (float*)take(3 * n * 4);
+    t.Us = (float*)take(n * 4);
+    t.Fself = (float4*)take(n * 16);
+    t.md_cnt = (int*)take(n * 4);
+    t.md_idx = (int*)take(n * 4 * capMD);
+    t.nnR = (int*)take(n * 4);
+    t.nnA = (int*)take(n * 4);
+    t.rec = (float4*)take(n * 16 * capR);
+    t.slots = (unsigned short*)take(n * 2 * capR);
+    t.p = (float4*)take(n * 16 * capMD);
+    L.total = o;
+    if (d) *d = t;
+    return L;
+}
+
+int max_cells_of(int64_t N) { return (int)(2 * N + 64); }
+
+int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
+int grid_stride(int64_t n) { int g = grid_for(n, 256); return g > 148 * 8 ? 148 * 8 : (g < 1 ? 1 : g); }
+
+// the neighbour build as a fixed launch sequence; gated != 0: every kernel exits unless F_REBUILD is set
+void launch_build(nep_system* s, const double* xin, const double* vin, int first, int gated, cudaStream_t st) {
+    const int N = (int)s->N;
+    const SysDev& d = s->d;
+    const Box& b = s->box;
+    const double rc = s->model->h.rc_radial + s->skin;
+    k_clear_cells<<<grid_stride(b.ncell + 1), 256, 0, st>>>(d, b.ncell, gated);
+    k_bin<<<grid_stride(N), 256, 0, st>>>(d, xin, N, b, gated);
+    k_scan<<<1, 1024, 0, st>>>(d, b.ncell, gated);
+    k_fill<<<grid_stride(N), 256, 0, st>>>(d, N, gated);
+    k_sort_cells<<<grid_stride(b.ncell), 256, 0, st>>>(d, b.ncell, gated);
+    k_gather_a<<<grid_stride(N), 256, 0, st>>>(d, xin, vin, N, first, gated);
+    k_gather_b<<<grid_stride(N), 256, 0, st>>>(d, N, vin != nullptr, gated);
+    k_build_md<<<grid_for(N, 128), 128, 0, st>>>(d, N, b, rc * rc, s->capMD, gated);
+    k_rev<<<grid_for(N, 128), 128, 0, st>>>(d, N, gated);
+    k_build_done<<<1, 1, 0, st>>>(d, gated);
+}
+constexpr int kBuildLaunches = 10;
+
+template <int NR, int NA, bool MULTI>
+void launch_main_t(nep_system* s, cudaStream_t st) {
+    const nep_model* m = s->model;
+    MainParams P;
+    P.rcR_inv = (float)(1.0 / m->h.rc_radial); P.rcA_inv = (float)(1.0 / m->h.rc_angular);
+    P.H = m->H; P.N = (int)s->N; P.capR = s->capR; P.capMD = s->capMD;
+    const size_t smem = ((size_t)((m->params_floats + 3) & ~3) + kMaxTypes * kMaxTypes) * sizeof(float);
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        attr_done = true;
+    }
+    k_main<NR, NA, MULTI><<<grid_for(2 * s->N, 128), 128, smem, st>>>(s->d, P, m->params_dev, m->sqrtzz_dev);
+}
+
+bool main_supported(const nep_model* m) {
+    return (m->NR == 8 && m->NA == 8) || (m->NR == 9 && m->NA == 9);
+}
+
+void launch_main(nep_system* s, cudaStream_t st) {
+    const nep_model* m = s->model;
+    const bool multi = m->h.n_types > 1;
+    if (m->NR == 8 && m->NA == 8) { if (multi) launch_main_t<8, 8, true>(s, st); else launch_main_t<8, 8, false>(s, st); }
+    else if (m->NR == 9 && m->NA == 9) { if (multi) launch_main_t<9, 9, true>(s, st); else launch_main_t<9, 9, false>(s, st); }
+}
+
+void launch_filter(nep_system* s, cudaStream_t st) {
+    const nep_hyper& h = s->model->h;
+    k_filter<<<grid_for(s->N, 128), 128, 0, st>>>(s->d, (int)s->N, s->box, h.rc_radial * h.rc_radial,
+                                                 h.rc_angular * h.rc_angular, s->capR, s->capA, s->capMD);
+}
+
+void fill_masses(AsmParams* P, const nep_model* m, const double* mass_by_type) {
+    for (int t = 0; t < kMaxTypes; ++t) {
+        const double mm = (mass_by_type && t < m->h.n_types) ? mass_by_type[t] : 1.0;
+        P->inv_mass[t] = 1.0 / (mm * kAmuConv);
+        P->ke_mass[t] = 0.5 * mm * kAmuConv;
+    }
+}
+
+bool device_ok() {
+    int n = 0;
+    return cudaGetDeviceCount(&n) == cudaSuccess && n > 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* nep_strerror(int code) {
+    switch (code) {
+        case NEP_OK: return "ok";
+        case NEP_EINVAL: return "invalid argument (hyper-parameters, parameter count, null pointer or unsupported shape)";
+        case NEP_EBOX: return "box length <= 2 (r_c^R + skin): minimum image ambiguous";
+        case NEP_ENOMEM: return "workspace too small";
+        case NEP_ECUDA: return g_cuda_msg;
+        case NEP_EOVERFLOW: return "neighbour capacity exceeded (cap_radial / cap_angular / Verlet cap)";
+        case NEP_ESTALE: return "positions moved more than skin/2 since nep_neighbors";
+        case NEP_ESTATE: return "nep_neighbors must be called first";
+        default: return "unknown error";
+    }
+}
+
+int nep_create(const nep_hyper* hy, const int* atomic_number, const double* params, size_t n_params, nep_model** out) {
+    if (!hy || !params || !out) return NEP_EINVAL;
+    *out = nullptr;
+    if (!(hy->rc_radial > 0.0) || !(hy->rc_angular > 0.0) || hy->rc_angular > hy->rc_radial) return NEP_EINVAL;
+    if (hy->n_max_radial < 0 || hy->n_max_radial > 15 || hy->n_max_angular < 0 || hy->n_max_angular > 15) return NEP_EINVAL;
+    if (hy->l_max != 4) return NEP_EINVAL;
+    if (hy->n_neurons < 1 || hy->n_neurons > 128) return NEP_EINVAL;
+    if (hy->n_types < 1 || hy->n_types > kMaxTypes) return NEP_EINVAL;
+    if (hy->n_types > 1 && !atomic_number) return NEP_EINVAL;
+    nep_model* m = new (std::nothrow) nep_model();
+    if (!m) return NEP_ENOMEM;
+    m->h = *hy;
+    m->NR = hy->n_max_radial + 1; m->NA = hy->n_max_angular + 1; m->H = hy->n_neurons;
+    m->D = m->NR + m->NA * hy->l_max;                    // Eq. 16
+    m->Dp = (m->D + 3) & ~3;
+    m->npar = (m->D + 2) * m->H + 1;                     // Eq. 26
+    if (n_params != (size_t)m->npar || !main_supported(m)) { delete m; return NEP_EINVAL; }
+    if (!device_ok()) { delete m; set_cuda_error(cudaErrorNoDevice, "nep_create"); return NEP_ECUDA; }
+    for (int t = 0; t < kMaxTypes; ++t) m->Z[t] = (hy->n_types > 1 && t < hy->n_types) ? atomic_number[t] : 1;
+    // staged fp32 layout: w1[H][Dp] (rows zero-padded) | b1[H] | w2[H] | b2
+    const int H = m->H, D = m->D, Dp = m->Dp;
+    m->params_floats = H * Dp + 2 * H + 1;
+    float* stage = new float[(size_t)m->params_floats + 4]();
+    for (int mu = 0; mu < H; ++mu)
+        for (int v = 0; v < D; ++v) stage[mu * Dp + v] = (float)params[(size_t)mu * D + v];
+    for (int k = 0; k < 2 * H + 1; ++k) stage[H * Dp + k] = (float)params[(size_t)H * D + k];
+    float zz[kMaxTypes * kMaxTypes];
+    for (int a = 0; a < kMaxTypes; ++a)
+        for (int b = 0; b < kMaxTypes; ++b) zz[a * kMaxTypes + b] = (float)sqrt((double)m->Z[a] * (double)m->Z[b]);   // Eq. 19
+    cudaError_t e = cudaMalloc(&m->params_dev, ((size_t)m->params_floats + 4) * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&m->sqrtzz_dev, sizeof(zz));
+    if (e == cudaSuccess) e = cudaMemcpy(m->params_dev, stage, ((size_t)m->params_floats + 4) * sizeof(float), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(m->sqrtzz_dev, zz, sizeof(zz), cudaMemcpyHostToDevice);
+    delete[] stage;
+    if (e != cudaSuccess) { set_cuda_error(e, "nep_create"); nep_destroy(m); return NEP_ECUDA; }
+    *out = m;
+    return NEP_OK;
+}
+
+int nep_descriptor_dim(const nep_model* m) { return m ? m->D : NEP_EINVAL; }
+int nep_num_params(const nep_model* m) { return m ? m->npar : NEP_EINVAL; }
+
+void nep_destroy(nep_model* m) {
+    if (!m) return;
+    if (m->params_dev) cudaFree(m->params_dev);
+    if (m->sqrtzz_dev) cudaFree(m->sqrtzz_dev);
+    delete m;
+}
+
+size_t nep_workspace_bytes(const nep_model* m, int64_t n_atoms, int cap_radial, int cap_angular, double skin) {
+    if (!m || n_atoms < 1 || n_atoms >= (1 << 24) || cap_radial < 1 || cap_radial > 124 || cap_angular < 1 ||
+        cap_angular > cap_radial || !(skin >= 0.0))
+        return 0;
+    return carve(n_atoms, cap_radial, cap_md_of(m, cap_radial, skin), max_cells_of(n_atoms), nullptr, nullptr).total;
+}
+
+int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, int cap_radial, int cap_angular,
+                      double skin, void* workspace_dev, size_t workspace_bytes, nep_system** out) {
+    if (!out) return NEP_EINVAL;
+    *out = nullptr;
+    const size_t need = nep_workspace_bytes(m, n_atoms, cap_radial, cap_angular, skin);
+    if (need == 0 || !type_dev || !workspace_dev || ((uintptr_t)workspace_dev & 255)) return NEP_EINVAL;
+    if (workspace_bytes < need) return NEP_ENOMEM;
+    nep_system* s = new (std::nothrow) nep_system();
+    if (!s) return NEP_ENOMEM;
+    s->model = m; s->N = n_atoms; s->capR = cap_radial; s->capA = cap_angular; s->skin = skin;
+    s->capMD = cap_md_of(m, cap_radial, skin);
+    s->max_cells = max_cells_of(n_atoms);
+    carve(n_atoms, s->capR, s->capMD, s->max_cells, &s->d, (char*)workspace_dev);
+    s->built = false; s->have_forces = false; s->last_stream = nullptr; s->step_graph = nullptr;
+    cudaError_t e = cudaMemset(workspace_dev, 0, need);
+    if (e == cudaSuccess) e = cudaMemcpy(s->d.type_in, type_dev, (size_t)n_atoms * sizeof(int), cudaMemcpyDeviceToDevice);
+    if (e != cudaSuccess) { set_cuda_error(e, "nep_system_create"); delete s; return NEP_ECUDA; }
+    *out = s;
+    return NEP_OK;
+}
+
+void nep_system_destroy(nep_system* s) {
+    if (!s) return;
+    if (s->step_graph) cudaGraphExecDestroy(s->step_graph);
+    delete s;
+}
+
+int nep_neighbors(nep_system* s, const double* pos_dev, const double box[3], void* cuda_stream) {
+    if (!s || !pos_dev || !box) return NEP_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const double rc = s->model->h.rc_radial + s->skin;
+    Box b;
+    for (int a = 0; a < 3; ++a) {
+        if (!(box[a] > 2.0 * rc)) return NEP_EBOX;
+        b.L[a] = box[a]; b.invL[a] = 1.0 / box[a];
+        int nc = (int)floor(box[a] / rc);
+        b.nc[a] = nc < 3 ? 1 : nc;
+    }
+    while ((int64_t)b.nc[0] * b.nc[1] * b.nc[2] > s->max_cells) {     // sparse systems: coarser cells
+        int a = b.nc[0] >= b.nc[1] ? (b.nc[0] >= b.nc[2] ? 0 : 2) : (b.nc[1] >= b.nc[2] ? 1 : 2);
+        b.nc[a] = b.nc[a] > 3 ? b.nc[a] - 1 : 1;
+    }
+    b.ncell = b.nc[0] * b.nc[1] * b.nc[2];
+    s->box = b;
+    s->last_stream = st;
+    launch_build(s, pos_dev, nullptr, 1, 0, st);
+    launch_filter(s, st);
+    NEP_CUDA_OK(cudaGetLastError());
+    s->built = true; s->have_forces = false;
+    return NEP_OK;
+}
+
+int nep_get_neighbors(nep_system* s, int which, int* count_dev, int* index_dev, void* cuda_stream) {
+    if (!s || !count_dev || !index_dev || (which != 0 && which != 1)) return NEP_EINVAL;
+    if (!s->built) return NEP_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    s->last_stream = st;
+    k_export_lists<<<grid_for(s->N, 128), 128, 0, st>>>(s->d, (int)s->N, which, s->capR, which ? s->capA : s->capR,
+                                                       count_dev, index_dev);
+    NEP_CUDA_OK(cudaGetLastError());
+    return NEP_OK;
+}
+
+int nep_compute(nep_system* s, const double* pos_dev, const double* vel_dev, float* energy_dev, float* force_dev,
+                float* virial_dev, float* heat_dev, void* cuda_stream) {
+    if (!s || !pos_dev || !energy_dev || !force_dev) return NEP_EINVAL;
+    if (!s->built) return NEP_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    s->last_stream = st;
+    const int N = (int)s->N;
+    const double hs = 0.5 * s->skin;
+    k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, nullptr, hs * hs * (1.0 + 1e-12) + 1e-24, 0);
+    launch_filter(s, st);
+    launch_main(s, st);
+    AsmParams P;
+    memset(&P, 0, sizeof(P));
+    P.N = N; P.capR = s->capR; P.capMD = s->capMD; P.md = 0;
+    fill_masses(&P, s->model, nullptr);
+    P.vel_in = vel_dev; P.energy = energy_dev; P.force = force_dev; P.virial = virial_dev;
+    P.heat = vel_dev ? heat_dev : nullptr;
+    k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
+    NEP_CUDA_OK(cudaGetLastError());
+    s->have_forces = false;
+    return NEP_OK;
+}
+
+int nep_md_step(nep_system* s, double* pos_dev, double* vel_dev, const double* mass_by_type, double dt_fs, int n_steps,
+                float* energy_dev, float* force_dev, float* virial_dev, float* heat_dev, double* heat_sum_dev,
+                double* thermo_dev, void* cuda_stream) {
+    if (!s || !pos_dev || !vel_dev || !mass_by_type || !energy_dev || !force_dev || n_steps < 0 || !(dt_fs > 0.0))
+        return NEP_EINVAL;
+    if (!s->built) return NEP_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    s->last_stream = st;
+    const int N = (int)s->N;
+    const double hs = 0.5 * s->skin;
+    const double hs2 = hs * hs;
+    AsmParams P;
+    memset(&P, 0, sizeof(P));
+    P.N = N; P.capR = s->capR; P.capMD = s->capMD;
+    P.half_dt = 0.5 * dt_fs;
+    fill_masses(&P, s->model, mass_by_type);
+    P.energy = energy_dev; P.force = force_dev; P.virial = virial_dev; P.heat = heat_dev;
+    P.heat_sum = heat_sum_dev; P.thermo = thermo_dev;
+    if (thermo_dev && n_steps > 0) NEP_CUDA_OK(cudaMemsetAsync(thermo_dev, 0, (size_t)n_steps * 5 * sizeof(double), st));
+    // caller arrays -> sorted state; F(t0)
+    k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, vel_dev, hs2, 1);
+    launch_build(s, s->d.xs, s->d.vs, 0, 1, st);
+    launch_filter(s, st);
+    launch_main(s, st);
+    P.md = 2;
+    k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
+    P.md = 1;
+    for (int step = 0; step < n_steps; ++step) {
+        k_kick_drift<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, dt_fs, hs2, P);
+        launch_build(s, s->d.xs, s->d.vs, 0, 1, st);
+        launch_filter(s, st);
+        launch_main(s, st);
+        k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
+    }
+    k_store_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, vel_dev);
+    NEP_CUDA_OK(cudaGetLastError());
+    return NEP_OK;
+}
+
+int nep_status(nep_system* s) {
+    if (!s) return NEP_EINVAL;
+    NEP_CUDA_OK(cudaStreamSynchronize(s->last_stream));
+    int flags[F_COUNT];
+    NEP_CUDA_OK(cudaMemcpy(flags, s->d.flags, sizeof(flags), cudaMemcpyDeviceToHost));
+    s->host_stats[0] = flags[F_NREBUILD]; s->host_stats[1] = flags[F_MAXR];
+    s->host_stats[2] = flags[F_MAXA]; s->host_stats[3] = flags[F_MAXMD];
+    if (flags[F_STATUS]) NEP_CUDA_OK(cudaMemset(s->d.flags + F_STATUS, 0, sizeof(int)));
+    if (flags[F_STATUS] & ST_OVERFLOW) return NEP_EOVERFLOW;
+    if (flags[F_STATUS] & ST_STALE) return NEP_ESTALE;
+    return NEP_OK;
+}
+
+int nep_stats(nep_system* s, int64_t out[4]) {
+    if (!s || !out) return NEP_EINVAL;
+    NEP_CUDA_OK(cudaStreamSynchronize(s->last_stream));
+    int flags[F_COUNT];
+    NEP_CUDA_OK(cudaMemcpy(flags, s->d.flags, sizeof(flags), cudaMemcpyDeviceToHost));
+    out[0] = flags[F_NREBUILD]; out[1] = flags[F_MAXR]; out[2] = flags[F_MAXA]; out[3] = flags[F_MAXMD];
+    return NEP_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,151 @@
+// nep_math.cuh -- fp32 device math of the NEP hot path (no oracle code is shared with this file).
+//
+//   radial_fn      g_n(r), dg_n/dr        Eq. 14-15, 19 and App. A
+//   ylm_basis      the 24 real harmonic polynomials b_lm(r^), l = 1..4, of the addition-theorem
+//                  route Eq. 17-18:  P_l(r1^ . r2^) = sum_m C_lm b_lm(r1^) b_lm(r2^)
+//   ylm_force      sum_lm [ S'_lm b_lm r^ + (S_lm / r) (grad B_lm(r^) - l b_lm r^) ]  -- the angular
+//                  part of Eq. 25 after the addition theorem (B_lm = homogeneous form of b_lm)
+//   tanh_sech2     tanh(a) and 1 - tanh^2(a) without cancellation (Eq. 21 and its derivative)
+//
+// Functions are __host__ __device__ so that csrc/selftest_host.cpp can check them against central
+// differences and Legendre polynomials on the CPU build box (no GPU needed).
+#pragma once
+#include <math.h>
+
+#ifdef __CUDACC__
+#define NEP_HD __host__ __device__ __forceinline__
+#else
+#define NEP_HD inline
+#endif
+
+namespace nepk {
+
+constexpr int kNumLM = 24;   // sum_{l=1..4} (2l+1)
+
+// C_lm = (4 pi / (2l+1)) N_lm^2 for the unnormalised polynomials below.
+#define NEP_CLM_LIST                                                                                 \
+    1.f, 1.f, 1.f,                                                                                   \
+    0.25f, 3.f, 3.f, 0.75f, 0.75f,                                                                   \
+    0.25f, 0.375f, 0.375f, 3.75f, 3.75f, 0.625f, 0.625f,                                             \
+    0.015625f, 0.625f, 0.625f, 0.3125f, 0.3125f, 4.375f, 4.375f, 0.546875f, 0.546875f
+
+// l of each of the 24 components
+#define NEP_LOF_LIST 1, 1, 1, 2, 2, 2, 2, 2, 3, 3, 3, 3, 3, 3, 3, 4, 4, 4, 4, 4, 4, 4, 4, 4
+
+NEP_HD float clm(int m) {
+    constexpr float t[kNumLM] = {NEP_CLM_LIST};
+    return t[m];
+}
+
+NEP_HD void sincospi_f(float a, float* s, float* c) {
+#ifdef __CUDA_ARCH__
+    sincospif(a, s, c);
+#else
+    *s = (float)sin(3.14159265358979323846 * (double)a);
+    *c = (float)cos(3.14159265358979323846 * (double)a);
+#endif
+}
+
+// g_n and dg_n/dr for n = 0..N-1 at distance r (r < rc), rcinv = 1/rc, omega = Eq. 19 weight.
+//   x  = 2 (r/rc - 1)^2 - 1,  x' = 4 (r/rc - 1)/rc
+//   fc = 1/2 (1 + cos(pi r/rc)) = cos^2(pi r / 2 rc),   fc' = -(pi/rc) sin(pi r/2rc) cos(pi r/2rc)
+//   g_n  = 1/2 (T_n + 1) fc omega
+//   g_n' = 1/2 [ n U_{n-1} x' fc + (T_n + 1) fc' ] omega                      (Eq. A2)
+template <int N, bool DERIV>
+NEP_HD void radial_fn(float r, float rcinv, float omega, float* g, float* dg) {
+    const float u = r * rcinv;
+    const float um1 = u - 1.f;
+    const float x = fmaf(2.f * um1, um1, -1.f);
+    float sn, cs;
+    sincospi_f(0.5f * u, &sn, &cs);
+    const float hf = 0.5f * omega * cs * cs;                          // omega fc / 2
+    const float hb = -0.5f * omega * 3.14159265358979f * rcinv * sn * cs;   // omega fc' / 2
+    const float ha = hf * 4.f * um1 * rcinv;                          // omega fc x' / 2
+    const float x2 = 2.f * x;
+    float Tm = 1.f, T = x;        // T_{n-1}, T_n
+    float Um = 0.f, U = 1.f;      // U_{n-2}, U_{n-1}
+    g[0] = 2.f * hf;
+    if (DERIV) dg[0] = 2.f * hb;
+#pragma unroll
+    for (int n = 1; n < N; ++n) {
+        g[n] = fmaf(hf, T, hf);
+        if (DERIV) dg[n] = fmaf(ha * (float)n, U, fmaf(hb, T, hb));
+        const float Tn = fmaf(x2, T, -Tm);  Tm = T;  T = Tn;          // Eq. A1
+        const float Un = fmaf(x2, U, -Um);  Um = U;  U = Un;          // Eq. A3
+    }
+}
+
+// b_lm(x,y,z) on the unit sphere.  Order: l=1: x y z | l=2: 20 21c 21s 22c 22s | l=3: 30 31c 31s
+// 32c 32s 33c 33s | l=4: 40 41c 41s 42c 42s 43c 43s 44c 44s.
+NEP_HD void ylm_basis(float x, float y, float z, float* b) {
+    const float z2 = z * z;
+    const float c2 = x * x - y * y, s2 = 2.f * x * y;            // rho^2 cos 2phi, rho^2 sin 2phi
+    const float c3 = x * c2 - y * s2, s3 = x * s2 + y * c2;      // rho^3 cos 3phi, sin 3phi
+    const float t5 = fmaf(5.f, z2, -1.f), t7 = fmaf(7.f, z2, -3.f), u7 = fmaf(7.f, z2, -1.f);
+    b[0] = x; b[1] = y; b[2] = z;
+    b[3] = fmaf(3.f, z2, -1.f); b[4] = x * z; b[5] = y * z; b[6] = c2; b[7] = s2;
+    b[8] = z * fmaf(5.f, z2, -3.f); b[9] = x * t5; b[10] = y * t5; b[11] = z * c2; b[12] = z * s2;
+    b[13] = c3; b[14] = s3;
+    b[15] = fmaf(z2, fmaf(35.f, z2, -30.f), 3.f); b[16] = b[4] * t7; b[17] = b[5] * t7;
+    b[18] = c2 * u7; b[19] = s2 * u7; b[20] = z * c3; b[21] = z * s3;
+    b[22] = c2 * c2 - s2 * s2; b[23] = 2.f * c2 * s2;
+}
+
+// Angular partial force of one neighbour from the per-lm sums
+//   Sp[m] = sum_n A[n][m] g_n'(r),   St[m] = sum_n A[n][m] g_n(r) / r :
+//   p = R r^ + V,   R = sum_m b_m (Sp_m - l_m St_m),   V = sum_m St_m grad B_m(r^).
+NEP_HD void ylm_force(float x, float y, float z, const float* Sp, const float* St, float* px, float* py,
+                      float* pz) {
+    float b[kNumLM];
+    ylm_basis(x, y, z, b);
+    constexpr int lof[kNumLM] = {NEP_LOF_LIST};
+    float R = 0.f;
+#pragma unroll
+    for (int m = 0; m < kNumLM; ++m) R = fmaf(b[m], fmaf(-(float)lof[m], St[m], Sp[m]), R);
+    const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y, xz = x * z, yz = y * z, xyz = xy * z;
+    const float c2 = x2 - y2, c3 = b[13], s3 = b[14];
+    const float rho2 = x2 + y2;
+    const float q4 = rho2 - 4.f * z2;            // x^2 + y^2 - 4 z^2
+    float vx = St[0], vy = St[1], vz = St[2];
+    // l = 2
+    vx = fmaf(St[3], -2.f * x, vx); vy = fmaf(St[3], -2.f * y, vy); vz = fmaf(St[3], 4.f * z, vz);
+    vx = fmaf(St[4], z, vx);                                        vz = fmaf(St[4], x, vz);
+                                    vy = fmaf(St[5], z, vy);        vz = fmaf(St[5], y, vz);
+    vx = fmaf(St[6], 2.f * x, vx);  vy = fmaf(St[6], -2.f * y, vy);
+    vx = fmaf(St[7], 2.f * y, vx);  vy = fmaf(St[7], 2.f * x, vy);
+    // l = 3
+    vx = fmaf(St[8], -6.f * xz, vx); vy = fmaf(St[8], -6.f * yz, vy); vz = fmaf(St[8], -3.f * (rho2 - 2.f * z2), vz);
+    vx = fmaf(St[9], 4.f * z2 - 3.f * x2 - y2, vx); vy = fmaf(St[9], -2.f * xy, vy); vz = fmaf(St[9], 8.f * xz, vz);
+    vx = fmaf(St[10], -2.f * xy, vx); vy = fmaf(St[10], 4.f * z2 - x2 - 3.f * y2, vy); vz = fmaf(St[10], 8.f * yz, vz);
+    vx = fmaf(St[11], 2.f * xz, vx); vy = fmaf(St[11], -2.f * yz, vy); vz = fmaf(St[11], c2, vz);
+    vx = fmaf(St[12], 2.f * yz, vx); vy = fmaf(St[12], 2.f * xz, vy); vz = fmaf(St[12], 2.f * xy, vz);
+    vx = fmaf(St[13], 3.f * c2, vx); vy = fmaf(St[13], -6.f * xy, vy);
+    vx = fmaf(St[14], 6.f * xy, vx); vy = fmaf(St[14], 3.f * c2, vy);
+    // l = 4
+    vx = fmaf(St[15], 12.f * x * q4, vx); vy = fmaf(St[15], 12.f * y * q4, vy);
+    vz = fmaf(St[15], -16.f * z * (3.f * rho2 - 2.f * z2), vz);
+    vx = fmaf(St[16], -z * (9.f * x2 + 3.f * y2 - 4.f * z2), vx); vy = fmaf(St[16], -6.f * xyz, vy);
+    vz = fmaf(St[16], -3.f * x * q4, vz);
+    vx = fmaf(St[17], -6.f * xyz, vx); vy = fmaf(St[17], -z * (3.f * x2 + 9.f * y2 - 4.f * z2), vy);
+    vz = fmaf(St[17], -3.f * y * q4, vz);
+    vx = fmaf(St[18], -4.f * x * (x2 - 3.f * z2), vx); vy = fmaf(St[18], 4.f * y * (y2 - 3.f * z2), vy);
+    vz = fmaf(St[18], 12.f * z * c2, vz);
+    vx = fmaf(St[19], -2.f * y * (3.f * x2 + y2 - 6.f * z2), vx);
+    vy = fmaf(St[19], -2.f * x * (x2 + 3.f * y2 - 6.f * z2), vy); vz = fmaf(St[19], 24.f * xyz, vz);
+    vx = fmaf(St[20], 3.f * z * c2, vx); vy = fmaf(St[20], -6.f * xyz, vy); vz = fmaf(St[20], c3, vz);
+    vx = fmaf(St[21], 6.f * xyz, vx); vy = fmaf(St[21], 3.f * z * c2, vy); vz = fmaf(St[21], s3, vz);
+    vx = fmaf(St[22], 4.f * c3, vx); vy = fmaf(St[22], -4.f * s3, vy);
+    vx = fmaf(St[23], 4.f * s3, vx); vy = fmaf(St[23], 4.f * c3, vy);
+    *px = fmaf(R, x, vx); *py = fmaf(R, y, vy); *pz = fmaf(R, z, vz);
+}
+
+// t = tanh(a), d = 1 - tanh^2(a) = 4 e / (1 + e)^2 with e = exp(-2|a|): no cancellation when |t| -> 1.
+NEP_HD void tanh_sech2(float a, float* t, float* d) {
+    const float e = expf(-2.f * fabsf(a));
+    const float inv = 1.f / (1.f + e);
+    const float tt = (1.f - e) * inv;
+    *t = copysignf(tt, a);
+    *d = 4.f * e * inv * inv;
+}
+
+}  // namespace nepk

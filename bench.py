@@ -1,0 +1,275 @@
+#!/usr/bin/env python
+"""bench.py -- NEP MD atom-steps/s on B200 (BASELINE.json metric), one JSON line on stdout.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4_1048576] [--impl ours|reference]
+
+A "step" is one velocity-Verlet MD step of the whole hot path over the workload: half-kick + drift,
+device-side list rebuild when needed, list filter, descriptor + network + partial forces, assembly
+of F / W / J, second half-kick, per-step thermo sums.  N > 1 runs N independent replicas
+("replicas only"): no data-path collective exists.
+`--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "NEP MD atom-steps/s"
+UNIT = "atom-steps/s"
+# FP32 non-tensor peak: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz max SM clock
+# (unit counts and clock from /opt/skills/guides/B200_PROFILING.md).
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+
+
+def algorithmic_flops_per_atom(n_r, n_a, dim, n_neu, m_r, m_a):
+    """SURVEY.md 8(d) / DESIGN.md section 7: necessary flops of descriptor + network + partial forces
+    per atom-step with the O(M) addition-theorem route (FMA = 2).  k_main covers all but the
+    25*M_R assembly term."""
+    k_desc = m_r * (17 + 5 * n_r) + m_a * (67 + 52 * n_a) + 48 * n_a
+    k_nn = 4 * dim * n_neu
+    k_force = 48 * n_a + m_r * (20 + 10 * n_r) + m_a * (370 + 104 * n_a)
+    return k_desc + k_nn + k_force
+
+
+def make_workload(name):
+    from paper_2107_08119_b200 import inputs
+    if name.startswith("c4_"):
+        return inputs.config4(int(name[3:]))
+    return {"c0": inputs.config0, "c1": inputs.config1, "c2": inputs.config2, "c3": inputs.config3}[name]()
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.proc = index, [], None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([c.strip() for c in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm, reasons, smax = [], set(), None
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); smax = float(r[1])
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def run_reference(args):
+    """The oracle as it stands, on the host cores, on a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    from paper_2107_08119_b200 import inputs
+    w = inputs.si_cells((12, 12, 12))           # 13824 atoms of the C4 lattice, C4 seeds, C0 weights
+    h = oracle.Hyper(w.rc_r, w.rc_a, w.n_max_r, w.n_max_a, w.l_max, w.n_neurons, 1)
+    ev = lambda: oracle.evaluate(h, w.atomic_numbers, w.params, w.pos, w.vel, w.types, w.box)
+    for _ in range(min(args.warmup, 1)):
+        ev()
+    steps = max(1, min(args.steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        ev()
+    dt = time.perf_counter() - t0
+    value = w.n_atoms * steps / dt
+    sample = "%d-atom replica of the C4 Si lattice (12^3 cells), %d full evaluations of U,F,W,J" % (w.n_atoms, steps)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4_1048576")
+    ap.add_argument("--skin", type=float, default=1.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2107_08119_b200 import api
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K, Wm = args.steps, max(args.warmup, 3)
+    w = make_workload(args.workload)
+    N = w.n_atoms
+    cap_r, cap_a = (64, 32) if len(w.atomic_numbers) == 1 else (80, 40)
+    model, system, pos, vel = api.from_workload(w, cap_r, cap_a, args.skin, dev)
+    out = system.alloc_outputs()
+    heat_sum = torch.zeros((3, N), dtype=torch.float64, device=dev)
+    thermo = torch.zeros((max(K, Wm), 5), dtype=torch.float64, device=dev)
+    system.neighbors(pos, w.box)
+    cnt_r, _ = system.get_neighbors(0)
+    cnt_a, _ = system.get_neighbors(1)
+    m_r0, m_a0 = cnt_r.float().mean().item(), cnt_a.float().mean().item()
+
+    # ---- warm-up, then the timed region: K steps, device-timed on the launching stream ----
+    system.md_step(pos, vel, w.masses, w.dt, Wm, out, heat_sum, thermo)
+    system.status()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    l0 = system.launch_count()
+    e0.record()
+    system.md_step(pos, vel, w.masses, w.dt, K, out, heat_sum, thermo)
+    e1.record()
+    barrier()
+    launches = system.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    system.status()
+    st = system.stats()
+    th = thermo[:K].cpu().numpy()
+    e_tot = th[:, 0] + th[:, 1]
+    if world > 1:
+        t = torch.tensor([ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = t.item()
+    value = world * N * K / (ms * 1e-3)
+
+    # ---- per-kernel device timing (same launch sequence, CUDA events inside the library) ----
+    kp = min(K, 100)
+    system.profile(True)
+    system.md_step(pos, vel, w.masses, w.dt, kp, out, heat_sum, thermo)
+    prof = system.get_profile()
+    system.profile(False)
+    cnt_r, _ = system.get_neighbors(0)
+    cnt_a, _ = system.get_neighbors(1)
+    m_r, m_a = cnt_r.float().mean().item(), cnt_a.float().mean().item()
+    main_ms = prof["main"]["ms"] / max(1, prof["main"]["count"])
+    flops_atom = algorithmic_flops_per_atom(w.n_max_r + 1, w.n_max_a + 1, w.dim, w.n_neurons, 0.5 * (m_r0 + m_r), 0.5 * (m_a0 + m_a))
+    achieved = flops_atom * N / (main_ms * 1e-3) / 1e12
+    phase_ms = {k: v["ms"] / kp for k, v in prof.items()}
+    tot_phase = sum(phase_ms.values())
+
+    # ---- end to end through the C ABI with HOST buffers: per step H2D(pos, vel) + one MD step + D2H ----
+    ke = min(K, 50)
+    h_pos = pos.cpu().pin_memory(); h_vel = vel.cpu().pin_memory()
+    h_out = [torch.empty_like(t, device="cpu").pin_memory() for t in out]
+    system.md_step(pos, vel, w.masses, w.dt, 1, out)          # warm the 1-step path
+    barrier()
+    t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for _ in range(ke):
+        pos.copy_(h_pos, non_blocking=True); vel.copy_(h_vel, non_blocking=True)
+        system.md_step(pos, vel, w.masses, w.dt, 1, out)
+        h_pos.copy_(pos, non_blocking=True); h_vel.copy_(vel, non_blocking=True)
+        for hd, dd in zip(h_out, out):
+            hd.copy_(dd, non_blocking=True)
+        torch.cuda.current_stream().synchronize()              # the host reads the step's result
+    t1.record()
+    barrier()
+    e2e_ms = t0.elapsed_time(t1)
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = t.item()
+    h2d = 2 * 3 * N * 8
+    d2h = 2 * 3 * N * 8 + sum(t.numel() * 4 for t in out)
+    system.status()
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        from paper_2107_08119_b200 import inputs
+        ws = inputs.si_cells((12, 12, 12))
+        h = oracle.Hyper(ws.rc_r, ws.rc_a, ws.n_max_r, ws.n_max_a, ws.l_max, ws.n_neurons, 1)
+        tt = time.perf_counter()
+        reps = 2
+        for _ in range(reps):
+            oracle.evaluate(h, ws.atomic_numbers, ws.params, ws.pos, ws.vel, ws.types, ws.box)
+        tt = time.perf_counter() - tt
+        cpu = {"value": ws.n_atoms * reps / tt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": "%d-atom replica of the C4 Si lattice (12^3 cells), %d full fp64 evaluations of U,F,W,J "
+                         "(O(M^2) literal Eq. 13/25), %.1f s" % (ws.n_atoms, reps, tt)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "%s: %d-atom diamond Si (C4), D=%d NN %d-%d-1, rc %.1f/%.1f A, NVE dt=%g fs, W and J every step"
+                                   % (args.workload, N, w.dim, w.dim, w.n_neurons, w.rc_r, w.rc_a, w.dt)
+                       if args.workload.startswith("c4") else args.workload,
+                       "n_atoms": N, "parallelism": "replicas x%d" % world, "skin": args.skin,
+                       "l2": "working set %.1f GB per replica >> 126 MB L2, no flush needed" % (system.workspace.numel() / 1e9),
+                       "mean_M_R": [m_r0, m_r], "mean_M_A": [m_a0, m_a], "rebuilds_total": st["rebuilds"],
+                       "max_M_R": st["max_radial"], "max_M_A": st["max_angular"],
+                       "energy_drift_eV_per_atom": float(np.abs(e_tot - e_tot[0]).max() / N)},
+            "clocks": clocks,
+            "e2e": {"value": world * N * ke / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "steps": ke,
+                    "what": "per step: pinned-host pos+vel -> device, nep_md_step(1), pos+vel+U+F+W+J -> pinned host"},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "alu", "kernel": "k_main (descriptor + network + partial forces)",
+                         "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
+                         "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (no FP32 figure in MEASURED_PEAKS.json)",
+                         "flops_per_atom": flops_atom, "kernel_ms": main_ms, "kernel_share_of_step": phase_ms["main"] / tot_phase,
+                         "traffic": None},
+            "phase_ms_per_step": phase_ms,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

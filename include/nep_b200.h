@@ -112,7 +112,10 @@ int  nep_compute(nep_system*, const double* pos_dev, const double* vel_dev, floa
 /* n_steps velocity-Verlet NVE steps (BASELINE.json north_star; the paper's own timing used NVT,
  * PAPER.md:395):  v += dt/2 F/m;  r += dt v;  [rebuild lists on device when an atom moved > skin/2];
  * evaluate;  v += dt/2 F/m;  J_i = W_i . v_i (Eq. 7, both at t+dt).  a = F / (m * 103.642697) A/fs^2.
- * Requires nep_neighbors at the current positions first; the first call evaluates F(t0) itself.
+ * Requires nep_neighbors at the current positions first.  The first nep_md_step after nep_neighbors /
+ * nep_compute evaluates F(t0) itself; a nep_md_step that directly follows another nep_md_step on the
+ * same system CONTINUES the trajectory from the forces of that call: the caller must pass back the
+ * positions it returned (velocities may be changed, e.g. rescaled).  Call nep_neighbors to restart.
  *   pos_dev, vel_dev [3][N] fp64: updated in place (positions are not wrapped).
  *   mass_by_type [n_types] host, amu.
  *   energy/force/virial/heat_dev: state after the last step (virial/heat nullable).
@@ -131,6 +134,18 @@ int  nep_status(nep_system*);
  * out[0] = list rebuilds, out[1] = max radial count seen, out[2] = max angular count seen,
  * out[3] = max Verlet-list count seen. */
 int  nep_stats(nep_system*, int64_t out[4]);
+
+/* Number of CUDA kernels this system has launched since nep_system_create (host counter). */
+int64_t nep_launch_count(const nep_system*);
+
+/* Per-phase device timing with CUDA events on the launching stream (for bench.py's roofline entry).
+ * nep_profile(s, 1) resets and enables it (adds one event record per phase; at most 2048 events between
+ * two nep_get_profile calls, further phases go untimed), nep_profile(s, 0) disables it.
+ * nep_get_profile synchronises and returns accumulated milliseconds and launch-group counts for the
+ * phases 0 kick+drift, 1 neighbour build (gated), 2 list filter, 3 descriptor+network+partial forces
+ * (k_main), 4 assembly, 5 state load/store; entries 6-7 are reserved (0). */
+int  nep_profile(nep_system*, int enable);
+int  nep_get_profile(nep_system*, double ms[8], int64_t count[8]);
 
 const char* nep_strerror(int code);
 

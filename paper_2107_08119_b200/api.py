@@ -16,7 +16,8 @@ _lib = None
 
 SYMBOLS = ["nep_create", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",
            "nep_system_create", "nep_system_destroy", "nep_neighbors", "nep_get_neighbors", "nep_compute",
-           "nep_md_step", "nep_status", "nep_stats", "nep_strerror"]
+           "nep_md_step", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile",
+           "nep_strerror"]
 
 
 class NepError(RuntimeError):
@@ -54,6 +55,10 @@ def lib():
         for f in ("nep_descriptor_dim", "nep_num_params", "nep_status"):
             getattr(L, f).argtypes = [C.c_void_p]
         L.nep_stats.argtypes = [C.c_void_p, C.c_void_p]
+        L.nep_launch_count.argtypes = [C.c_void_p]
+        L.nep_launch_count.restype = C.c_int64
+        L.nep_profile.argtypes = [C.c_void_p, C.c_int]
+        L.nep_get_profile.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -155,6 +160,19 @@ class System:
         out = (C.c_int64 * 4)()
         _check(lib().nep_stats(self._h, C.cast(out, C.c_void_p)), "nep_stats")
         return dict(rebuilds=out[0], max_radial=out[1], max_angular=out[2], max_verlet=out[3])
+
+    PHASES = ("kick_drift", "build", "filter", "main", "assemble", "state")
+
+    def launch_count(self):
+        return lib().nep_launch_count(self._h)
+
+    def profile(self, enable: bool):
+        _check(lib().nep_profile(self._h, int(enable)), "nep_profile")
+
+    def get_profile(self):
+        ms = (C.c_double * 8)(); cnt = (C.c_int64 * 8)()
+        _check(lib().nep_get_profile(self._h, C.cast(ms, C.c_void_p), C.cast(cnt, C.c_void_p)), "nep_get_profile")
+        return {name: dict(ms=ms[k], count=cnt[k]) for k, name in enumerate(self.PHASES)}
 
     def __del__(self):
         if getattr(self, "_h", None) and self._h.value and _lib is not None:

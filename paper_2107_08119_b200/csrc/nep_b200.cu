@@ -67,6 +67,9 @@ inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 }  // namespace
 
+constexpr int kProfMaxEvents = 2048;
+enum { PH_KICK = 0, PH_BUILD = 1, PH_FILTER = 2, PH_MAIN = 3, PH_ASSEMBLE = 4, PH_STATE = 5, NEP_PHASES = 8 };
+
 struct nep_model {
     nep_hyper h;
     int D, Dp, NR, NA, H, npar;
@@ -91,6 +94,14 @@ struct nep_system {
     double g_dt;
     double g_mass[kMaxTypes];
     int64_t host_stats[4];
+    int64_t launches;                      // kernels launched since creation
+    // optional per-phase event timing (nep_profile)
+    bool prof_on;
+    int prof_n;                            // events recorded
+    cudaEvent_t prof_ev[kProfMaxEvents];
+    int prof_phase[kProfMaxEvents];        // phase that STARTS at event k (-1: end marker)
+    double prof_ms[NEP_PHASES];
+    int64_t prof_cnt[NEP_PHASES];
 };
 
 namespace {
@@ -766,6 +777,8 @@ int max_cells_of(int64_t N) { return (int)(2 * N + 64); }
 int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
 int grid_stride(int64_t n) { int g = grid_for(n, 256); return g > 148 * 8 ? 148 * 8 : (g < 1 ? 1 : g); }
 
+constexpr int kBuildLaunches = 10;
+
 // the neighbour build as a fixed launch sequence; gated != 0: every kernel exits unless F_REBUILD is set
 void launch_build(nep_system* s, const double* xin, const double* vin, int first, int gated, cudaStream_t st) {
     const int N = (int)s->N;
@@ -782,8 +795,8 @@ void launch_build(nep_system* s, const double* xin, const double* vin, int first
     k_build_md<<<grid_for(N, 128), 128, 0, st>>>(d, N, b, rc * rc, s->capMD, gated);
     k_rev<<<grid_for(N, 128), 128, 0, st>>>(d, N, gated);
     k_build_done<<<1, 1, 0, st>>>(d, gated);
+    s->launches += kBuildLaunches;
 }
-constexpr int kBuildLaunches = 10;
 
 template <int NR, int NA, bool MULTI>
 void launch_main_t(nep_system* s, cudaStream_t st) {
@@ -798,6 +811,7 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
         attr_done = true;
     }
     k_main<NR, NA, MULTI><<<grid_for(2 * s->N, 128), 128, smem, st>>>(s->d, P, m->params_dev, m->sqrtzz_dev);
+    s->launches += 1;
 }
 
 bool main_supported(const nep_model* m) {
@@ -815,6 +829,7 @@ void launch_filter(nep_system* s, cudaStream_t st) {
     const nep_hyper& h = s->model->h;
     k_filter<<<grid_for(s->N, 128), 128, 0, st>>>(s->d, (int)s->N, s->box, h.rc_radial * h.rc_radial,
                                                  h.rc_angular * h.rc_angular, s->capR, s->capA, s->capMD);
+    s->launches += 1;
 }
 
 void fill_masses(AsmParams* P, const nep_model* m, const double* mass_by_type) {
@@ -823,6 +838,25 @@ void fill_masses(AsmParams* P, const nep_model* m, const double* mass_by_type) {
         P->inv_mass[t] = 1.0 / (mm * kAmuConv);
         P->ke_mass[t] = 0.5 * mm * kAmuConv;
     }
+}
+
+// marks the start of a phase on the stream (only when nep_profile is on)
+void phase(nep_system* s, int ph, cudaStream_t st) {
+    if (!s->prof_on || s->prof_n >= kProfMaxEvents) return;
+    cudaEventRecord(s->prof_ev[s->prof_n], st);
+    s->prof_phase[s->prof_n++] = ph;
+}
+
+void prof_resolve(nep_system* s) {
+    for (int k = 0; k + 1 < s->prof_n; ++k) {
+        if (s->prof_phase[k] < 0) continue;
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, s->prof_ev[k], s->prof_ev[k + 1]) == cudaSuccess) {
+            s->prof_ms[s->prof_phase[k]] += ms;
+            s->prof_cnt[s->prof_phase[k]] += 1;
+        }
+    }
+    s->prof_n = 0;
 }
 
 bool device_ok() {
@@ -918,6 +952,9 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
     s->max_cells = max_cells_of(n_atoms);
     carve(n_atoms, s->capR, s->capMD, s->max_cells, &s->d, (char*)workspace_dev);
     s->built = false; s->have_forces = false; s->last_stream = nullptr; s->step_graph = nullptr;
+    s->launches = 0; s->prof_on = false; s->prof_n = 0;
+    for (int k = 0; k < NEP_PHASES; ++k) { s->prof_ms[k] = 0.0; s->prof_cnt[k] = 0; }
+    for (int k = 0; k < kProfMaxEvents; ++k) s->prof_ev[k] = nullptr;
     cudaError_t e = cudaMemset(workspace_dev, 0, need);
     if (e == cudaSuccess) e = cudaMemcpy(s->d.type_in, type_dev, (size_t)n_atoms * sizeof(int), cudaMemcpyDeviceToDevice);
     if (e != cudaSuccess) { set_cuda_error(e, "nep_system_create"); delete s; return NEP_ECUDA; }
@@ -928,6 +965,7 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
 void nep_system_destroy(nep_system* s) {
     if (!s) return;
     if (s->step_graph) cudaGraphExecDestroy(s->step_graph);
+    for (int k = 0; k < kProfMaxEvents; ++k) if (s->prof_ev[k]) cudaEventDestroy(s->prof_ev[k]);
     delete s;
 }
 
@@ -949,8 +987,11 @@ int nep_neighbors(nep_system* s, const double* pos_dev, const double box[3], voi
     b.ncell = b.nc[0] * b.nc[1] * b.nc[2];
     s->box = b;
     s->last_stream = st;
+    phase(s, PH_BUILD, st);
     launch_build(s, pos_dev, nullptr, 1, 0, st);
+    phase(s, PH_FILTER, st);
     launch_filter(s, st);
+    phase(s, -1, st);
     NEP_CUDA_OK(cudaGetLastError());
     s->built = true; s->have_forces = false;
     return NEP_OK;
@@ -963,6 +1004,7 @@ int nep_get_neighbors(nep_system* s, int which, int* count_dev, int* index_dev, 
     s->last_stream = st;
     k_export_lists<<<grid_for(s->N, 128), 128, 0, st>>>(s->d, (int)s->N, which, s->capR, which ? s->capA : s->capR,
                                                        count_dev, index_dev);
+    s->launches += 1;
     NEP_CUDA_OK(cudaGetLastError());
     return NEP_OK;
 }
@@ -975,8 +1017,11 @@ int nep_compute(nep_system* s, const double* pos_dev, const double* vel_dev, flo
     s->last_stream = st;
     const int N = (int)s->N;
     const double hs = 0.5 * s->skin;
+    phase(s, PH_STATE, st);
     k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, nullptr, hs * hs * (1.0 + 1e-12) + 1e-24, 0);
+    phase(s, PH_FILTER, st);
     launch_filter(s, st);
+    phase(s, PH_MAIN, st);
     launch_main(s, st);
     AsmParams P;
     memset(&P, 0, sizeof(P));
@@ -984,7 +1029,10 @@ int nep_compute(nep_system* s, const double* pos_dev, const double* vel_dev, flo
     fill_masses(&P, s->model, nullptr);
     P.vel_in = vel_dev; P.energy = energy_dev; P.force = force_dev; P.virial = virial_dev;
     P.heat = vel_dev ? heat_dev : nullptr;
+    phase(s, PH_ASSEMBLE, st);
     k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
+    phase(s, -1, st);
+    s->launches += 2;
     NEP_CUDA_OK(cudaGetLastError());
     s->have_forces = false;
     return NEP_OK;
@@ -1009,23 +1057,42 @@ int nep_md_step(nep_system* s, double* pos_dev, double* vel_dev, const double* m
     P.energy = energy_dev; P.force = force_dev; P.virial = virial_dev; P.heat = heat_dev;
     P.heat_sum = heat_sum_dev; P.thermo = thermo_dev;
     if (thermo_dev && n_steps > 0) NEP_CUDA_OK(cudaMemsetAsync(thermo_dev, 0, (size_t)n_steps * 5 * sizeof(double), st));
-    // caller arrays -> sorted state; F(t0)
+    // caller arrays -> sorted state
+    phase(s, PH_STATE, st);
     k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, vel_dev, hs2, 1);
-    launch_build(s, s->d.xs, s->d.vs, 0, 1, st);
-    launch_filter(s, st);
-    launch_main(s, st);
-    P.md = 2;
-    k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
+    s->launches += 1;
+    if (!s->have_forces) {       // F(t0); a call that directly follows nep_md_step continues from its forces
+        phase(s, PH_BUILD, st);
+        launch_build(s, s->d.xs, s->d.vs, 0, 1, st);
+        phase(s, PH_FILTER, st);
+        launch_filter(s, st);
+        phase(s, PH_MAIN, st);
+        launch_main(s, st);
+        P.md = 2;
+        phase(s, PH_ASSEMBLE, st);
+        k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
+        s->launches += 1;
+    }
     P.md = 1;
     for (int step = 0; step < n_steps; ++step) {
+        phase(s, PH_KICK, st);
         k_kick_drift<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, dt_fs, hs2, P);
+        phase(s, PH_BUILD, st);
         launch_build(s, s->d.xs, s->d.vs, 0, 1, st);
+        phase(s, PH_FILTER, st);
         launch_filter(s, st);
+        phase(s, PH_MAIN, st);
         launch_main(s, st);
+        phase(s, PH_ASSEMBLE, st);
         k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
+        s->launches += 2;
     }
+    phase(s, PH_STATE, st);
     k_store_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, vel_dev);
+    phase(s, -1, st);
+    s->launches += 1;
     NEP_CUDA_OK(cudaGetLastError());
+    s->have_forces = true;
     return NEP_OK;
 }
 
@@ -1048,6 +1115,28 @@ int nep_stats(nep_system* s, int64_t out[4]) {
     int flags[F_COUNT];
     NEP_CUDA_OK(cudaMemcpy(flags, s->d.flags, sizeof(flags), cudaMemcpyDeviceToHost));
     out[0] = flags[F_NREBUILD]; out[1] = flags[F_MAXR]; out[2] = flags[F_MAXA]; out[3] = flags[F_MAXMD];
+    return NEP_OK;
+}
+
+int64_t nep_launch_count(const nep_system* s) { return s ? s->launches : 0; }
+
+int nep_profile(nep_system* s, int enable) {
+    if (!s) return NEP_EINVAL;
+    NEP_CUDA_OK(cudaStreamSynchronize(s->last_stream));
+    s->prof_n = 0;
+    for (int k = 0; k < NEP_PHASES; ++k) { s->prof_ms[k] = 0.0; s->prof_cnt[k] = 0; }
+    if (enable)
+        for (int k = 0; k < kProfMaxEvents; ++k)
+            if (!s->prof_ev[k]) NEP_CUDA_OK(cudaEventCreate(&s->prof_ev[k]));
+    s->prof_on = enable != 0;
+    return NEP_OK;
+}
+
+int nep_get_profile(nep_system* s, double ms[8], int64_t count[8]) {
+    if (!s || !ms || !count) return NEP_EINVAL;
+    NEP_CUDA_OK(cudaStreamSynchronize(s->last_stream));
+    prof_resolve(s);
+    for (int k = 0; k < NEP_PHASES; ++k) { ms[k] = s->prof_ms[k]; count[k] = s->prof_cnt[k]; }
     return NEP_OK;
 }
 

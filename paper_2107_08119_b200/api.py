@@ -11,7 +11,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libnep_b200.so")
+_LIB_PATH = os.environ.get("NEP_B200_LIB", os.path.join(_HERE, "libnep_b200.so"))   # override: kernel experiments
 _lib = None
 
 SYMBOLS = ["nep_create", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",

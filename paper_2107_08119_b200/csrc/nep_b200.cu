@@ -48,6 +48,7 @@ struct SysDev {                 // device pointers into the caller's workspace
     int* cell_fill;             // [max_cells]
     int* type_s;                // [N] sorted
     double* xs;                 // [3][N] sorted positions (unwrapped)
+    double4* xs4;               // [N] the same as {x, y, z, bits(type)}: one 32-B sector per gathered neighbour
     double* vs;                 // [3][N] sorted velocities
     double* xref;               // [3][N] sorted positions at the last build
     double* tmp3;               // [3][N]
@@ -58,9 +59,10 @@ struct SysDev {                 // device pointers into the caller's workspace
     int* md_idx;                // [cap_md][N]  j | rev << 24
     int* nnR;                   // [N]
     int* nnA;                   // [N]
-    float4* rec;                // [cap_R][N]  {dx, dy, dz, bits(j | type_j << 24)}
-    unsigned short* slots;      // [cap_R][N]  md_slot | rev << 8
-    float4* p;                  // [N][cap_md] partial forces dU_i/dr_ij at Verlet slots
+    float4* rec;                // [cap_R][N]  {dx, dy, dz, bits(md_slot | type_j << 8)}   (read by k_main)
+    int* jrev;                  // [cap_R][N]  j | rev << 24                               (read by k_assemble)
+    uint4* masks;               // [N][2] bit s set: Verlet slot s is inside r_c^R ([0]) / r_c^A ([1])
+    float4* p;                  // [N][cap_R] partial forces dU_i/dr_ij at the record slots
 };
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -213,7 +215,9 @@ __global__ void k_gather_b(SysDev d, int N, int have_v, int gated) {
         }
         const int p = d.cell_of[k];
         d.perm[k] = p;
-        d.type_s[k] = d.type_in[p];
+        const int ty = d.type_in[p];
+        d.type_s[k] = ty;
+        d.xs4[k] = make_double4(d.xref[k], d.xref[N + k], d.xref[2 * N + k], __longlong_as_double((long long)ty));
     }
 }
 
@@ -246,9 +250,10 @@ __global__ void __launch_bounds__(128) k_build_md(SysDev d, int N, Box b, double
         const int lo = d.cell_start[cells[q]], hi = d.cell_start[cells[q] + 1];
         for (int j = lo; j < hi; ++j) {
             if (j == i) continue;
-            const double dx = min_image(d.xs[j] - xi, b.L[0], b.invL[0]);
-            const double dy = min_image(d.xs[N + j] - yi, b.L[1], b.invL[1]);
-            const double dz = min_image(d.xs[2 * N + j] - zi, b.L[2], b.invL[2]);
+            const double4 pj = d.xs4[j];
+            const double dx = min_image(pj.x - xi, b.L[0], b.invL[0]);
+            const double dy = min_image(pj.y - yi, b.L[1], b.invL[1]);
+            const double dz = min_image(pj.z - zi, b.L[2], b.invL[2]);
             const double r2 = dx * dx + dy * dy + dz * dz;
             if (r2 < rc2) {
                 if (cnt < capMD) d.md_idx[(size_t)cnt * N + i] = j;
@@ -298,25 +303,44 @@ __global__ void __launch_bounds__(128) k_filter(SysDev d, int N, Box b, double r
                                                 int capMD) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
-    const double xi = d.xs[i], yi = d.xs[N + i], zi = d.xs[2 * N + i];
+    const double4 pi = d.xs4[i];
     const int cnt = d.md_cnt[i];
     int nA = 0, nO = 0;
-    for (int s = 0; s < cnt; ++s) {
-        const int e = d.md_idx[(size_t)s * N + i];
-        const int j = e & kJMask;
-        const double dx = min_image(d.xs[j] - xi, b.L[0], b.invL[0]);
-        const double dy = min_image(d.xs[N + j] - yi, b.L[1], b.invL[1]);
-        const double dz = min_image(d.xs[2 * N + j] - zi, b.L[2], b.invL[2]);
-        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-        if (r2 < rcR2) {
-            const bool ang = r2 < rcA2;
-            if (nA + nO < capR) {
-                const int slot = ang ? nA : capR - 1 - nO;
-                const int w = j | (d.type_s[j] << 24);
-                d.rec[(size_t)slot * N + i] = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(w));
-                d.slots[(size_t)slot * N + i] = (unsigned short)(s | ((e >> 24) << 8));
+    unsigned mR[4] = {0u, 0u, 0u, 0u}, mA[4] = {0u, 0u, 0u, 0u};
+    constexpr int B = 8;                 // batch: B list entries, then B position gathers, in flight together
+    for (int s0 = 0; s0 < cnt; s0 += B) {
+        int eb[B];
+        double4 pb[B];
+#pragma unroll
+        for (int u = 0; u < B; ++u) eb[u] = s0 + u < cnt ? d.md_idx[(size_t)(s0 + u) * N + i] : i;
+#pragma unroll
+        for (int u = 0; u < B; ++u) pb[u] = d.xs4[eb[u] & kJMask];
+#pragma unroll
+        for (int u = 0; u < B; ++u) {
+            const int s = s0 + u;
+            if (s >= cnt) break;
+            const int e = eb[u];
+            const double4 pj = pb[u];
+            const double dx = min_image(pj.x - pi.x, b.L[0], b.invL[0]);
+            const double dy = min_image(pj.y - pi.y, b.L[1], b.invL[1]);
+            const double dz = min_image(pj.z - pi.z, b.L[2], b.invL[2]);
+            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            if (r2 < rcR2) {
+                const bool ang = r2 < rcA2;
+                if (nA + nO < capR) {
+                    const int slot = ang ? nA : capR - 1 - nO;
+                    const int ty = (int)__double_as_longlong(pj.w);
+                    d.rec[(size_t)slot * N + i] = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(ty));
+                    d.jrev[(size_t)slot * N + i] = e;
+                }
+#pragma unroll
+                for (int wq = 0; wq < 4; ++wq) {
+                    const unsigned bit = (s >> 5) == wq ? 1u << (s & 31) : 0u;
+                    mR[wq] |= bit;
+                    if (ang) mA[wq] |= bit;
+                }
+                if (ang) ++nA; else ++nO;
             }
-            if (ang) ++nA; else ++nO;
         }
     }
     const int nR = nA + nO;
@@ -324,15 +348,17 @@ __global__ void __launch_bounds__(128) k_filter(SysDev d, int N, Box b, double r
     d.nnA[i] = over ? 0 : nA;          // an overflowing atom is dropped (and reported), never truncated
     d.nnR[i] = over ? 0 : nR;
     if (over) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
+    d.masks[2 * (size_t)i] = make_uint4(mR[0], mR[1], mR[2], mR[3]);
+    d.masks[2 * (size_t)i + 1] = make_uint4(mA[0], mA[1], mA[2], mA[3]);
     // warp-aggregated statistics
-    int mR = nR, mA = nA;
+    int xR = nR, xA = nA;
     for (int o = 16; o > 0; o >>= 1) {
-        mR = max(mR, __shfl_xor_sync(0xffffffffu, mR, o));
-        mA = max(mA, __shfl_xor_sync(0xffffffffu, mA, o));
+        xR = max(xR, __shfl_xor_sync(0xffffffffu, xR, o));
+        xA = max(xA, __shfl_xor_sync(0xffffffffu, xA, o));
     }
     if ((threadIdx.x & 31) == 0) {
-        if (mR > d.flags[F_MAXR]) atomicMax(&d.flags[F_MAXR], mR);
-        if (mA > d.flags[F_MAXA]) atomicMax(&d.flags[F_MAXA], mA);
+        if (xR > d.flags[F_MAXR]) atomicMax(&d.flags[F_MAXR], xR);
+        if (xA > d.flags[F_MAXA]) atomicMax(&d.flags[F_MAXA], xA);
     }
 }
 
@@ -348,229 +374,16 @@ __global__ void k_export_lists(SysDev d, int N, int which, int capR, int cap_out
         int v = -1;
         if (k < n) {
             const int slot = k < nA ? k : capR - 1 - (k - nA);
-            v = d.perm[__float_as_int(d.rec[(size_t)slot * N + i].w) & kJMask];
+            v = d.perm[d.jrev[(size_t)slot * N + i] & kJMask];
         }
         index[(size_t)row * cap_out + k] = v;
     }
 }
 
-// ------------------------------------------------------------------------------------------------
-// descriptor + network + partial forces, two lanes per atom
-// ------------------------------------------------------------------------------------------------
-struct MainParams {
-    float rcR_inv, rcA_inv;
-    int H, N, capR, capMD;
-};
-
-// Lane h of an atom's pair owns the angular radial indices n = h*NH .. h*NH+NH-1 (all 24 lm of each),
-// so both lanes run the same instruction stream; q and the per-neighbour partial force cross the pair
-// with __shfl_xor.  The network is evaluated by both lanes (weights are warp-uniform smem broadcasts).
-template <int NR, int NA, bool MULTI>
-__global__ void __launch_bounds__(128) k_main(SysDev d, MainParams P, const float* __restrict__ params,
-                                              const float* __restrict__ sqrtzz) {
-    constexpr int NH = (NA + 1) / 2;
-    constexpr int D = NR + 4 * NA;
-    constexpr int Dp = (D + 3) & ~3;
-    constexpr float C[kNumLM] = {NEP_CLM_LIST};
-    constexpr int LOF[kNumLM] = {NEP_LOF_LIST};
-    extern __shared__ __align__(16) float sm[];
-    const int H = P.H, N = P.N;
-    const int nfl = H * Dp + 2 * H + 1;
-    float* szz = sm + ((nfl + 3) & ~3);
-    for (int k = threadIdx.x; k < nfl; k += blockDim.x) sm[k] = params[k];
-    if (MULTI) for (int k = threadIdx.x; k < kMaxTypes * kMaxTypes; k += blockDim.x) szz[k] = sqrtzz[k];
-    __syncthreads();
-
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool active = (t >> 1) < N;
-    const int i = active ? (t >> 1) : N - 1;
-    const int h = t & 1;
-    const unsigned FULL = 3u << (threadIdx.x & 30);   // the atom's lane pair (loop trip counts differ across pairs)
-    const int nR = d.nnR[i], nA = d.nnA[i];
-    const float* zrow = MULTI ? szz + d.type_s[i] * kMaxTypes : nullptr;
-    const float4* rec = d.rec + i;
-    auto slot_of = [&](int k) { return k < nA ? k : P.capR - 1 - (k - nA); };
-
-    // ---- radial descriptor, Eq. 12: neighbours split between the two lanes ----
-    float q[Dp];
-#pragma unroll
-    for (int v = 0; v < Dp; ++v) q[v] = 0.f;
-    for (int k = h; k < nR; k += 2) {
-        const float4 e = rec[(size_t)slot_of(k) * N];
-        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
-        float rinv = rsqrtf(r2);
-        rinv = rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);
-        const float om = MULTI ? zrow[(__float_as_int(e.w) >> 24) & 7] : 1.f;
-        float g[NR];
-        radial_fn<NR, false>(r2 * rinv, P.rcR_inv, om, g, nullptr);
-#pragma unroll
-        for (int n = 0; n < NR; ++n) q[n] += g[n];
-    }
-#pragma unroll
-    for (int n = 0; n < NR; ++n) q[n] += __shfl_xor_sync(FULL, q[n], 1);
-
-    // ---- angular sums s[n][lm] = sum_j g_n(r_ij) b_lm(r^_ij)  (Eq. 18 in real form) ----
-    float s[NH][kNumLM];
-#pragma unroll
-    for (int k = 0; k < NH; ++k)
-#pragma unroll
-        for (int m = 0; m < kNumLM; ++m) s[k][m] = 0.f;
-    for (int k = 0; k < nA; ++k) {
-        const float4 e = rec[(size_t)k * N];
-        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
-        float rinv = rsqrtf(r2);
-        rinv = rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);
-        const float om = MULTI ? zrow[(__float_as_int(e.w) >> 24) & 7] : 1.f;
-        float g[NA];
-        radial_fn<NA, false>(r2 * rinv, P.rcA_inv, om, g, nullptr);
-        float go[NH];
-#pragma unroll
-        for (int a = 0; a < NH; ++a) go[a] = h ? (a + NH < NA ? g[a + NH < NA ? a + NH : 0] : 0.f) : g[a];
-        float b[kNumLM];
-        ylm_basis(e.x * rinv, e.y * rinv, e.z * rinv, b);
-#pragma unroll
-        for (int a = 0; a < NH; ++a)
-#pragma unroll
-            for (int m = 0; m < kNumLM; ++m) s[a][m] = fmaf(go[a], b[m], s[a][m]);
-    }
-
-    // ---- q_nl = sum_m C_lm s_nlm^2 (Eq. 17 with n' = n), exchanged across the pair ----
-    {
-        float qa[NH][4];
-#pragma unroll
-        for (int a = 0; a < NH; ++a) {
-#pragma unroll
-            for (int l = 0; l < 4; ++l) qa[a][l] = 0.f;
-#pragma unroll
-            for (int m = 0; m < kNumLM; ++m) qa[a][LOF[m] - 1] = fmaf(C[m] * s[a][m], s[a][m], qa[a][LOF[m] - 1]);
-        }
-#pragma unroll
-        for (int a = 0; a < NH; ++a)
-#pragma unroll
-            for (int l = 0; l < 4; ++l) {
-                const float mine = qa[a][l];
-                const float other = __shfl_xor_sync(FULL, mine, 1);
-                q[NR + 4 * a + l] = h ? other : mine;                       // n = a       (lane 0's)
-                if (a + NH < NA) q[NR + 4 * (a + NH) + l] = h ? mine : other;   // n = a + NH  (lane 1's)
-            }
-    }
-
-    // ---- network Eq. 21-22 and Fp = dU/dq; two neurons per iteration for ILP ----
-    float Fp[Dp];
-#pragma unroll
-    for (int v = 0; v < Dp; ++v) Fp[v] = 0.f;
-    const float* b1 = sm + H * Dp;
-    const float* w2 = b1 + H;
-    float U = -w2[H];                                                    // - b2
-    for (int mu = 0; mu < H; mu += 2) {
-        const bool two = mu + 1 < H;
-        const float4* r0 = reinterpret_cast<const float4*>(sm + mu * Dp);
-        const float4* r1 = reinterpret_cast<const float4*>(sm + (two ? mu + 1 : mu) * Dp);
-        float a0 = -b1[mu], a1 = two ? -b1[mu + 1] : 0.f, a2 = 0.f, a3 = 0.f;
-#pragma unroll
-        for (int v = 0; v < Dp / 4; ++v) {
-            const float4 w0 = r0[v], w1 = r1[v];
-            a0 = fmaf(w0.x, q[4 * v], a0); a2 = fmaf(w0.y, q[4 * v + 1], a2);
-            a0 = fmaf(w0.z, q[4 * v + 2], a0); a2 = fmaf(w0.w, q[4 * v + 3], a2);
-            a1 = fmaf(w1.x, q[4 * v], a1); a3 = fmaf(w1.y, q[4 * v + 1], a3);
-            a1 = fmaf(w1.z, q[4 * v + 2], a1); a3 = fmaf(w1.w, q[4 * v + 3], a3);
-        }
-        float t0, d0, t1, d1;
-        tanh_sech2(a0 + a2, &t0, &d0);
-        tanh_sech2(a1 + a3, &t1, &d1);
-        const float g0 = w2[mu] * d0, g1 = two ? w2[mu + 1] * d1 : 0.f;
-        U = fmaf(w2[mu], t0, U);
-        if (two) U = fmaf(w2[mu + 1], t1, U);
-#pragma unroll
-        for (int v = 0; v < Dp / 4; ++v) {
-            const float4 w0 = r0[v], w1 = r1[v];
-            Fp[4 * v] = fmaf(g0, w0.x, fmaf(g1, w1.x, Fp[4 * v]));
-            Fp[4 * v + 1] = fmaf(g0, w0.y, fmaf(g1, w1.y, Fp[4 * v + 1]));
-            Fp[4 * v + 2] = fmaf(g0, w0.z, fmaf(g1, w1.z, Fp[4 * v + 2]));
-            Fp[4 * v + 3] = fmaf(g0, w0.w, fmaf(g1, w1.w, Fp[4 * v + 3]));
-        }
-    }
-    if (active && h == 0) d.Us[i] = U;
-
-    // ---- A[n][lm] = 2 Fp_nl C_lm s_nlm, in place ----
-#pragma unroll
-    for (int a = 0; a < NH; ++a)
-#pragma unroll
-        for (int m = 0; m < kNumLM; ++m) {
-            const float f0 = Fp[NR + 4 * a + LOF[m] - 1];
-            const float f1 = (a + NH < NA) ? Fp[NR + 4 * (a + NH < NA ? a + NH : 0) + LOF[m] - 1] : 0.f;
-            s[a][m] *= 2.f * C[m] * (h ? f1 : f0);
-        }
-    float FpR[NR];      // this lane's share of the radial-family force on shared (angular) neighbours
-#pragma unroll
-    for (int n = 0; n < NR; ++n) FpR[n] = ((n & 1) == h) ? Fp[n] : 0.f;
-
-    // ---- partial forces, Eq. 23-25 ----
-    float fsx = 0.f, fsy = 0.f, fsz = 0.f;
-    float4* prow = d.p + (size_t)i * P.capMD;
-    const unsigned short* slots = d.slots + i;
-    for (int k = 0; k < nA; ++k) {          // both lanes: same neighbour, own half of n
-        const float4 e = rec[(size_t)k * N];
-        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
-        float rinv = rsqrtf(r2);
-        rinv = rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);
-        const float r = r2 * rinv;
-        const float om = MULTI ? zrow[(__float_as_int(e.w) >> 24) & 7] : 1.f;
-        const float x = e.x * rinv, y = e.y * rinv, z = e.z * rinv;
-        float g[NA], dg[NA];
-        radial_fn<NA, true>(r, P.rcA_inv, om, g, dg);
-        float Sp[kNumLM], St[kNumLM];
-#pragma unroll
-        for (int m = 0; m < kNumLM; ++m) { Sp[m] = 0.f; St[m] = 0.f; }
-#pragma unroll
-        for (int a = 0; a < NH; ++a) {
-            const int a1 = a + NH < NA ? a + NH : 0;
-            const float ga = (h ? (a + NH < NA ? g[a1] : 0.f) : g[a]) * rinv;
-            const float da = h ? (a + NH < NA ? dg[a1] : 0.f) : dg[a];
-#pragma unroll
-            for (int m = 0; m < kNumLM; ++m) {
-                Sp[m] = fmaf(s[a][m], da, Sp[m]);
-                St[m] = fmaf(s[a][m], ga, St[m]);
-            }
-        }
-        float px, py, pz;
-        ylm_force(x, y, z, Sp, St, &px, &py, &pz);
-        float gr[NR], dgr[NR];
-        radial_fn<NR, true>(r, P.rcR_inv, om, gr, dgr);
-        float sr = 0.f;
-#pragma unroll
-        for (int n = 0; n < NR; ++n) sr = fmaf(FpR[n], dgr[n], sr);
-        px = fmaf(sr, x, px); py = fmaf(sr, y, py); pz = fmaf(sr, z, pz);
-        px += __shfl_xor_sync(FULL, px, 1);
-        py += __shfl_xor_sync(FULL, py, 1);
-        pz += __shfl_xor_sync(FULL, pz, 1);
-        if (h == 0) {
-            fsx += px; fsy += py; fsz += pz;
-            if (active) prow[slots[(size_t)k * N] & 0xff] = make_float4(px, py, pz, 0.f);
-        }
-    }
-    for (int k = nA + h; k < nR; k += 2) {  // radial-only neighbours, split between the lanes
-        const int sl = P.capR - 1 - (k - nA);
-        const float4 e = rec[(size_t)sl * N];
-        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
-        float rinv = rsqrtf(r2);
-        rinv = rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);
-        const float om = MULTI ? zrow[(__float_as_int(e.w) >> 24) & 7] : 1.f;
-        float gr[NR], dgr[NR];
-        radial_fn<NR, true>(r2 * rinv, P.rcR_inv, om, gr, dgr);
-        float sr = 0.f;
-#pragma unroll
-        for (int n = 0; n < NR; ++n) sr = fmaf(Fp[n], dgr[n], sr);
-        sr *= rinv;
-        const float px = sr * e.x, py = sr * e.y, pz = sr * e.z;
-        fsx += px; fsy += py; fsz += pz;
-        if (active) prow[slots[(size_t)sl * N] & 0xff] = make_float4(px, py, pz, 0.f);
-    }
-    fsx += __shfl_xor_sync(FULL, fsx, 1);
-    fsy += __shfl_xor_sync(FULL, fsy, 1);
-    fsz += __shfl_xor_sync(FULL, fsz, 1);
-    if (active && h == 0) d.Fself[i] = make_float4(fsx, fsy, fsz, 0.f);
-}
+#ifndef NEP_MAIN_MIN_BLOCKS
+#define NEP_MAIN_MIN_BLOCKS 2
+#endif
+#include "nep_main.cuh"
 
 // ------------------------------------------------------------------------------------------------
 // assembly (Eq. 4-7) + second half-kick + thermo, and the integrator's first half
@@ -586,6 +399,25 @@ struct AsmParams {
     double* heat_sum; double* thermo;
 };
 
+__device__ __forceinline__ int rank_below(const uint4& m, int t) {      // number of set bits at positions < t
+    const unsigned w[4] = {m.x, m.y, m.z, m.w};
+    int r = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int lo = t - 32 * q;                                      // bits of word q below t
+        const unsigned msk = lo >= 32 ? 0xffffffffu : (lo <= 0 ? 0u : ((1u << lo) - 1u));
+        r += __popc(w[q] & msk);
+    }
+    return r;
+}
+__device__ __forceinline__ bool bit_set(const uint4& m, int t) {
+    const unsigned w[4] = {m.x, m.y, m.z, m.w};
+    unsigned v = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) if ((t >> 5) == q) v = w[q];
+    return (v >> (t & 31)) & 1u;
+}
+
 __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
     const int N = P.N;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -594,17 +426,41 @@ __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
         const int nR = d.nnR[i], nA = d.nnA[i];
         float fx = 0.f, fy = 0.f, fz = 0.f;
         float w[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-#pragma unroll 4
-        for (int k = 0; k < nR; ++k) {
-            const int slot = k < nA ? k : P.capR - 1 - (k - nA);
-            const float4 e = d.rec[(size_t)slot * N + i];
-            const int j = __float_as_int(e.w) & kJMask;
-            const int rev = d.slots[(size_t)slot * N + i] >> 8;
-            const float4 pj = d.p[(size_t)j * P.capMD + rev];          // dU_j/dr_ji
-            fx += pj.x; fy += pj.y; fz += pj.z;
-            w[0] = fmaf(e.x, pj.x, w[0]); w[1] = fmaf(e.x, pj.y, w[1]); w[2] = fmaf(e.x, pj.z, w[2]);
-            w[3] = fmaf(e.y, pj.x, w[3]); w[4] = fmaf(e.y, pj.y, w[4]); w[5] = fmaf(e.y, pj.z, w[5]);
-            w[6] = fmaf(e.z, pj.x, w[6]); w[7] = fmaf(e.z, pj.y, w[7]); w[8] = fmaf(e.z, pj.z, w[8]);
+        constexpr int B = 8;             // batch the three dependent loads (jrev -> masks -> p) for MLP
+        for (int k0 = 0; k0 < nR; k0 += B) {
+            int jr[B];
+            float4 eb[B], pb[B];
+            uint4 mrb[B], mab[B];
+#pragma unroll
+            for (int u = 0; u < B; ++u) {
+                const int k = min(k0 + u, nR - 1);
+                const int slot = k < nA ? k : P.capR - 1 - (k - nA);
+                jr[u] = d.jrev[(size_t)slot * N + i];
+                eb[u] = d.rec[(size_t)slot * N + i];
+            }
+#pragma unroll
+            for (int u = 0; u < B; ++u) {
+                const int j = jr[u] & kJMask;
+                mrb[u] = d.masks[2 * (size_t)j];
+                mab[u] = d.masks[2 * (size_t)j + 1];
+            }
+#pragma unroll
+            for (int u = 0; u < B; ++u) {
+                const int j = jr[u] & kJMask, rev = jr[u] >> 24;      // rev: Verlet slot of i in j's row
+                // record slot of i in j's row = rank of Verlet slot rev among j's accepted slots
+                const int cs = rank_below(mab[u], rev);
+                const int cslot = bit_set(mab[u], rev) ? cs : P.capR - 1 - (rank_below(mrb[u], rev) - cs);
+                pb[u] = d.p[(size_t)j * P.capR + cslot];              // dU_j/dr_ji
+            }
+#pragma unroll
+            for (int u = 0; u < B; ++u) {
+                if (k0 + u >= nR) break;
+                const float4 e = eb[u], pj = pb[u];
+                fx += pj.x; fy += pj.y; fz += pj.z;
+                w[0] = fmaf(e.x, pj.x, w[0]); w[1] = fmaf(e.x, pj.y, w[1]); w[2] = fmaf(e.x, pj.z, w[2]);
+                w[3] = fmaf(e.y, pj.x, w[3]); w[4] = fmaf(e.y, pj.y, w[4]); w[5] = fmaf(e.y, pj.z, w[5]);
+                w[6] = fmaf(e.z, pj.x, w[6]); w[7] = fmaf(e.z, pj.y, w[7]); w[8] = fmaf(e.z, pj.z, w[8]);
+            }
         }
         const float4 fs = d.Fself[i];
         fx = fs.x - fx; fy = fs.y - fy; fz = fs.z - fz;               // Eq. 4-5
@@ -665,17 +521,20 @@ __global__ void k_kick_drift(SysDev d, int N, double dt, double half_skin2, AsmP
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i == 0) d.flags[F_STEP] += 1;
     if (i >= N) return;
-    const double im = P.inv_mass[d.type_s[i]] * P.half_dt;
-    double disp2 = 0.0;
+    const int ty = d.type_s[i];
+    const double im = P.inv_mass[ty] * P.half_dt;
+    double disp2 = 0.0, xn[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const double v = d.vs[a * N + i] + im * (double)d.Fs[a * N + i];
         const double x = d.xs[a * N + i] + dt * v;
         d.vs[a * N + i] = v;
         d.xs[a * N + i] = x;
+        xn[a] = x;
         const double dd = x - d.xref[a * N + i];
         disp2 += dd * dd;
     }
+    d.xs4[i] = make_double4(xn[0], xn[1], xn[2], __longlong_as_double((long long)ty));
     if (disp2 > half_skin2) d.flags[F_REBUILD] = 1;
 }
 
@@ -687,15 +546,17 @@ __global__ void k_load_state(SysDev d, int N, const double* __restrict__ pos, co
     if (k == 0 && mode == 1) d.flags[F_STEP] = 0;
     if (k >= N) return;
     const int src = d.perm[k];
-    double disp2 = 0.0;
+    double disp2 = 0.0, xn[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const double x = pos[a * N + src];
         d.xs[a * N + k] = x;
+        xn[a] = x;
         const double dd = x - d.xref[a * N + k];
         disp2 += dd * dd;
         if (vel) d.vs[a * N + k] = vel[a * N + src];
     }
+    d.xs4[k] = make_double4(xn[0], xn[1], xn[2], __longlong_as_double((long long)d.type_s[k]));
     if (disp2 > half_skin2) {
         if (mode == 0) atomicOr(&d.flags[F_STATUS], ST_STALE); else d.flags[F_REBUILD] = 1;
     }
@@ -765,8 +626,10 @@ Layout carve(int64_t N, int capR, int capMD, int max_cells, SysDev* d, char* bas
     t.nnR = (int*)take(n * 4);
     t.nnA = (int*)take(n * 4);
     t.rec = (float4*)take(n * 16 * capR);
-    t.slots = (unsigned short*)take(n * 2 * capR);
-    t.p = (float4*)take(n * 16 * capMD);
+    t.jrev = (int*)take(n * 4 * capR);
+    t.masks = (uint4*)take(n * 32);
+    t.xs4 = (double4*)take(n * 32);
+    t.p = (float4*)take(n * 16 * capR);
     L.total = o;
     if (d) *d = t;
     return L;
@@ -804,13 +667,14 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
     MainParams P;
     P.rcR_inv = (float)(1.0 / m->h.rc_radial); P.rcA_inv = (float)(1.0 / m->h.rc_angular);
     P.H = m->H; P.N = (int)s->N; P.capR = s->capR; P.capMD = s->capMD;
-    const size_t smem = ((size_t)((m->params_floats + 3) & ~3) + kMaxTypes * kMaxTypes) * sizeof(float);
+    const size_t smem = ((size_t)((m->params_floats + 3) & ~3) + kMaxTypes * kMaxTypes) * sizeof(float) +
+                        (size_t)s->capR * kMainAtoms * sizeof(float4);
     static bool attr_done = false;
     if (!attr_done) {
-        cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         attr_done = true;
     }
-    k_main<NR, NA, MULTI><<<grid_for(2 * s->N, 128), 128, smem, st>>>(s->d, P, m->params_dev, m->sqrtzz_dev);
+    k_main<NR, NA, MULTI><<<grid_for(s->N, kMainAtoms), kMainThreads, smem, st>>>(s->d, P, m->params_dev, m->sqrtzz_dev);
     s->launches += 1;
 }
 

@@ -1,0 +1,262 @@
+// nep_main.cuh -- k_main: descriptor + network + partial forces (included by nep_b200.cu inside its
+// anonymous namespace, after SysDev and nep_math.cuh).
+//
+// Block = 128 threads = 64 atoms x 2 lanes.  Lane h of an atom's pair owns the angular radial
+// indices n = h*NH .. h*NH+NH-1 (all 24 lm of each) and every second hidden neuron, so both lanes run
+// one instruction stream; q, dU/dq and the per-neighbour partial force cross the pair with __shfl_xor.
+//
+// Neighbour records of the block's 64 atoms are staged once into shared memory with cp.async
+// (16 B per thread, rows of 64 records = 1 KB contiguous in the [slot][atom] layout), so the three
+// passes over the neighbours read shared memory instead of stalling on global loads.
+#pragma once
+
+struct MainParams {
+    float rcR_inv, rcA_inv;
+    int H, N, capR, capMD;
+};
+
+constexpr int kMainThreads = 128;
+constexpr int kMainAtoms = kMainThreads / 2;
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+__device__ __forceinline__ float inv_norm(float r2) {
+    float rinv = rsqrtf(r2);
+    return rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);      // one Newton step: < 1 ulp
+}
+
+template <int NR, int NA, bool MULTI>
+__global__ void __launch_bounds__(kMainThreads, NEP_MAIN_MIN_BLOCKS) k_main(SysDev d, MainParams P,
+                                                                          const float* __restrict__ params,
+                                                                          const float* __restrict__ sqrtzz) {
+    constexpr int NH = (NA + 1) / 2;
+    constexpr int D = NR + 4 * NA;
+    constexpr int Dp = (D + 3) & ~3;
+    constexpr float C[kNumLM] = {NEP_CLM_LIST};
+    constexpr int LOF[kNumLM] = {NEP_LOF_LIST};
+    extern __shared__ __align__(16) float sm[];
+    __shared__ int s_max[2];
+    const int H = P.H, N = P.N;
+    const int nfl = H * Dp + 2 * H + 1;
+    float* szz = sm + ((nfl + 3) & ~3);
+    float4* srec = reinterpret_cast<float4*>(szz + kMaxTypes * kMaxTypes);     // [rows][64]
+
+    const int tid = threadIdx.x;
+    const int a_loc = tid >> 1;                       // atom within the block
+    const int i0 = blockIdx.x * kMainAtoms;
+    const bool active = i0 + a_loc < N;
+    const int i = active ? i0 + a_loc : N - 1;
+    const int h = tid & 1;
+    const unsigned PAIR = 3u << (tid & 30);           // the atom's lane pair (trip counts differ across pairs)
+    const int nR = d.nnR[i], nA = d.nnA[i];
+    const int nO = nR - nA;
+
+    // ---- stage weights and this block's neighbour records ----
+    if (tid < 2) s_max[tid] = 0;
+    __syncthreads();
+    {
+        int mA = nA, mO = nO;
+        mA = __reduce_max_sync(0xffffffffu, mA);
+        mO = __reduce_max_sync(0xffffffffu, mO);
+        if ((tid & 31) == 0) { atomicMax(&s_max[0], mA); atomicMax(&s_max[1], mO); }
+    }
+    for (int k = tid; k < nfl; k += kMainThreads) sm[k] = params[k];
+    if (MULTI) for (int k = tid; k < kMaxTypes * kMaxTypes; k += kMainThreads) szz[k] = sqrtzz[k];
+    __syncthreads();
+    const int maxA = s_max[0], maxO = s_max[1];
+    {
+        // smem row r < maxA holds global slot r; row maxA + o holds global slot capR-1-o
+        const int rows = maxA + maxO;
+        const int col = tid & (kMainAtoms - 1);
+        const int src_atom = min(i0 + col, N - 1);
+        for (int r = tid >> 6; r < rows; r += 2) {
+            const int slot = r < maxA ? r : P.capR - 1 - (r - maxA);
+            cp_async16(&srec[r * kMainAtoms + col], &d.rec[(size_t)slot * N + src_atom]);
+        }
+        cp_async_wait_all();
+    }
+    __syncthreads();
+    const float4* myrec = srec + a_loc;
+    const float* zrow = MULTI ? szz + d.type_s[i] * kMaxTypes : nullptr;
+    auto omega = [&](const float4& e) { return MULTI ? zrow[__float_as_int(e.w) & 7] : 1.f; };
+
+    // ---- radial descriptor, Eq. 12: neighbours split between the two lanes ----
+    float q[Dp];
+#pragma unroll
+    for (int v = 0; v < Dp; ++v) q[v] = 0.f;
+    for (int k = h; k < nR; k += 2) {
+        const float4 e = myrec[(k < nA ? k : maxA + (k - nA)) * kMainAtoms];
+        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+        const float rinv = inv_norm(r2);
+        float g[NR];
+        radial_fn<NR, false>(r2 * rinv, P.rcR_inv, omega(e), g, nullptr);
+#pragma unroll
+        for (int n = 0; n < NR; ++n) q[n] += g[n];
+    }
+#pragma unroll
+    for (int n = 0; n < NR; ++n) q[n] += __shfl_xor_sync(PAIR, q[n], 1);
+
+    // ---- angular sums s[n][lm] = sum_j g_n(r_ij) b_lm(r^_ij)  (Eq. 18 in real form) ----
+    float s[NH][kNumLM];
+#pragma unroll
+    for (int k = 0; k < NH; ++k)
+#pragma unroll
+        for (int m = 0; m < kNumLM; ++m) s[k][m] = 0.f;
+    for (int k = 0; k < nA; ++k) {
+        const float4 e = myrec[k * kMainAtoms];
+        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+        const float rinv = inv_norm(r2);
+        float g[NA];
+        radial_fn<NA, false>(r2 * rinv, P.rcA_inv, omega(e), g, nullptr);
+        float go[NH];
+#pragma unroll
+        for (int a = 0; a < NH; ++a) go[a] = h ? (a + NH < NA ? g[a + NH < NA ? a + NH : 0] : 0.f) : g[a];
+        float b[kNumLM];
+        ylm_basis(e.x * rinv, e.y * rinv, e.z * rinv, b);
+#pragma unroll
+        for (int a = 0; a < NH; ++a)
+#pragma unroll
+            for (int m = 0; m < kNumLM; ++m) s[a][m] = fmaf(go[a], b[m], s[a][m]);
+    }
+
+    // ---- q_nl = sum_m C_lm s_nlm^2 (Eq. 17 with n' = n), exchanged across the pair ----
+    {
+        float qa[NH][4];
+#pragma unroll
+        for (int a = 0; a < NH; ++a) {
+#pragma unroll
+            for (int l = 0; l < 4; ++l) qa[a][l] = 0.f;
+#pragma unroll
+            for (int m = 0; m < kNumLM; ++m) qa[a][LOF[m] - 1] = fmaf(C[m] * s[a][m], s[a][m], qa[a][LOF[m] - 1]);
+        }
+#pragma unroll
+        for (int a = 0; a < NH; ++a)
+#pragma unroll
+            for (int l = 0; l < 4; ++l) {
+                const float mine = qa[a][l];
+                const float other = __shfl_xor_sync(PAIR, mine, 1);
+                q[NR + 4 * a + l] = h ? other : mine;                           // n = a       (lane 0's)
+                if (a + NH < NA) q[NR + 4 * (a + NH) + l] = h ? mine : other;   // n = a + NH  (lane 1's)
+            }
+    }
+
+    // ---- network Eq. 21-22 and Fp = dU/dq.  Lane h evaluates neurons mu = h, h+2, ... (two per
+    //      iteration for ILP); the partial U and Fp are summed across the pair. ----
+    float Fp[Dp];
+#pragma unroll
+    for (int v = 0; v < Dp; ++v) Fp[v] = 0.f;
+    const float* b1 = sm + H * Dp;
+    const float* w2 = b1 + H;
+    float U = h ? 0.f : -w2[H];                                              // - b2 (once)
+    for (int mu = h; mu < H; mu += 4) {
+        const bool two = mu + 2 < H;
+        const int mu1 = two ? mu + 2 : mu;
+        const float4* r0 = reinterpret_cast<const float4*>(sm + mu * Dp);
+        const float4* r1 = reinterpret_cast<const float4*>(sm + mu1 * Dp);
+        float a0 = -b1[mu], a1 = -b1[mu1], a2 = 0.f, a3 = 0.f;
+#pragma unroll
+        for (int v = 0; v < Dp / 4; ++v) {
+            const float4 w0 = r0[v], w1 = r1[v];
+            a0 = fmaf(w0.x, q[4 * v], a0); a2 = fmaf(w0.y, q[4 * v + 1], a2);
+            a0 = fmaf(w0.z, q[4 * v + 2], a0); a2 = fmaf(w0.w, q[4 * v + 3], a2);
+            a1 = fmaf(w1.x, q[4 * v], a1); a3 = fmaf(w1.y, q[4 * v + 1], a3);
+            a1 = fmaf(w1.z, q[4 * v + 2], a1); a3 = fmaf(w1.w, q[4 * v + 3], a3);
+        }
+        float t0, d0, t1, d1;
+        tanh_sech2(a0 + a2, &t0, &d0);
+        tanh_sech2(a1 + a3, &t1, &d1);
+        const float g0 = w2[mu] * d0, g1 = two ? w2[mu1] * d1 : 0.f;
+        U = fmaf(w2[mu], t0, U);
+        if (two) U = fmaf(w2[mu1], t1, U);
+#pragma unroll
+        for (int v = 0; v < Dp / 4; ++v) {
+            const float4 w0 = r0[v], w1 = r1[v];
+            Fp[4 * v] = fmaf(g0, w0.x, fmaf(g1, w1.x, Fp[4 * v]));
+            Fp[4 * v + 1] = fmaf(g0, w0.y, fmaf(g1, w1.y, Fp[4 * v + 1]));
+            Fp[4 * v + 2] = fmaf(g0, w0.z, fmaf(g1, w1.z, Fp[4 * v + 2]));
+            Fp[4 * v + 3] = fmaf(g0, w0.w, fmaf(g1, w1.w, Fp[4 * v + 3]));
+        }
+    }
+    U += __shfl_xor_sync(PAIR, U, 1);
+#pragma unroll
+    for (int v = 0; v < D; ++v) Fp[v] += __shfl_xor_sync(PAIR, Fp[v], 1);
+    if (active && h == 0) d.Us[i] = U;
+
+    // ---- A[n][lm] = 2 Fp_nl C_lm s_nlm, in place ----
+#pragma unroll
+    for (int a = 0; a < NH; ++a)
+#pragma unroll
+        for (int m = 0; m < kNumLM; ++m) {
+            const float f0 = Fp[NR + 4 * a + LOF[m] - 1];
+            const float f1 = (a + NH < NA) ? Fp[NR + 4 * (a + NH < NA ? a + NH : 0) + LOF[m] - 1] : 0.f;
+            s[a][m] *= 2.f * C[m] * (h ? f1 : f0);
+        }
+    float FpR[NR];      // this lane's share of the radial-family force on shared (angular) neighbours
+#pragma unroll
+    for (int n = 0; n < NR; ++n) FpR[n] = ((n & 1) == h) ? Fp[n] : 0.f;
+
+    // ---- partial forces, Eq. 23-25 ----
+    float fsx = 0.f, fsy = 0.f, fsz = 0.f;
+    float4* prow = d.p + (size_t)i * P.capR;       // p_ij lives at the record's own slot
+    for (int k = 0; k < nA; ++k) {          // both lanes: same neighbour, own half of n
+        const float4 e = myrec[k * kMainAtoms];
+        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+        const float rinv = inv_norm(r2);
+        const float r = r2 * rinv;
+        const float om = omega(e);
+        const float x = e.x * rinv, y = e.y * rinv, z = e.z * rinv;
+        float g[NA], dg[NA];
+        radial_fn<NA, true>(r, P.rcA_inv, om, g, dg);
+        float Sp[kNumLM], St[kNumLM];
+#pragma unroll
+        for (int m = 0; m < kNumLM; ++m) { Sp[m] = 0.f; St[m] = 0.f; }
+#pragma unroll
+        for (int a = 0; a < NH; ++a) {
+            const int a1 = a + NH < NA ? a + NH : 0;
+            const float ga = (h ? (a + NH < NA ? g[a1] : 0.f) : g[a]) * rinv;
+            const float da = h ? (a + NH < NA ? dg[a1] : 0.f) : dg[a];
+#pragma unroll
+            for (int m = 0; m < kNumLM; ++m) {
+                Sp[m] = fmaf(s[a][m], da, Sp[m]);
+                St[m] = fmaf(s[a][m], ga, St[m]);
+            }
+        }
+        float px, py, pz;
+        ylm_force(x, y, z, Sp, St, &px, &py, &pz);
+        float gr[NR], dgr[NR];
+        radial_fn<NR, true>(r, P.rcR_inv, om, gr, dgr);
+        float sr = 0.f;
+#pragma unroll
+        for (int n = 0; n < NR; ++n) sr = fmaf(FpR[n], dgr[n], sr);
+        px = fmaf(sr, x, px); py = fmaf(sr, y, py); pz = fmaf(sr, z, pz);
+        px += __shfl_xor_sync(PAIR, px, 1);
+        py += __shfl_xor_sync(PAIR, py, 1);
+        pz += __shfl_xor_sync(PAIR, pz, 1);
+        if (h == 0) {
+            fsx += px; fsy += py; fsz += pz;
+            if (active) prow[k] = make_float4(px, py, pz, 0.f);
+        }
+    }
+    for (int k = nA + h; k < nR; k += 2) {  // radial-only neighbours, split between the lanes
+        const float4 e = myrec[(maxA + (k - nA)) * kMainAtoms];
+        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+        const float rinv = inv_norm(r2);
+        float gr[NR], dgr[NR];
+        radial_fn<NR, true>(r2 * rinv, P.rcR_inv, omega(e), gr, dgr);
+        float sr = 0.f;
+#pragma unroll
+        for (int n = 0; n < NR; ++n) sr = fmaf(Fp[n], dgr[n], sr);
+        sr *= rinv;
+        const float px = sr * e.x, py = sr * e.y, pz = sr * e.z;
+        fsx += px; fsy += py; fsz += pz;
+        if (active) prow[P.capR - 1 - (k - nA)] = make_float4(px, py, pz, 0.f);
+    }
+    fsx += __shfl_xor_sync(PAIR, fsx, 1);
+    fsy += __shfl_xor_sync(PAIR, fsy, 1);
+    fsz += __shfl_xor_sync(PAIR, fsz, 1);
+    if (active && h == 0) d.Fself[i] = make_float4(fsx, fsy, fsz, 0.f);
+}

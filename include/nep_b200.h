@@ -147,6 +147,10 @@ int64_t nep_launch_count(const nep_system*);
 int  nep_profile(nep_system*, int enable);
 int  nep_get_profile(nep_system*, double ms[8], int64_t count[8]);
 
+/* Register-resident FMA-chain microbenchmark (a few ms): achieved FP32 non-tensor TFLOP/s with scalar
+ * FFMA and with packed fma.rn.f32x2 -- the measured denominator of the "alu" roofline. */
+int  nep_measure_fp32_peak(double* tflops_ffma, double* tflops_ffma2, void* cuda_stream);
+
 const char* nep_strerror(int code);
 
 #ifdef __cplusplus

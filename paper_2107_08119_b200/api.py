@@ -16,7 +16,7 @@ _lib = None
 
 SYMBOLS = ["nep_create", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",
            "nep_system_create", "nep_system_destroy", "nep_neighbors", "nep_get_neighbors", "nep_compute",
-           "nep_md_step", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile",
+           "nep_md_step", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile", "nep_measure_fp32_peak",
            "nep_strerror"]
 
 
@@ -178,6 +178,13 @@ class System:
         if getattr(self, "_h", None) and self._h.value and _lib is not None:
             _lib.nep_system_destroy(self._h)
             self._h = C.c_void_p()
+
+
+def measure_fp32_peak():
+    """(TFLOP/s with scalar FFMA, TFLOP/s with packed fma.f32x2) from the library's FMA-chain microbenchmark."""
+    a, b = C.c_double(), C.c_double()
+    _check(lib().nep_measure_fp32_peak(C.byref(a), C.byref(b), _stream()), "nep_measure_fp32_peak")
+    return a.value, b.value
 
 
 def from_workload(w, cap_radial=64, cap_angular=32, skin=1.0, device="cuda:0"):

@@ -384,6 +384,7 @@ __global__ void k_export_lists(SysDev d, int N, int which, int capR, int cap_out
 #define NEP_MAIN_MIN_BLOCKS 2
 #endif
 #include "nep_main.cuh"
+#include "fp32_peak.cuh"
 
 // ------------------------------------------------------------------------------------------------
 // assembly (Eq. 4-7) + second half-kick + thermo, and the integrator's first half
@@ -668,7 +669,7 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
     P.rcR_inv = (float)(1.0 / m->h.rc_radial); P.rcA_inv = (float)(1.0 / m->h.rc_angular);
     P.H = m->H; P.N = (int)s->N; P.capR = s->capR; P.capMD = s->capMD;
     const size_t smem = ((size_t)((m->params_floats + 3) & ~3) + kMaxTypes * kMaxTypes) * sizeof(float) +
-                        (size_t)s->capR * kMainAtoms * sizeof(float4);
+                        (size_t)s->capR * kMainAtoms * (sizeof(float4) + sizeof(float));
     static bool attr_done = false;
     if (!attr_done) {
         cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -983,6 +984,36 @@ int nep_stats(nep_system* s, int64_t out[4]) {
 }
 
 int64_t nep_launch_count(const nep_system* s) { return s ? s->launches : 0; }
+
+int nep_measure_fp32_peak(double* tflops_ffma, double* tflops_ffma2, void* cuda_stream) {
+    if (!tflops_ffma || !tflops_ffma2) return NEP_EINVAL;
+    if (!device_ok()) { set_cuda_error(cudaErrorNoDevice, "nep_measure_fp32_peak"); return NEP_ECUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaDeviceProp prop;
+    NEP_CUDA_OK(cudaGetDeviceProperties(&prop, 0));
+    float* out = nullptr;
+    NEP_CUDA_OK(cudaMalloc(&out, 16));
+    cudaEvent_t e0, e1;
+    NEP_CUDA_OK(cudaEventCreate(&e0)); NEP_CUDA_OK(cudaEventCreate(&e1));
+    const int blocks = prop.multiProcessorCount * 8, iters = 1 << 15;
+    double* res[2] = {tflops_ffma, tflops_ffma2};
+    for (int v = 0; v < 2; ++v) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; ++rep) {
+            NEP_CUDA_OK(cudaEventRecord(e0, st));
+            if (v == 0) k_fma_chain<false><<<blocks, 256, 0, st>>>(out, iters, 0.999f, 0.001f);
+            else k_fma_chain<true><<<blocks, 256, 0, st>>>(out, iters, 0.999f, 0.001f);
+            NEP_CUDA_OK(cudaEventRecord(e1, st));
+            NEP_CUDA_OK(cudaEventSynchronize(e1));
+            float ms = 0.f;
+            NEP_CUDA_OK(cudaEventElapsedTime(&ms, e0, e1));
+            if (rep > 0 && ms < best) best = ms;
+        }
+        *res[v] = 2.0 * 16.0 * iters * 256.0 * blocks / (best * 1e-3) / 1e12;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
+    return NEP_OK;
+}
 
 int nep_profile(nep_system* s, int enable) {
     if (!s) return NEP_EINVAL;

@@ -25,7 +25,8 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
 __device__ __forceinline__ float inv_norm(float r2) {
-    float rinv = rsqrtf(r2);
+    float rinv;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(r2));       // MUFU.RSQ, no denormal fix-up (r2 >> 0)
     return rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);      // one Newton step: < 1 ulp
 }
 
@@ -43,7 +44,8 @@ __global__ void __launch_bounds__(kMainThreads, NEP_MAIN_MIN_BLOCKS) k_main(SysD
     const int H = P.H, N = P.N;
     const int nfl = H * Dp + 2 * H + 1;
     float* szz = sm + ((nfl + 3) & ~3);
-    float4* srec = reinterpret_cast<float4*>(szz + kMaxTypes * kMaxTypes);     // [rows][64]
+    float4* srec = reinterpret_cast<float4*>(szz + kMaxTypes * kMaxTypes);     // [rows][64] neighbour records
+    float* scr = reinterpret_cast<float*>(srec + P.capR * kMainAtoms);         // [rows][64] radial-family scalars
 
     const int tid = threadIdx.x;
     const int a_loc = tid >> 1;                       // atom within the block
@@ -78,11 +80,18 @@ __global__ void __launch_bounds__(kMainThreads, NEP_MAIN_MIN_BLOCKS) k_main(SysD
             cp_async16(&srec[r * kMainAtoms + col], &d.rec[(size_t)slot * N + src_atom]);
         }
         cp_async_wait_all();
+        if (MULTI) {        // Eq. 19: replace the neighbour's type by omega_ij = sqrt(Z_i Z_j), once
+            const float* zr = szz + d.type_s[src_atom] * kMaxTypes;
+            for (int r = tid >> 6; r < rows; r += 2) {
+                float* w = &srec[r * kMainAtoms + col].w;
+                *w = zr[__float_as_int(*w) & 7];
+            }
+        }
     }
     __syncthreads();
     const float4* myrec = srec + a_loc;
-    const float* zrow = MULTI ? szz + d.type_s[i] * kMaxTypes : nullptr;
-    auto omega = [&](const float4& e) { return MULTI ? zrow[__float_as_int(e.w) & 7] : 1.f; };
+    float* mycr = scr + a_loc;
+    auto omega = [&](const float4& e) { return MULTI ? e.w : 1.f; };
 
     // ---- radial descriptor, Eq. 12: neighbours split between the two lanes ----
     float q[Dp];
@@ -195,65 +204,67 @@ __global__ void __launch_bounds__(kMainThreads, NEP_MAIN_MIN_BLOCKS) k_main(SysD
             const float f1 = (a + NH < NA) ? Fp[NR + 4 * (a + NH < NA ? a + NH : 0) + LOF[m] - 1] : 0.f;
             s[a][m] *= 2.f * C[m] * (h ? f1 : f0);
         }
-    float FpR[NR];      // this lane's share of the radial-family force on shared (angular) neighbours
-#pragma unroll
-    for (int n = 0; n < NR; ++n) FpR[n] = ((n & 1) == h) ? Fp[n] : 0.f;
-
     // ---- partial forces, Eq. 23-25 ----
     float fsx = 0.f, fsy = 0.f, fsz = 0.f;
     float4* prow = d.p + (size_t)i * P.capR;       // p_ij lives at the record's own slot
-    for (int k = 0; k < nA; ++k) {          // both lanes: same neighbour, own half of n
-        const float4 e = myrec[k * kMainAtoms];
-        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
-        const float rinv = inv_norm(r2);
-        const float r = r2 * rinv;
-        const float om = omega(e);
-        const float x = e.x * rinv, y = e.y * rinv, z = e.z * rinv;
-        float g[NA], dg[NA];
-        radial_fn<NA, true>(r, P.rcA_inv, om, g, dg);
-        float Sp[kNumLM], St[kNumLM];
-#pragma unroll
-        for (int m = 0; m < kNumLM; ++m) { Sp[m] = 0.f; St[m] = 0.f; }
-#pragma unroll
-        for (int a = 0; a < NH; ++a) {
-            const int a1 = a + NH < NA ? a + NH : 0;
-            const float ga = (h ? (a + NH < NA ? g[a1] : 0.f) : g[a]) * rinv;
-            const float da = h ? (a + NH < NA ? dg[a1] : 0.f) : dg[a];
-#pragma unroll
-            for (int m = 0; m < kNumLM; ++m) {
-                Sp[m] = fmaf(s[a][m], da, Sp[m]);
-                St[m] = fmaf(s[a][m], ga, St[m]);
-            }
-        }
-        float px, py, pz;
-        ylm_force(x, y, z, Sp, St, &px, &py, &pz);
-        float gr[NR], dgr[NR];
-        radial_fn<NR, true>(r, P.rcR_inv, om, gr, dgr);
-        float sr = 0.f;
-#pragma unroll
-        for (int n = 0; n < NR; ++n) sr = fmaf(FpR[n], dgr[n], sr);
-        px = fmaf(sr, x, px); py = fmaf(sr, y, py); pz = fmaf(sr, z, pz);
-        px += __shfl_xor_sync(PAIR, px, 1);
-        py += __shfl_xor_sync(PAIR, py, 1);
-        pz += __shfl_xor_sync(PAIR, pz, 1);
-        if (h == 0) {
-            fsx += px; fsy += py; fsz += pz;
-            if (active) prow[k] = make_float4(px, py, pz, 0.f);
-        }
-    }
-    for (int k = nA + h; k < nR; k += 2) {  // radial-only neighbours, split between the lanes
-        const float4 e = myrec[(maxA + (k - nA)) * kMainAtoms];
+    // radial family (Eq. 24), neighbours split between the lanes: radial-only neighbours are finished
+    // here; for angular neighbours the scalar c = sum_n Fp_n g_n'(r)/r is parked in shared memory
+    for (int k = h; k < nR; k += 2) {
+        const int row = k < nA ? k : maxA + (k - nA);
+        const float4 e = myrec[row * kMainAtoms];
         const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
         const float rinv = inv_norm(r2);
         float gr[NR], dgr[NR];
         radial_fn<NR, true>(r2 * rinv, P.rcR_inv, omega(e), gr, dgr);
-        float sr = 0.f;
+        float c0 = 0.f, c1 = 0.f;
 #pragma unroll
-        for (int n = 0; n < NR; ++n) sr = fmaf(Fp[n], dgr[n], sr);
-        sr *= rinv;
-        const float px = sr * e.x, py = sr * e.y, pz = sr * e.z;
-        fsx += px; fsy += py; fsz += pz;
-        if (active) prow[P.capR - 1 - (k - nA)] = make_float4(px, py, pz, 0.f);
+        for (int n = 0; n + 1 < NR; n += 2) { c0 = fmaf(Fp[n], dgr[n], c0); c1 = fmaf(Fp[n + 1], dgr[n + 1], c1); }
+        if (NR & 1) c0 = fmaf(Fp[NR - 1], dgr[NR - 1], c0);
+        const float c = (c0 + c1) * rinv;
+        if (k < nA) {
+            mycr[row * kMainAtoms] = c;
+        } else {
+            const float px = c * e.x, py = c * e.y, pz = c * e.z;
+            fsx += px; fsy += py; fsz += pz;
+            if (active) prow[P.capR - 1 - (k - nA)] = make_float4(px, py, pz, 0.f);
+        }
+    }
+    __syncwarp(PAIR);
+    for (int k = 0; k < nA; ++k) {          // angular family (Eq. 25): both lanes, own half of n
+        const float4 e = myrec[k * kMainAtoms];
+        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+        const float rinv = inv_norm(r2);
+        const float x = e.x * rinv, y = e.y * rinv, z = e.z * rinv;
+        float g[NA], dg[NA];
+        radial_fn<NA, true>(r2 * rinv, P.rcA_inv, omega(e), g, dg);
+        float Sq[kNumLM], St[kNumLM];
+#pragma unroll
+        for (int m = 0; m < kNumLM; ++m) { Sq[m] = 0.f; St[m] = 0.f; }
+#pragma unroll
+        for (int a = 0; a < NH; ++a) {
+            const int a1 = a + NH < NA ? a + NH : 0;
+            const float ga = (h ? (a + NH < NA ? g[a1] : 0.f) : g[a]) * rinv;       // g_n / r
+            const float da = h ? (a + NH < NA ? dg[a1] : 0.f) : dg[a];              // g_n'
+            float dl[4];
+#pragma unroll
+            for (int l = 0; l < 4; ++l) dl[l] = fmaf(-(float)(l + 1), ga, da);       // g_n' - l g_n / r
+#pragma unroll
+            for (int m = 0; m < kNumLM; ++m) {
+                Sq[m] = fmaf(s[a][m], dl[LOF[m] - 1], Sq[m]);
+                St[m] = fmaf(s[a][m], ga, St[m]);
+            }
+        }
+        float px, py, pz;
+        ylm_force(x, y, z, Sq, St, &px, &py, &pz);
+        px += __shfl_xor_sync(PAIR, px, 1);
+        py += __shfl_xor_sync(PAIR, py, 1);
+        pz += __shfl_xor_sync(PAIR, pz, 1);
+        if (h == 0) {
+            const float c = mycr[k * kMainAtoms];
+            px = fmaf(c, e.x, px); py = fmaf(c, e.y, py); pz = fmaf(c, e.z, pz);
+            fsx += px; fsy += py; fsz += pz;
+            if (active) prow[k] = make_float4(px, py, pz, 0.f);
+        }
     }
     fsx += __shfl_xor_sync(PAIR, fsx, 1);
     fsy += __shfl_xor_sync(PAIR, fsy, 1);

@@ -37,13 +37,24 @@ NEP_HD float clm(int m) {
     return t[m];
 }
 
-NEP_HD void sincospi_f(float a, float* s, float* c) {
-#ifdef __CUDA_ARCH__
-    sincospif(a, s, c);
-#else
-    *s = (float)sin(3.14159265358979323846 * (double)a);
-    *c = (float)cos(3.14159265358979323846 * (double)a);
-#endif
+// sin(pi u / 2) and cos(pi u / 2) for u in [0, 1]: Taylor polynomials in t^2, t = pi u / 2 <= pi/2
+// (truncation < 6e-8 at the end of the range, where f_c -> 0); no range reduction, no branches.
+NEP_HD void sincos_halfpi(float u, float* s, float* c) {
+    const float t = 1.57079632679489662f * u;
+    const float t2 = t * t;
+    float ps = -2.50521083854417188e-8f;                 // -1/11!
+    ps = fmaf(ps, t2, 2.75573192239858907e-6f);          //  1/9!
+    ps = fmaf(ps, t2, -1.98412698412698413e-4f);         // -1/7!
+    ps = fmaf(ps, t2, 8.33333333333333333e-3f);          //  1/5!
+    ps = fmaf(ps, t2, -1.66666666666666667e-1f);         // -1/3!
+    *s = fmaf(ps * t2, t, t);
+    float pc = 2.08767569878680990e-9f;                  //  1/12!
+    pc = fmaf(pc, t2, -2.75573192239858907e-7f);         // -1/10!
+    pc = fmaf(pc, t2, 2.48015873015873016e-5f);          //  1/8!
+    pc = fmaf(pc, t2, -1.38888888888888889e-3f);         // -1/6!
+    pc = fmaf(pc, t2, 4.16666666666666667e-2f);          //  1/4!
+    pc = fmaf(pc, t2, -0.5f);
+    *c = fmaf(pc, t2, 1.f);
 }
 
 // g_n and dg_n/dr for n = 0..N-1 at distance r (r < rc), rcinv = 1/rc, omega = Eq. 19 weight.
@@ -57,7 +68,7 @@ NEP_HD void radial_fn(float r, float rcinv, float omega, float* g, float* dg) {
     const float um1 = u - 1.f;
     const float x = fmaf(2.f * um1, um1, -1.f);
     float sn, cs;
-    sincospi_f(0.5f * u, &sn, &cs);
+    sincos_halfpi(u, &sn, &cs);
     const float hf = 0.5f * omega * cs * cs;                          // omega fc / 2
     const float hb = -0.5f * omega * 3.14159265358979f * rcinv * sn * cs;   // omega fc' / 2
     const float ha = hf * 4.f * um1 * rcinv;                          // omega fc x' / 2
@@ -92,21 +103,24 @@ NEP_HD void ylm_basis(float x, float y, float z, float* b) {
 }
 
 // Angular partial force of one neighbour from the per-lm sums
-//   Sp[m] = sum_n A[n][m] g_n'(r),   St[m] = sum_n A[n][m] g_n(r) / r :
-//   p = R r^ + V,   R = sum_m b_m (Sp_m - l_m St_m),   V = sum_m St_m grad B_m(r^).
-NEP_HD void ylm_force(float x, float y, float z, const float* Sp, const float* St, float* px, float* py,
+//   Sq[m] = sum_n A[n][m] (g_n'(r) - l_m g_n(r)/r),   St[m] = sum_n A[n][m] g_n(r) / r :
+//   p = R r^ + V,   R = sum_m b_m Sq_m,   V = sum_m St_m grad B_m(r^)
+// (B_m = homogeneous form of b_m; grad(g b_m(r^)) = g' b_m r^ + (g/r)(grad B_m(r^) - l b_m r^)).
+// Each of R, Vx, Vy, Vz is accumulated in two independent chains for instruction-level parallelism.
+NEP_HD void ylm_force(float x, float y, float z, const float* Sq, const float* St, float* px, float* py,
                       float* pz) {
     float b[kNumLM];
     ylm_basis(x, y, z, b);
-    constexpr int lof[kNumLM] = {NEP_LOF_LIST};
-    float R = 0.f;
+    float R0 = 0.f, R1 = 0.f;
 #pragma unroll
-    for (int m = 0; m < kNumLM; ++m) R = fmaf(b[m], fmaf(-(float)lof[m], St[m], Sp[m]), R);
+    for (int m = 0; m < kNumLM; m += 2) { R0 = fmaf(b[m], Sq[m], R0); R1 = fmaf(b[m + 1], Sq[m + 1], R1); }
+    const float R = R0 + R1;
     const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y, xz = x * z, yz = y * z, xyz = xy * z;
     const float c2 = x2 - y2, c3 = b[13], s3 = b[14];
     const float rho2 = x2 + y2;
     const float q4 = rho2 - 4.f * z2;            // x^2 + y^2 - 4 z^2
-    float vx = St[0], vy = St[1], vz = St[2];
+    float vx = St[0], vy = St[1], vz = St[2];    // l = 1, 2, 3
+    float wx = 0.f, wy = 0.f, wz = 0.f;          // l = 4
     // l = 2
     vx = fmaf(St[3], -2.f * x, vx); vy = fmaf(St[3], -2.f * y, vy); vz = fmaf(St[3], 4.f * z, vz);
     vx = fmaf(St[4], z, vx);                                        vz = fmaf(St[4], x, vz);
@@ -122,21 +136,21 @@ NEP_HD void ylm_force(float x, float y, float z, const float* Sp, const float* S
     vx = fmaf(St[13], 3.f * c2, vx); vy = fmaf(St[13], -6.f * xy, vy);
     vx = fmaf(St[14], 6.f * xy, vx); vy = fmaf(St[14], 3.f * c2, vy);
     // l = 4
-    vx = fmaf(St[15], 12.f * x * q4, vx); vy = fmaf(St[15], 12.f * y * q4, vy);
-    vz = fmaf(St[15], -16.f * z * (3.f * rho2 - 2.f * z2), vz);
-    vx = fmaf(St[16], -z * (9.f * x2 + 3.f * y2 - 4.f * z2), vx); vy = fmaf(St[16], -6.f * xyz, vy);
-    vz = fmaf(St[16], -3.f * x * q4, vz);
-    vx = fmaf(St[17], -6.f * xyz, vx); vy = fmaf(St[17], -z * (3.f * x2 + 9.f * y2 - 4.f * z2), vy);
-    vz = fmaf(St[17], -3.f * y * q4, vz);
-    vx = fmaf(St[18], -4.f * x * (x2 - 3.f * z2), vx); vy = fmaf(St[18], 4.f * y * (y2 - 3.f * z2), vy);
-    vz = fmaf(St[18], 12.f * z * c2, vz);
-    vx = fmaf(St[19], -2.f * y * (3.f * x2 + y2 - 6.f * z2), vx);
-    vy = fmaf(St[19], -2.f * x * (x2 + 3.f * y2 - 6.f * z2), vy); vz = fmaf(St[19], 24.f * xyz, vz);
-    vx = fmaf(St[20], 3.f * z * c2, vx); vy = fmaf(St[20], -6.f * xyz, vy); vz = fmaf(St[20], c3, vz);
-    vx = fmaf(St[21], 6.f * xyz, vx); vy = fmaf(St[21], 3.f * z * c2, vy); vz = fmaf(St[21], s3, vz);
-    vx = fmaf(St[22], 4.f * c3, vx); vy = fmaf(St[22], -4.f * s3, vy);
-    vx = fmaf(St[23], 4.f * s3, vx); vy = fmaf(St[23], 4.f * c3, vy);
-    *px = fmaf(R, x, vx); *py = fmaf(R, y, vy); *pz = fmaf(R, z, vz);
+    wx = fmaf(St[15], 12.f * x * q4, wx); wy = fmaf(St[15], 12.f * y * q4, wy);
+    wz = fmaf(St[15], -16.f * z * (3.f * rho2 - 2.f * z2), wz);
+    wx = fmaf(St[16], -z * (9.f * x2 + 3.f * y2 - 4.f * z2), wx); wy = fmaf(St[16], -6.f * xyz, wy);
+    wz = fmaf(St[16], -3.f * x * q4, wz);
+    wx = fmaf(St[17], -6.f * xyz, wx); wy = fmaf(St[17], -z * (3.f * x2 + 9.f * y2 - 4.f * z2), wy);
+    wz = fmaf(St[17], -3.f * y * q4, wz);
+    wx = fmaf(St[18], -4.f * x * (x2 - 3.f * z2), wx); wy = fmaf(St[18], 4.f * y * (y2 - 3.f * z2), wy);
+    wz = fmaf(St[18], 12.f * z * c2, wz);
+    wx = fmaf(St[19], -2.f * y * (3.f * x2 + y2 - 6.f * z2), wx);
+    wy = fmaf(St[19], -2.f * x * (x2 + 3.f * y2 - 6.f * z2), wy); wz = fmaf(St[19], 24.f * xyz, wz);
+    wx = fmaf(St[20], 3.f * z * c2, wx); wy = fmaf(St[20], -6.f * xyz, wy); wz = fmaf(St[20], c3, wz);
+    wx = fmaf(St[21], 6.f * xyz, wx); wy = fmaf(St[21], 3.f * z * c2, wy); wz = fmaf(St[21], s3, wz);
+    wx = fmaf(St[22], 4.f * c3, wx); wy = fmaf(St[22], -4.f * s3, wy);
+    wx = fmaf(St[23], 4.f * s3, wx); wy = fmaf(St[23], 4.f * c3, wy);
+    *px = fmaf(R, x, vx + wx); *py = fmaf(R, y, vy + wy); *pz = fmaf(R, z, vz + wz);
 }
 
 // t = tanh(a), d = 1 - tanh^2(a) = 4 e / (1 + e)^2 with e = exp(-2|a|): no cancellation when |t| -> 1.

@@ -62,7 +62,7 @@ int main() {
                 35*z2*z2-30*z2+3,x*z*(7*z2-3),y*z*(7*z2-3),c2*(7*z2-1),s2*(7*z2-1),z*c3,z*s3,c2*c2-s2*s2,2*c2*s2};
             (void)b; double s = 0; for (int m = 0; m < kNumLM; ++m) s += (alpha[m] + beta[m]*rr) * B[m]; return s; };
         float Sp[kNumLM], St[kNumLM];
-        for (int m = 0; m < kNumLM; ++m) { Sp[m] = (float)beta[m]; St[m] = (float)((alpha[m] + beta[m]*r) / r); }
+        for (int m = 0; m < kNumLM; ++m) { St[m] = (float)((alpha[m] + beta[m]*r) / r); Sp[m] = (float)(beta[m] - lof[m] * (alpha[m] + beta[m]*r) / r); }
         float px, py, pz;
         ylm_force((float)u[0], (float)u[1], (float)u[2], Sp, St, &px, &py, &pz);
         double P[3] = {px, py, pz};

@@ -226,6 +226,12 @@ def main():
     system.status()
 
     peak_ffma, peak_ffma2 = api.measure_fp32_peak()
+    traffic = None          # dram bytes per k_main launch from the committed ncu capture (1M-atom workload only)
+    try:
+        if args.workload == "c4_1048576":
+            traffic = json.load(open(os.path.join(ROOT, "profiles", "r1_traffic.json")))["k_main_dram_bytes_per_launch"]
+    except Exception:
+        traffic = None
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -267,7 +273,7 @@ def main():
                          "peak_measured_fma_chain": {"ffma": peak_ffma, "ffma2": peak_ffma2, "unit": "TFLOP/s"},
                          "frac_of_measured_ffma": achieved / peak_ffma,
                          "flops_per_atom": flops_atom, "kernel_ms": main_ms, "kernel_share_of_step": phase_ms["main"] / tot_phase,
-                         "traffic": None},
+                         "traffic": traffic},
             "phase_ms_per_step": phase_ms,
             "cpu_baseline": cpu,
         }

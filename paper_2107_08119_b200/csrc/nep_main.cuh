@@ -30,6 +30,22 @@ __device__ __forceinline__ float inv_norm(float r2) {
     return rinv * fmaf(-0.5f * r2 * rinv, rinv, 1.5f);      // one Newton step: < 1 ulp
 }
 
+// Packed FP32x2 arithmetic (sm_100+: FFMA2 issues two FMAs per lane in one instruction slot).
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+
 template <int NR, int NA, bool MULTI>
 __global__ void __launch_bounds__(kMainThreads, NEP_MAIN_MIN_BLOCKS) k_main(SysDev d, MainParams P,
                                                                           const float* __restrict__ params,
@@ -110,27 +126,36 @@ __global__ void __launch_bounds__(kMainThreads, NEP_MAIN_MIN_BLOCKS) k_main(SysD
     for (int n = 0; n < NR; ++n) q[n] += __shfl_xor_sync(PAIR, q[n], 1);
 
     // ---- angular sums s[n][lm] = sum_j g_n(r_ij) b_lm(r^_ij)  (Eq. 18 in real form) ----
-    float s[NH][kNumLM];
+    constexpr int NP = kNumLM / 2;           // lm pairs: s2[a][mm] = {s[a][2mm], s[a][2mm+1]}
+    f32x2 s2[NH][NP];
 #pragma unroll
     for (int k = 0; k < NH; ++k)
 #pragma unroll
-        for (int m = 0; m < kNumLM; ++m) s[k][m] = 0.f;
+        for (int mm = 0; mm < NP; ++mm) s2[k][mm] = pack2(0.f, 0.f);
     for (int k = 0; k < nA; ++k) {
         const float4 e = myrec[k * kMainAtoms];
         const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
         const float rinv = inv_norm(r2);
         float g[NA];
         radial_fn<NA, false>(r2 * rinv, P.rcA_inv, omega(e), g, nullptr);
-        float go[NH];
-#pragma unroll
-        for (int a = 0; a < NH; ++a) go[a] = h ? (a + NH < NA ? g[a + NH < NA ? a + NH : 0] : 0.f) : g[a];
         float b[kNumLM];
         ylm_basis(e.x * rinv, e.y * rinv, e.z * rinv, b);
+        f32x2 bp[NP];
 #pragma unroll
-        for (int a = 0; a < NH; ++a)
+        for (int mm = 0; mm < NP; ++mm) bp[mm] = pack2(b[2 * mm], b[2 * mm + 1]);
 #pragma unroll
-            for (int m = 0; m < kNumLM; ++m) s[a][m] = fmaf(go[a], b[m], s[a][m]);
+        for (int a = 0; a < NH; ++a) {
+            const float go = h ? (a + NH < NA ? g[a + NH < NA ? a + NH : 0] : 0.f) : g[a];
+            const f32x2 gp = pack2(go, go);
+#pragma unroll
+            for (int mm = 0; mm < NP; ++mm) s2[a][mm] = ffma2(gp, bp[mm], s2[a][mm]);
+        }
     }
+    float s[NH][kNumLM];
+#pragma unroll
+    for (int a = 0; a < NH; ++a)
+#pragma unroll
+        for (int mm = 0; mm < NP; ++mm) unpack2(s2[a][mm], s[a][2 * mm], s[a][2 * mm + 1]);
 
     // ---- q_nl = sum_m C_lm s_nlm^2 (Eq. 17 with n' = n), exchanged across the pair ----
     {
@@ -156,39 +181,43 @@ __global__ void __launch_bounds__(kMainThreads, NEP_MAIN_MIN_BLOCKS) k_main(SysD
     // ---- network Eq. 21-22 and Fp = dU/dq.  Lane h evaluates neurons mu = h, h+2, ... (two per
     //      iteration for ILP); the partial U and Fp are summed across the pair. ----
     float Fp[Dp];
-#pragma unroll
-    for (int v = 0; v < Dp; ++v) Fp[v] = 0.f;
     const float* b1 = sm + H * Dp;
     const float* w2 = b1 + H;
     float U = h ? 0.f : -w2[H];                                              // - b2 (once)
-    for (int mu = h; mu < H; mu += 4) {
-        const bool two = mu + 2 < H;
-        const int mu1 = two ? mu + 2 : mu;
-        const float4* r0 = reinterpret_cast<const float4*>(sm + mu * Dp);
-        const float4* r1 = reinterpret_cast<const float4*>(sm + mu1 * Dp);
-        float a0 = -b1[mu], a1 = -b1[mu1], a2 = 0.f, a3 = 0.f;
+    {
+        f32x2 qp[Dp / 2], Fpp[Dp / 2];
 #pragma unroll
-        for (int v = 0; v < Dp / 4; ++v) {
-            const float4 w0 = r0[v], w1 = r1[v];
-            a0 = fmaf(w0.x, q[4 * v], a0); a2 = fmaf(w0.y, q[4 * v + 1], a2);
-            a0 = fmaf(w0.z, q[4 * v + 2], a0); a2 = fmaf(w0.w, q[4 * v + 3], a2);
-            a1 = fmaf(w1.x, q[4 * v], a1); a3 = fmaf(w1.y, q[4 * v + 1], a3);
-            a1 = fmaf(w1.z, q[4 * v + 2], a1); a3 = fmaf(w1.w, q[4 * v + 3], a3);
-        }
-        float t0, d0, t1, d1;
-        tanh_sech2(a0 + a2, &t0, &d0);
-        tanh_sech2(a1 + a3, &t1, &d1);
-        const float g0 = w2[mu] * d0, g1 = two ? w2[mu1] * d1 : 0.f;
-        U = fmaf(w2[mu], t0, U);
-        if (two) U = fmaf(w2[mu1], t1, U);
+        for (int v = 0; v < Dp / 2; ++v) { qp[v] = pack2(q[2 * v], q[2 * v + 1]); Fpp[v] = pack2(0.f, 0.f); }
+        for (int mu = h; mu < H; mu += 4) {
+            const bool two = mu + 2 < H;
+            const int mu1 = two ? mu + 2 : mu;
+            const ulonglong2* r0 = reinterpret_cast<const ulonglong2*>(sm + mu * Dp);
+            const ulonglong2* r1 = reinterpret_cast<const ulonglong2*>(sm + mu1 * Dp);
+            f32x2 a0 = pack2(-b1[mu], 0.f), a1 = pack2(-b1[mu1], 0.f), a2 = pack2(0.f, 0.f), a3 = pack2(0.f, 0.f);
 #pragma unroll
-        for (int v = 0; v < Dp / 4; ++v) {
-            const float4 w0 = r0[v], w1 = r1[v];
-            Fp[4 * v] = fmaf(g0, w0.x, fmaf(g1, w1.x, Fp[4 * v]));
-            Fp[4 * v + 1] = fmaf(g0, w0.y, fmaf(g1, w1.y, Fp[4 * v + 1]));
-            Fp[4 * v + 2] = fmaf(g0, w0.z, fmaf(g1, w1.z, Fp[4 * v + 2]));
-            Fp[4 * v + 3] = fmaf(g0, w0.w, fmaf(g1, w1.w, Fp[4 * v + 3]));
+            for (int v = 0; v < Dp / 4; ++v) {
+                const ulonglong2 w0 = r0[v], w1 = r1[v];
+                a0 = ffma2(w0.x, qp[2 * v], a0); a2 = ffma2(w0.y, qp[2 * v + 1], a2);
+                a1 = ffma2(w1.x, qp[2 * v], a1); a3 = ffma2(w1.y, qp[2 * v + 1], a3);
+            }
+            float x0, x1, x2, x3, y0, y1, y2, y3;
+            unpack2(a0, x0, x1); unpack2(a2, x2, x3); unpack2(a1, y0, y1); unpack2(a3, y2, y3);
+            float t0, d0, t1, d1;
+            tanh_sech2((x0 + x1) + (x2 + x3), &t0, &d0);
+            tanh_sech2((y0 + y1) + (y2 + y3), &t1, &d1);
+            const float g0 = w2[mu] * d0, g1 = two ? w2[mu1] * d1 : 0.f;
+            U = fmaf(w2[mu], t0, U);
+            if (two) U = fmaf(w2[mu1], t1, U);
+            const f32x2 g0p = pack2(g0, g0), g1p = pack2(g1, g1);
+#pragma unroll
+            for (int v = 0; v < Dp / 4; ++v) {
+                const ulonglong2 w0 = r0[v], w1 = r1[v];
+                Fpp[2 * v] = ffma2(g0p, w0.x, ffma2(g1p, w1.x, Fpp[2 * v]));
+                Fpp[2 * v + 1] = ffma2(g0p, w0.y, ffma2(g1p, w1.y, Fpp[2 * v + 1]));
+            }
         }
+#pragma unroll
+        for (int v = 0; v < Dp / 2; ++v) unpack2(Fpp[v], Fp[2 * v], Fp[2 * v + 1]);
     }
     U += __shfl_xor_sync(PAIR, U, 1);
 #pragma unroll
@@ -204,6 +233,10 @@ __global__ void __launch_bounds__(kMainThreads, NEP_MAIN_MIN_BLOCKS) k_main(SysD
             const float f1 = (a + NH < NA) ? Fp[NR + 4 * (a + NH < NA ? a + NH : 0) + LOF[m] - 1] : 0.f;
             s[a][m] *= 2.f * C[m] * (h ? f1 : f0);
         }
+#pragma unroll
+    for (int a = 0; a < NH; ++a)
+#pragma unroll
+        for (int mm = 0; mm < NP; ++mm) s2[a][mm] = pack2(s[a][2 * mm], s[a][2 * mm + 1]);
     // ---- partial forces, Eq. 23-25 ----
     float fsx = 0.f, fsy = 0.f, fsz = 0.f;
     float4* prow = d.p + (size_t)i * P.capR;       // p_ij lives at the record's own slot
@@ -237,23 +270,29 @@ __global__ void __launch_bounds__(kMainThreads, NEP_MAIN_MIN_BLOCKS) k_main(SysD
         const float x = e.x * rinv, y = e.y * rinv, z = e.z * rinv;
         float g[NA], dg[NA];
         radial_fn<NA, true>(r2 * rinv, P.rcA_inv, omega(e), g, dg);
-        float Sq[kNumLM], St[kNumLM];
+        f32x2 Sp2[NP], St2[NP];
 #pragma unroll
-        for (int m = 0; m < kNumLM; ++m) { Sq[m] = 0.f; St[m] = 0.f; }
+        for (int mm = 0; mm < NP; ++mm) { Sp2[mm] = pack2(0.f, 0.f); St2[mm] = pack2(0.f, 0.f); }
 #pragma unroll
         for (int a = 0; a < NH; ++a) {
             const int a1 = a + NH < NA ? a + NH : 0;
             const float ga = (h ? (a + NH < NA ? g[a1] : 0.f) : g[a]) * rinv;       // g_n / r
             const float da = h ? (a + NH < NA ? dg[a1] : 0.f) : dg[a];              // g_n'
-            float dl[4];
+            const f32x2 gp = pack2(ga, ga), dp = pack2(da, da);
 #pragma unroll
-            for (int l = 0; l < 4; ++l) dl[l] = fmaf(-(float)(l + 1), ga, da);       // g_n' - l g_n / r
-#pragma unroll
-            for (int m = 0; m < kNumLM; ++m) {
-                Sq[m] = fmaf(s[a][m], dl[LOF[m] - 1], Sq[m]);
-                St[m] = fmaf(s[a][m], ga, St[m]);
+            for (int mm = 0; mm < NP; ++mm) {
+                Sp2[mm] = ffma2(s2[a][mm], dp, Sp2[mm]);
+                St2[mm] = ffma2(s2[a][mm], gp, St2[mm]);
             }
         }
+        float Sq[kNumLM], St[kNumLM];
+#pragma unroll
+        for (int mm = 0; mm < NP; ++mm) {
+            unpack2(Sp2[mm], Sq[2 * mm], Sq[2 * mm + 1]);
+            unpack2(St2[mm], St[2 * mm], St[2 * mm + 1]);
+        }
+#pragma unroll
+        for (int m = 0; m < kNumLM; ++m) Sq[m] = fmaf(-(float)LOF[m], St[m], Sq[m]);   // S' - l S/r
         float px, py, pz;
         ylm_force(x, y, z, Sq, St, &px, &py, &pz);
         px += __shfl_xor_sync(PAIR, px, 1);

@@ -56,7 +56,7 @@ typedef struct {
     int    n_max_radial;    /* 0..15                                                                  */
     int    n_max_angular;   /* 0..15 (kernels are instantiated for n_max_angular+1 in {8, 9})         */
     int    l_max;           /* must be 4 in this build                                                */
-    int    n_neurons;       /* N_neu, single hidden layer (Eq. 21-22), 1..128                         */
+    int    n_neurons;       /* N_neu, single hidden layer (Eq. 21-22), 1..64                          */
     int    n_types;         /* 1..8; >1 switches on the sqrt(Z_i Z_j) weighting of Eq. 19             */
 } nep_hyper;
 

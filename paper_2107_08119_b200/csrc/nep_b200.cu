@@ -63,6 +63,20 @@ struct SysDev {                 // device pointers into the caller's workspace
     int* jrev;                  // [cap_R][N]  j | rev << 24                               (read by k_assemble)
     uint4* masks;               // [N][2] bit s set: Verlet slot s is inside r_c^R ([0]) / r_c^A ([1])
     float4* p;                  // [N][cap_R] partial forces dU_i/dr_ij at the record slots
+    int* order;                 // [ceil(N/256)*256] atoms of each 256-window sorted by neighbour count (-1: none)
+};
+
+constexpr int kMaxH = 64;           // hidden neurons supported by the constant-bank weight block
+constexpr int kMaxD = 45;           // descriptor dimension of the largest instantiation (9 + 9*4)
+constexpr int kMaxW = kMaxH * kMaxD + 2 * kMaxH + 1;
+
+
+// Network parameters, passed by value: they live in the kernel-parameter constant bank, so every
+// weight is a uniform constant operand and costs no shared-memory or L1 traffic.
+// Layout: w1[H][D] row-major | b1[H] | w2[H] | b2 | sqrt(Z_a Z_b)[8][8] at zz.
+struct NetParams {
+    float w[kMaxW];
+    float zz[kMaxTypes * kMaxTypes];
 };
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -74,11 +88,9 @@ enum { PH_KICK = 0, PH_BUILD = 1, PH_FILTER = 2, PH_MAIN = 3, PH_ASSEMBLE = 4, P
 
 struct nep_model {
     nep_hyper h;
-    int D, Dp, NR, NA, H, npar;
+    int D, NR, NA, H, npar;
     int Z[kMaxTypes];
-    float* params_dev;          // staged layout: w1[H][Dp] | b1[H] | w2[H] | b2 | pad, fp32
-    int params_floats;
-    float* sqrtzz_dev;          // [kMaxTypes*kMaxTypes]
+    NetParams net;              // fp32 network parameters + sqrt(Z_a Z_b), passed to k_main by value
 };
 
 struct nep_system {
@@ -381,7 +393,7 @@ __global__ void k_export_lists(SysDev d, int N, int which, int capR, int cap_out
 }
 
 #ifndef NEP_MAIN_MIN_BLOCKS
-#define NEP_MAIN_MIN_BLOCKS 2
+#define NEP_MAIN_MIN_BLOCKS 8
 #endif
 #include "nep_main.cuh"
 #include "fp32_peak.cuh"
@@ -631,6 +643,7 @@ Layout carve(int64_t N, int capR, int capMD, int max_cells, SysDev* d, char* bas
     t.masks = (uint4*)take(n * 32);
     t.xs4 = (double4*)take(n * 32);
     t.p = (float4*)take(n * 16 * capR);
+    t.order = (int*)take(((n + kWin - 1) / kWin) * kWin * 4);
     L.total = o;
     if (d) *d = t;
     return L;
@@ -667,15 +680,16 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
     const nep_model* m = s->model;
     MainParams P;
     P.rcR_inv = (float)(1.0 / m->h.rc_radial); P.rcA_inv = (float)(1.0 / m->h.rc_angular);
-    P.H = m->H; P.N = (int)s->N; P.capR = s->capR; P.capMD = s->capMD;
-    const size_t smem = ((size_t)((m->params_floats + 3) & ~3) + kMaxTypes * kMaxTypes) * sizeof(float) +
-                        (size_t)s->capR * kMainAtoms * (sizeof(float4) + sizeof(float));
+    P.H = m->H; P.N = (int)s->N; P.capR = s->capR;
+    const size_t smem = (size_t)(kRowsS * 32 * 4 + NA * kHalfLM * 32 + (MULTI ? kRowsS * 32 : 0)) * sizeof(float);
     static bool attr_done = false;
     if (!attr_done) {
-        cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                             cudaSharedmemCarveoutMaxShared);
         attr_done = true;
     }
-    k_main<NR, NA, MULTI><<<grid_for(s->N, kMainAtoms), kMainThreads, smem, st>>>(s->d, P, m->params_dev, m->sqrtzz_dev);
+    const int windows = (int)((s->N + kWin - 1) / kWin);
+    k_main<NR, NA, MULTI><<<windows * (kWin / 32), 32, smem, st>>>(s->d, P, m->net);
     s->launches += 1;
 }
 
@@ -694,7 +708,8 @@ void launch_filter(nep_system* s, cudaStream_t st) {
     const nep_hyper& h = s->model->h;
     k_filter<<<grid_for(s->N, 128), 128, 0, st>>>(s->d, (int)s->N, s->box, h.rc_radial * h.rc_radial,
                                                  h.rc_angular * h.rc_angular, s->capR, s->capA, s->capMD);
-    s->launches += 1;
+    k_order<<<(int)((s->N + kWin - 1) / kWin), kWin, 0, st>>>(s->d, (int)s->N);
+    s->launches += 2;
 }
 
 void fill_masses(AsmParams* P, const nep_model* m, const double* mass_by_type) {
@@ -753,7 +768,7 @@ int nep_create(const nep_hyper* hy, const int* atomic_number, const double* para
     if (!(hy->rc_radial > 0.0) || !(hy->rc_angular > 0.0) || hy->rc_angular > hy->rc_radial) return NEP_EINVAL;
     if (hy->n_max_radial < 0 || hy->n_max_radial > 15 || hy->n_max_angular < 0 || hy->n_max_angular > 15) return NEP_EINVAL;
     if (hy->l_max != 4) return NEP_EINVAL;
-    if (hy->n_neurons < 1 || hy->n_neurons > 128) return NEP_EINVAL;
+    if (hy->n_neurons < 1 || hy->n_neurons > kMaxH) return NEP_EINVAL;
     if (hy->n_types < 1 || hy->n_types > kMaxTypes) return NEP_EINVAL;
     if (hy->n_types > 1 && !atomic_number) return NEP_EINVAL;
     nep_model* m = new (std::nothrow) nep_model();
@@ -761,27 +776,15 @@ int nep_create(const nep_hyper* hy, const int* atomic_number, const double* para
     m->h = *hy;
     m->NR = hy->n_max_radial + 1; m->NA = hy->n_max_angular + 1; m->H = hy->n_neurons;
     m->D = m->NR + m->NA * hy->l_max;                    // Eq. 16
-    m->Dp = (m->D + 3) & ~3;
     m->npar = (m->D + 2) * m->H + 1;                     // Eq. 26
     if (n_params != (size_t)m->npar || !main_supported(m)) { delete m; return NEP_EINVAL; }
     if (!device_ok()) { delete m; set_cuda_error(cudaErrorNoDevice, "nep_create"); return NEP_ECUDA; }
     for (int t = 0; t < kMaxTypes; ++t) m->Z[t] = (hy->n_types > 1 && t < hy->n_types) ? atomic_number[t] : 1;
-    // staged fp32 layout: w1[H][Dp] (rows zero-padded) | b1[H] | w2[H] | b2
-    const int H = m->H, D = m->D, Dp = m->Dp;
-    m->params_floats = H * Dp + 2 * H + 1;
-    float* stage = new float[(size_t)m->params_floats + 4]();
-    for (int mu = 0; mu < H; ++mu)
-        for (int v = 0; v < D; ++v) stage[mu * Dp + v] = (float)params[(size_t)mu * D + v];
-    for (int k = 0; k < 2 * H + 1; ++k) stage[H * Dp + k] = (float)params[(size_t)H * D + k];
-    float zz[kMaxTypes * kMaxTypes];
+    // fp32 copy in the caller's order: w1[H][D] | b1[H] | w2[H] | b2   (Eq. 26: N_par floats)
+    memset(&m->net, 0, sizeof(m->net));
+    for (int k = 0; k < m->npar; ++k) m->net.w[k] = (float)params[k];
     for (int a = 0; a < kMaxTypes; ++a)
-        for (int b = 0; b < kMaxTypes; ++b) zz[a * kMaxTypes + b] = (float)sqrt((double)m->Z[a] * (double)m->Z[b]);   // Eq. 19
-    cudaError_t e = cudaMalloc(&m->params_dev, ((size_t)m->params_floats + 4) * sizeof(float));
-    if (e == cudaSuccess) e = cudaMalloc(&m->sqrtzz_dev, sizeof(zz));
-    if (e == cudaSuccess) e = cudaMemcpy(m->params_dev, stage, ((size_t)m->params_floats + 4) * sizeof(float), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(m->sqrtzz_dev, zz, sizeof(zz), cudaMemcpyHostToDevice);
-    delete[] stage;
-    if (e != cudaSuccess) { set_cuda_error(e, "nep_create"); nep_destroy(m); return NEP_ECUDA; }
+        for (int b = 0; b < kMaxTypes; ++b) m->net.zz[a * kMaxTypes + b] = (float)sqrt((double)m->Z[a] * (double)m->Z[b]);   // Eq. 19
     *out = m;
     return NEP_OK;
 }
@@ -791,8 +794,6 @@ int nep_num_params(const nep_model* m) { return m ? m->npar : NEP_EINVAL; }
 
 void nep_destroy(nep_model* m) {
     if (!m) return;
-    if (m->params_dev) cudaFree(m->params_dev);
-    if (m->sqrtzz_dev) cudaFree(m->sqrtzz_dev);
     delete m;
 }
 

@@ -153,6 +153,133 @@ NEP_HD void ylm_force(float x, float y, float z, const float* Sq, const float* S
     *px = fmaf(R, x, vx + wx); *py = fmaf(R, y, vy + wy); *pz = fmaf(R, z, vz + wz);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Half-split forms used by k_main: the 24 lm components are processed in two sequential halves of
+// 12 so that the per-atom sums s[n][lm] of one half fit in registers beside the working set.
+//   half 0: l = 1 (m 0..2)  and l = 4 (m 15..23)        half 1: l = 2 (m 3..7) and l = 3 (m 8..14)
+// Local index k of a half maps to the global component half_m(HALF, k); the polynomials are the
+// same as in ylm_basis / ylm_force above (which stay as the host self-test's reference).
+// ------------------------------------------------------------------------------------------------
+constexpr int kHalfLM = 12;
+
+template <int HALF>
+NEP_HD constexpr int half_m(int k) { return HALF == 0 ? (k < 3 ? k : k + 12) : k + 3; }
+template <int HALF>
+NEP_HD constexpr int half_l(int k) { return HALF == 0 ? (k < 3 ? 1 : 4) : (k < 5 ? 2 : 3); }
+
+template <int HALF>
+NEP_HD void ylm_basis_half(float x, float y, float z, float* b) {
+    const float z2 = z * z;
+    const float c2 = fmaf(x, x, -y * y), xy = x * y, s2 = xy + xy;
+    const float c3 = fmaf(x, c2, -y * s2), s3 = fmaf(x, s2, y * c2);
+    if (HALF == 0) {
+        const float t7 = fmaf(7.f, z2, -3.f), u7 = fmaf(7.f, z2, -1.f);
+        b[0] = x; b[1] = y; b[2] = z;
+        b[3] = fmaf(z2, fmaf(35.f, z2, -30.f), 3.f);
+        b[4] = (x * z) * t7; b[5] = (y * z) * t7;
+        b[6] = c2 * u7; b[7] = s2 * u7;
+        b[8] = z * c3; b[9] = z * s3;
+        b[10] = fmaf(c2, c2, -s2 * s2); b[11] = 2.f * c2 * s2;
+    } else {
+        const float t5 = fmaf(5.f, z2, -1.f);
+        b[0] = fmaf(3.f, z2, -1.f); b[1] = x * z; b[2] = y * z; b[3] = c2; b[4] = s2;
+        b[5] = z * fmaf(5.f, z2, -3.f); b[6] = x * t5; b[7] = y * t5;
+        b[8] = z * c2; b[9] = z * s2; b[10] = c3; b[11] = s3;
+    }
+}
+
+// V = sum_{k in half} St[k] grad B_k(r^)   (the non-radial part of ylm_force restricted to one half)
+template <int HALF>
+NEP_HD void ylm_grad_half(float x, float y, float z, const float* St, float* Vx, float* Vy, float* Vz) {
+    const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y, xz = x * z, yz = y * z;
+    const float c2 = x2 - y2;
+    if (HALF == 0) {
+        const float xyz = xy * z, s2 = xy + xy;
+        const float c3 = fmaf(x, c2, -y * s2), s3 = fmaf(x, s2, y * c2);
+        const float rho2 = x2 + y2;
+        const float q4 = fmaf(-4.f, z2, rho2);            // x^2 + y^2 - 4 z^2
+        const float m6xyz = -6.f * xyz, zc2_3 = 3.f * z * c2;
+        float vx = St[0], vy = St[1], vz = St[2];        // l = 1
+        float wx, wy, wz;                                // l = 4 (second chain)
+        wx = St[3] * (12.f * x * q4); wy = St[3] * (12.f * y * q4);
+        wz = St[3] * (-16.f * z * fmaf(3.f, rho2, -2.f * z2));
+        vx = fmaf(St[4], -z * (fmaf(9.f, x2, 3.f * y2) - 4.f * z2), vx); vy = fmaf(St[4], m6xyz, vy);
+        vz = fmaf(St[4], -3.f * x * q4, vz);
+        wx = fmaf(St[5], m6xyz, wx); wy = fmaf(St[5], -z * (fmaf(3.f, x2, 9.f * y2) - 4.f * z2), wy);
+        wz = fmaf(St[5], -3.f * y * q4, wz);
+        vx = fmaf(St[6], -4.f * x * fmaf(-3.f, z2, x2), vx); vy = fmaf(St[6], 4.f * y * fmaf(-3.f, z2, y2), vy);
+        vz = fmaf(St[6], 12.f * z * c2, vz);
+        wx = fmaf(St[7], -2.f * y * (fmaf(3.f, x2, y2) - 6.f * z2), wx);
+        wy = fmaf(St[7], -2.f * x * (fmaf(3.f, y2, x2) - 6.f * z2), wy); wz = fmaf(St[7], 24.f * xyz, wz);
+        vx = fmaf(St[8], zc2_3, vx); vy = fmaf(St[8], m6xyz, vy); vz = fmaf(St[8], c3, vz);
+        wx = fmaf(St[9], -m6xyz, wx); wy = fmaf(St[9], zc2_3, wy); wz = fmaf(St[9], s3, wz);
+        vx = fmaf(St[10], 4.f * c3, vx); vy = fmaf(St[10], -4.f * s3, vy);
+        wx = fmaf(St[11], 4.f * s3, wx); wy = fmaf(St[11], 4.f * c3, wy);
+        *Vx = vx + wx; *Vy = vy + wy; *Vz = vz + wz;
+    } else {
+        const float rho2 = x2 + y2;
+        float vx, vy, vz, wx, wy, wz;
+        // l = 2
+        vx = St[0] * (-2.f * x); vy = St[0] * (-2.f * y); vz = St[0] * (4.f * z);
+        vx = fmaf(St[1], z, vx); vz = fmaf(St[1], x, vz);
+        vy = fmaf(St[2], z, vy); vz = fmaf(St[2], y, vz);
+        vx = fmaf(St[3], 2.f * x, vx); vy = fmaf(St[3], -2.f * y, vy);
+        vx = fmaf(St[4], 2.f * y, vx); vy = fmaf(St[4], 2.f * x, vy);
+        // l = 3
+        wx = St[5] * (-6.f * xz); wy = St[5] * (-6.f * yz); wz = St[5] * (-3.f * fmaf(-2.f, z2, rho2));
+        wx = fmaf(St[6], fmaf(4.f, z2, -3.f * x2) - y2, wx); wy = fmaf(St[6], -2.f * xy, wy); wz = fmaf(St[6], 8.f * xz, wz);
+        vx = fmaf(St[7], -2.f * xy, vx); vy = fmaf(St[7], fmaf(4.f, z2, -3.f * y2) - x2, vy); vz = fmaf(St[7], 8.f * yz, vz);
+        wx = fmaf(St[8], 2.f * xz, wx); wy = fmaf(St[8], -2.f * yz, wy); wz = fmaf(St[8], c2, wz);
+        vx = fmaf(St[9], 2.f * yz, vx); vy = fmaf(St[9], 2.f * xz, vy); vz = fmaf(St[9], 2.f * xy, vz);
+        wx = fmaf(St[10], 3.f * c2, wx); wy = fmaf(St[10], -6.f * xy, wy);
+        vx = fmaf(St[11], 6.f * xy, vx); vy = fmaf(St[11], 3.f * c2, vy);
+        *Vx = vx + wx; *Vy = vy + wy; *Vz = vz + wz;
+    }
+}
+
+// Radial functions in the two forms k_main consumes (same mathematics as radial_fn):
+//   radial_g :  g_n(r)                                                     (descriptor passes)
+//   radial_gd:  gs_n = g_n(r) * gscale  and  dg_n = dg_n/dr                 (force passes; gscale = 1/r)
+template <int N>
+NEP_HD void radial_g(float r, float rcinv, float omega, float* g) {
+    const float u = r * rcinv, um1 = u - 1.f;
+    const float x2 = fmaf(4.f * um1, um1, -2.f);                       // 2 x
+    float sn, cs;
+    sincos_halfpi(u, &sn, &cs);
+    const float hf = (0.5f * omega) * cs * cs;                         // omega fc / 2
+    float Tm = hf, T = 0.5f * x2 * hf;                                 // hf T_{n-1}, hf T_n (scaled recurrence)
+    g[0] = hf + hf;
+#pragma unroll
+    for (int n = 1; n < N; ++n) {
+        g[n] = T + hf;
+        const float Tn = fmaf(x2, T, -Tm); Tm = T; T = Tn;             // Eq. A1
+    }
+}
+
+template <int N>
+NEP_HD void radial_gd(float r, float rcinv, float omega, float gscale, float* gs, float* dg) {
+    const float u = r * rcinv, um1 = u - 1.f;
+    const float x2 = fmaf(4.f * um1, um1, -2.f);                       // 2 x
+    float sn, cs;
+    sincos_halfpi(u, &sn, &cs);
+    const float ho = 0.5f * omega;
+    const float hf = ho * cs * cs;                                     // omega fc / 2
+    const float hb = (-3.14159265358979f * rcinv * ho) * sn * cs;      // omega fc' / 2
+    const float ha = hf * 4.f * um1 * rcinv;                           // omega fc x' / 2
+    const float hs = hf * gscale;
+    float Tm = 1.f, T = 0.5f * x2;                                     // T_{n-1}, T_n
+    float Um = 0.f, U = ha;                                            // ha U_{n-2}, ha U_{n-1}
+    gs[0] = hs + hs;
+    dg[0] = hb + hb;
+#pragma unroll
+    for (int n = 1; n < N; ++n) {
+        gs[n] = fmaf(hs, T, hs);
+        dg[n] = fmaf((float)n, U, fmaf(hb, T, hb));                    // Eq. A2: n U_{n-1} x' fc + (T_n + 1) fc'
+        const float Tn = fmaf(x2, T, -Tm); Tm = T; T = Tn;             // Eq. A1
+        const float Un = fmaf(x2, U, -Um); Um = U; U = Un;             // Eq. A3 (scaled by ha)
+    }
+}
+
 // t = tanh(a), d = 1 - tanh^2(a) = 4 e / (1 + e)^2 with e = exp(-2|a|): no cancellation when |t| -> 1.
 NEP_HD void tanh_sech2(float a, float* t, float* d) {
     const float e = expf(-2.f * fabsf(a));

@@ -78,6 +78,38 @@ int main() {
         float t, d; tanh_sech2((float)a, &t, &d);
         if (fabs(t - tanh(a)) > 2e-7 || fabs(d - 1 / (cosh((double)(float)a) * cosh((double)(float)a))) > 2e-6 * (1 / (cosh(a)*cosh(a))) + 1e-30) { printf("tanh %g\n", a); ++fails; }
     }
+    // 5. half-split forms == the full forms (basis slices, gradient halves, radial_g / radial_gd)
+    for (int t = 0; t < 200; ++t) {
+        double u[3]; unit(u);
+        const float x = (float)u[0], y = (float)u[1], z = (float)u[2];
+        float b[kNumLM], h0[kHalfLM], h1[kHalfLM], St[kNumLM], Sq[kNumLM], zero[kNumLM] = {0};
+        ylm_basis(x, y, z, b);
+        ylm_basis_half<0>(x, y, z, h0);
+        ylm_basis_half<1>(x, y, z, h1);
+        for (int k = 0; k < kHalfLM; ++k) {
+            if (fabs(h0[k] - b[half_m<0>(k)]) > 2e-6) { printf("basis half0 %d\n", k); ++fails; }
+            if (fabs(h1[k] - b[half_m<1>(k)]) > 2e-6) { printf("basis half1 %d\n", k); ++fails; }
+            if (half_l<0>(k) != lof[half_m<0>(k)] || half_l<1>(k) != lof[half_m<1>(k)]) { printf("half_l %d\n", k); ++fails; }
+        }
+        for (int m = 0; m < kNumLM; ++m) { St[m] = (float)(2 * urand() - 1); Sq[m] = 0.f; }
+        float px, py, pz, ax, ay, az, bx, by, bz, S0[kHalfLM], S1[kHalfLM];
+        ylm_force(x, y, z, zero, St, &px, &py, &pz);          // Sq = 0: only V
+        for (int k = 0; k < kHalfLM; ++k) { S0[k] = St[half_m<0>(k)]; S1[k] = St[half_m<1>(k)]; }
+        ylm_grad_half<0>(x, y, z, S0, &ax, &ay, &az);
+        ylm_grad_half<1>(x, y, z, S1, &bx, &by, &bz);
+        if (fabs(ax + bx - px) > 2e-5 || fabs(ay + by - py) > 2e-5 || fabs(az + bz - pz) > 2e-5) {
+            printf("grad halves: %g %g %g vs %g %g %g\n", ax + bx, ay + by, az + bz, px, py, pz); ++fails; }
+        const double rc = 4.0 + urand() * 2, r = 0.3 + urand() * (rc - 0.35), om = 1 + 60 * urand();
+        float g[9], dg[9], g2[9], gs[9], dg2[9];
+        radial_fn<9, true>((float)r, (float)(1 / rc), (float)om, g, dg);
+        radial_g<9>((float)r, (float)(1 / rc), (float)om, g2);
+        radial_gd<9>((float)r, (float)(1 / rc), (float)om, (float)(1 / r), gs, dg2);
+        for (int n = 0; n < 9; ++n) {
+            if (fabs(g2[n] - g[n]) > 2e-6 * om) { printf("radial_g[%d] %g vs %g\n", n, g2[n], g[n]); ++fails; }
+            if (fabs(gs[n] * r - g[n]) > 2e-6 * om) { printf("radial_gd gs[%d] %g vs %g\n", n, gs[n] * r, g[n]); ++fails; }
+            if (fabs(dg2[n] - dg[n]) > 2e-5 * om) { printf("radial_gd dg[%d] %g vs %g\n", n, dg2[n], dg[n]); ++fails; }
+        }
+    }
     printf(fails ? "FAILED %d\n" : "OK\n", fails);
     return fails ? 1 : 0;
 }

@@ -63,19 +63,15 @@ struct SysDev {                 // device pointers into the caller's workspace
     int* jrev;                  // [cap_R][N]  j | rev << 24                               (read by k_assemble)
     uint4* masks;               // [N][2] bit s set: Verlet slot s is inside r_c^R ([0]) / r_c^A ([1])
     float4* p;                  // [N][cap_R] partial forces dU_i/dr_ij at the record slots
+    float2* spark0;             // [NA*6][ceil(N/256)*256] angular sums s[n][lm] of lm half 0 / half 1: parked here by k_main
+    float2* spark1;             //   (coalesced rows, L2-resident between write and read) while the registers hold other phases
     int* order;                 // [ceil(N/256)*256] atoms of each 256-window sorted by neighbour count (-1: none)
 };
 
-constexpr int kMaxH = 64;           // hidden neurons supported by the constant-bank weight block
-constexpr int kMaxD = 45;           // descriptor dimension of the largest instantiation (9 + 9*4)
-constexpr int kMaxW = kMaxH * kMaxD + 2 * kMaxH + 1;
+constexpr int kMaxH = 64;           // hidden neurons supported (weights are staged in shared memory by k_main)
 
-
-// Network parameters, passed by value: they live in the kernel-parameter constant bank, so every
-// weight is a uniform constant operand and costs no shared-memory or L1 traffic.
-// Layout: w1[H][D] row-major | b1[H] | w2[H] | b2 | sqrt(Z_a Z_b)[8][8] at zz.
-struct NetParams {
-    float w[kMaxW];
+// sqrt(Z_a Z_b) of Eq. 19, passed to k_main by value (kernel-parameter constant bank)
+struct ZZParams {
     float zz[kMaxTypes * kMaxTypes];
 };
 
@@ -90,7 +86,9 @@ struct nep_model {
     nep_hyper h;
     int D, NR, NA, H, npar;
     int Z[kMaxTypes];
-    NetParams net;              // fp32 network parameters + sqrt(Z_a Z_b), passed to k_main by value
+    float* params_dev;          // staged fp32 layout: w1[H][Dp] (rows zero-padded) | b1[H] | w2[H] | b2 | pad
+    int params_floats;
+    ZZParams zz;
 };
 
 struct nep_system {
@@ -393,7 +391,7 @@ __global__ void k_export_lists(SysDev d, int N, int which, int capR, int cap_out
 }
 
 #ifndef NEP_MAIN_MIN_BLOCKS
-#define NEP_MAIN_MIN_BLOCKS 8
+#define NEP_MAIN_MIN_BLOCKS 4
 #endif
 #include "nep_main.cuh"
 #include "fp32_peak.cuh"
@@ -613,7 +611,7 @@ struct Layout {
 };
 
 // carve the workspace; the same routine sizes it (base == nullptr)
-Layout carve(int64_t N, int capR, int capMD, int max_cells, SysDev* d, char* base) {
+Layout carve(int64_t N, int capR, int capMD, int max_cells, int NA, SysDev* d, char* base) {
     Layout L; size_t o = 0; int k = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align256(o + bytes); L.off[k++] = at; return base ? base + at : nullptr; };
     const size_t n = (size_t)N;
@@ -644,6 +642,8 @@ Layout carve(int64_t N, int capR, int capMD, int max_cells, SysDev* d, char* bas
     t.xs4 = (double4*)take(n * 32);
     t.p = (float4*)take(n * 16 * capR);
     t.order = (int*)take(((n + kWin - 1) / kWin) * kWin * 4);
+    t.spark0 = (float2*)take(((n + kWin - 1) / kWin) * kWin * 8 * (size_t)(NA * kHalfLM / 2));
+    t.spark1 = (float2*)take(((n + kWin - 1) / kWin) * kWin * 8 * (size_t)(NA * kHalfLM / 2));
     L.total = o;
     if (d) *d = t;
     return L;
@@ -681,27 +681,32 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
     MainParams P;
     P.rcR_inv = (float)(1.0 / m->h.rc_radial); P.rcA_inv = (float)(1.0 / m->h.rc_angular);
     P.H = m->H; P.N = (int)s->N; P.capR = s->capR;
-    const size_t smem = (size_t)(kRowsS * 32 * 4 + NA * kHalfLM * 32 + (MULTI ? kRowsS * 32 : 0)) * sizeof(float);
+    const size_t smem = ((size_t)m->params_floats + kMainWarps * main_warp_floats<NA, MULTI>()) * sizeof(float);
     static bool attr_done = false;
     if (!attr_done) {
+        cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
         cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributePreferredSharedMemoryCarveout,
                              cudaSharedmemCarveoutMaxShared);
         attr_done = true;
     }
     const int windows = (int)((s->N + kWin - 1) / kWin);
-    k_main<NR, NA, MULTI><<<windows * (kWin / 32), 32, smem, st>>>(s->d, P, m->net);
+    k_main<NR, NA, MULTI><<<windows * (kWin / (32 * kMainWarps)), 32 * kMainWarps, smem, st>>>(s->d, P, m->params_dev, m->zz);
     s->launches += 1;
 }
 
 bool main_supported(const nep_model* m) {
-    return (m->NR == 8 && m->NA == 8) || (m->NR == 9 && m->NA == 9);
+    return ((m->NR == 8 && m->NA == 8) || (m->NR == 9 && m->NA == 9)) && m->H <= kMaxH;
 }
 
 void launch_main(nep_system* s, cudaStream_t st) {
     const nep_model* m = s->model;
     const bool multi = m->h.n_types > 1;
+#ifdef NEP_FAST_BUILD            // kernel experiments: one instantiation only
+    launch_main_t<8, 8, false>(s, st);
+#else
     if (m->NR == 8 && m->NA == 8) { if (multi) launch_main_t<8, 8, true>(s, st); else launch_main_t<8, 8, false>(s, st); }
     else if (m->NR == 9 && m->NA == 9) { if (multi) launch_main_t<9, 9, true>(s, st); else launch_main_t<9, 9, false>(s, st); }
+#endif
 }
 
 void launch_filter(nep_system* s, cudaStream_t st) {
@@ -780,11 +785,19 @@ int nep_create(const nep_hyper* hy, const int* atomic_number, const double* para
     if (n_params != (size_t)m->npar || !main_supported(m)) { delete m; return NEP_EINVAL; }
     if (!device_ok()) { delete m; set_cuda_error(cudaErrorNoDevice, "nep_create"); return NEP_ECUDA; }
     for (int t = 0; t < kMaxTypes; ++t) m->Z[t] = (hy->n_types > 1 && t < hy->n_types) ? atomic_number[t] : 1;
-    // fp32 copy in the caller's order: w1[H][D] | b1[H] | w2[H] | b2   (Eq. 26: N_par floats)
-    memset(&m->net, 0, sizeof(m->net));
-    for (int k = 0; k < m->npar; ++k) m->net.w[k] = (float)params[k];
+    // staged fp32 layout: w1[H][Dp] (rows zero-padded to a multiple of 4) | b1[H] | w2[H] | b2
+    const int H = m->H, D = m->D, Dp = (D + 3) & ~3;
+    m->params_floats = (H * Dp + 2 * H + 1 + 3) & ~3;
+    float* stage = new float[(size_t)m->params_floats]();
+    for (int mu = 0; mu < H; ++mu)
+        for (int v = 0; v < D; ++v) stage[mu * Dp + v] = (float)params[(size_t)mu * D + v];
+    for (int k = 0; k < 2 * H + 1; ++k) stage[H * Dp + k] = (float)params[(size_t)H * D + k];
     for (int a = 0; a < kMaxTypes; ++a)
-        for (int b = 0; b < kMaxTypes; ++b) m->net.zz[a * kMaxTypes + b] = (float)sqrt((double)m->Z[a] * (double)m->Z[b]);   // Eq. 19
+        for (int b = 0; b < kMaxTypes; ++b) m->zz.zz[a * kMaxTypes + b] = (float)sqrt((double)m->Z[a] * (double)m->Z[b]);   // Eq. 19
+    cudaError_t e = cudaMalloc(&m->params_dev, (size_t)m->params_floats * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemcpy(m->params_dev, stage, (size_t)m->params_floats * sizeof(float), cudaMemcpyHostToDevice);
+    delete[] stage;
+    if (e != cudaSuccess) { set_cuda_error(e, "nep_create"); nep_destroy(m); return NEP_ECUDA; }
     *out = m;
     return NEP_OK;
 }
@@ -794,6 +807,7 @@ int nep_num_params(const nep_model* m) { return m ? m->npar : NEP_EINVAL; }
 
 void nep_destroy(nep_model* m) {
     if (!m) return;
+    if (m->params_dev) cudaFree(m->params_dev);
     delete m;
 }
 
@@ -801,7 +815,7 @@ size_t nep_workspace_bytes(const nep_model* m, int64_t n_atoms, int cap_radial, 
     if (!m || n_atoms < 1 || n_atoms >= (1 << 24) || cap_radial < 1 || cap_radial > 124 || cap_angular < 1 ||
         cap_angular > cap_radial || !(skin >= 0.0))
         return 0;
-    return carve(n_atoms, cap_radial, cap_md_of(m, cap_radial, skin), max_cells_of(n_atoms), nullptr, nullptr).total;
+    return carve(n_atoms, cap_radial, cap_md_of(m, cap_radial, skin), max_cells_of(n_atoms), m->NA, nullptr, nullptr).total;
 }
 
 int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, int cap_radial, int cap_angular,
@@ -816,7 +830,7 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
     s->model = m; s->N = n_atoms; s->capR = cap_radial; s->capA = cap_angular; s->skin = skin;
     s->capMD = cap_md_of(m, cap_radial, skin);
     s->max_cells = max_cells_of(n_atoms);
-    carve(n_atoms, s->capR, s->capMD, s->max_cells, &s->d, (char*)workspace_dev);
+    carve(n_atoms, s->capR, s->capMD, s->max_cells, m->NA, &s->d, (char*)workspace_dev);
     s->built = false; s->have_forces = false; s->last_stream = nullptr; s->step_graph = nullptr;
     s->launches = 0; s->prof_on = false; s->prof_n = 0;
     for (int k = 0; k < NEP_PHASES; ++k) { s->prof_ms[k] = 0.0; s->prof_cnt[k] = 0; }

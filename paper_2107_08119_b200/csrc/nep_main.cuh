@@ -15,6 +15,7 @@
 #pragma once
 
 constexpr int kRowsS = 24;          // angular neighbour rows staged in shared memory (more: read from global)
+constexpr int kRowsO = 20;          // radial-only neighbour rows staged in shared memory (more: read from global)
 constexpr int kWin = 256;           // k_order's sort window (atoms)
 struct MainParams {
     float rcR_inv, rcA_inv;
@@ -177,26 +178,54 @@ __device__ __forceinline__ void force_half(const f32x2 (&A2)[NA][kHalfLM / 2], f
     px = fmaf(R, x, vx); py = fmaf(R, y, vy); pz = fmaf(R, z, vz);
 }
 
+constexpr int kMainWarps = 2;       // independent warps per block; they share only the staged weights
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+// floats of shared memory: staged weights, then one region per warp
+__host__ __device__ constexpr int main_wfloats(int H, int Dp) { return (H * Dp + 2 * H + 1 + 3) & ~3; }
+template <int NA, bool MULTI>
+__host__ __device__ constexpr int main_warp_floats() { return (kRowsS + kRowsO) * 32 * 4 + (MULTI ? kRowsS * 32 : 0); }
+
 template <int NR, int NA, bool MULTI>
-__global__ void __launch_bounds__(32, NEP_MAIN_MIN_BLOCKS) k_main(SysDev d, MainParams P,
-                                                                 const __grid_constant__ NetParams W) {
+__global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(SysDev d, MainParams P,
+                                                                              const float* __restrict__ params,
+                                                                              const __grid_constant__ ZZParams Z) {
     constexpr int D = NR + 4 * NA;
+    constexpr int Dp = (D + 3) & ~3;
     constexpr int NP = kHalfLM / 2;
     extern __shared__ __align__(16) float sm[];
-    float4* srec = reinterpret_cast<float4*>(sm);                      // [kRowsS][32] {r^_ij, r_ij} of angular neighbours
-    float2* spark = reinterpret_cast<float2*>(sm + kRowsS * 32 * 4);   // [NA*6][32] parked s (half 0)
-    float* som = sm + kRowsS * 32 * 4 + NA * kHalfLM * 32;            // [kRowsS][32] omega_ij (MULTI only)
+    const int H = P.H;
+    const int wfl = main_wfloats(H, Dp);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float* wsm = sm + wfl + warp * main_warp_floats<NA, MULTI>();
+    float4* srec = reinterpret_cast<float4*>(wsm);                     // [kRowsS][32] angular neighbours: raw, then {r^_ij, r_ij}
+    float4* praw = srec + kRowsS * 32;                                 // [kRowsO][32] radial-only neighbours, raw records
+    float* som = wsm + (kRowsS + kRowsO) * 32 * 4;                     // [kRowsS][32] omega_ij (MULTI only)
 
-    const int lane = threadIdx.x;
     const int N = P.N;
-    const int i_ord = d.order[blockIdx.x * 32 + lane];
+    const int i_ord = d.order[(blockIdx.x * kMainWarps + warp) * 32 + lane];
     const bool active = i_ord >= 0;
     const int i = active ? i_ord : 0;
     const int nR = active ? d.nnR[i] : 0, nA = active ? d.nnA[i] : 0;
     const int nO = nR - nA;
     const float4* grec = d.rec + i;                  // record of slot s: grec[(size_t)s * N]
-    const float* zrow = W.zz + (MULTI ? d.type_s[i] * kMaxTypes : 0);
+    const float* zrow = Z.zz + (MULTI ? d.type_s[i] * kMaxTypes : 0);
     auto omega_of = [&](const float4& e) { return MULTI ? zrow[__float_as_int(e.w) & (kMaxTypes - 1)] : 1.f; };
+
+    // ---- P0: every neighbour record of the atom in flight at once (cp.async), weights staged meanwhile ----
+    {
+        const int ka = min(nA, kRowsS), ko = min(nO, kRowsO);
+        for (int k = 0; k < ka; ++k) cp_async16(&srec[k * 32 + lane], &grec[(size_t)k * N]);
+        for (int o = 0; o < ko; ++o) cp_async16(&praw[o * 32 + lane], &grec[(size_t)(P.capR - 1 - o) * N]);
+        for (int k = threadIdx.x; k < wfl / 4; k += 32 * kMainWarps) cp_async16(sm + 4 * k, params + 4 * k);
+        cp_async_wait_all();
+        __syncthreads();
+    }
 
     // neighbour k (an angular one) as unit vector, distance and Eq. 19 weight
     auto load_nbr = [&](int k, float& x, float& y, float& z, float& r, float& om) {
@@ -213,104 +242,135 @@ __global__ void __launch_bounds__(32, NEP_MAIN_MIN_BLOCKS) k_main(SysDev d, Main
         }
     };
 
-    // ---- P1: radial descriptor, Eq. 12; stages the angular neighbours ----
-    float q[D];
+    // ---- P1: radial descriptor, Eq. 12; the angular neighbours are left normalised in shared memory ----
+    float q[Dp];
 #pragma unroll
-    for (int v = 0; v < D; ++v) q[v] = 0.f;
-    for (int k0 = 0; k0 < nR; k0 += 4) {
-        float4 e[4];
+    for (int v = 0; v < Dp; ++v) q[v] = 0.f;
+    auto radial_acc = [&](const float4& e, bool on, float& rinv, float& r, float& om) {
+        const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+        rinv = inv_norm(r2);
+        r = r2 * rinv;
+        om = omega_of(e);
+        float g[NR];
+        radial_g<NR>(r, P.rcR_inv, on ? om : 0.f, g);
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int kk = min(k0 + u, nR - 1);
-            const int slot = kk < nA ? kk : P.capR - 1 - (kk - nA);
-            e[u] = __ldg(&grec[(size_t)slot * N]);
+        for (int n = 0; n < NR; ++n) q[n] += g[n];
+    };
+    for (int k = 0; k < nA; k += 2) {                // two neighbours per iteration: independent chains
+        const int k1 = min(k + 1, nA - 1);
+        const float4 e0 = k < kRowsS ? srec[k * 32 + lane] : grec[(size_t)k * N];
+        const float4 e1 = k1 < kRowsS ? srec[k1 * 32 + lane] : grec[(size_t)k1 * N];
+        float ri0, r0, om0, ri1, r1, om1;
+        radial_acc(e0, true, ri0, r0, om0);
+        radial_acc(e1, k + 1 < nA, ri1, r1, om1);
+        if (k < kRowsS) {
+            srec[k * 32 + lane] = make_float4(e0.x * ri0, e0.y * ri0, e0.z * ri0, r0);
+            if (MULTI) som[k * 32 + lane] = om0;
         }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const int kk = k0 + u;
-            if (kk < nR) {
-                const float r2 = e[u].x * e[u].x + e[u].y * e[u].y + e[u].z * e[u].z;
-                const float rinv = inv_norm(r2);
-                const float r = r2 * rinv;
-                const float om = omega_of(e[u]);
-                float g[NR];
-                radial_g<NR>(r, P.rcR_inv, om, g);
-#pragma unroll
-                for (int n = 0; n < NR; ++n) q[n] += g[n];
-                if (kk < nA && kk < kRowsS) {
-                    srec[kk * 32 + lane] = make_float4(e[u].x * rinv, e[u].y * rinv, e[u].z * rinv, r);
-                    if (MULTI) som[kk * 32 + lane] = om;
-                }
-            }
+        if (k1 < kRowsS) {                           // k1 == k at a ragged end: rewrites the same values' source
+            if (k1 != k) srec[k1 * 32 + lane] = make_float4(e1.x * ri1, e1.y * ri1, e1.z * ri1, r1);
+            if (MULTI) som[k1 * 32 + lane] = om1;
         }
+    }
+    auto raw_only = [&](int o) { return o < kRowsO ? praw[o * 32 + lane] : grec[(size_t)(P.capR - 1 - o) * N]; };
+    for (int o = 0; o < nO; o += 2) {
+        const int o1 = min(o + 1, nO - 1);
+        const float4 e0 = raw_only(o), e1 = raw_only(o1);
+        float ri, r, om;
+        radial_acc(e0, true, ri, r, om);
+        radial_acc(e1, o + 1 < nO, ri, r, om);
     }
 
     // ---- P2: angular sums, half 0 (parked in shared memory) then half 1 (stays in registers) ----
+    // A finished half leaves the registers for coalesced rows of spark0 / spark1 (written and read by the
+    // same thread a few microseconds apart: L2 traffic) while other phases need them.
     f32x2 s2[NA][NP];
+    const size_t npad = (size_t)gridDim.x * (32 * kMainWarps);
+    const size_t gcol = (size_t)(blockIdx.x * kMainWarps + warp) * 32 + lane;
+    auto park = [&](float2* base) {
+#pragma unroll
+        for (int n = 0; n < NA; ++n)
+#pragma unroll
+            for (int mm = 0; mm < NP; ++mm) {
+                float s0, s1;
+                unpack2(s2[n][mm], s0, s1);
+                base[(size_t)(n * NP + mm) * npad + gcol] = make_float2(s0, s1);
+            }
+    };
+    auto unpark = [&](const float2* base) {
+#pragma unroll
+        for (int n = 0; n < NA; ++n)
+#pragma unroll
+            for (int mm = 0; mm < NP; ++mm) {
+                const float2 v = base[(size_t)(n * NP + mm) * npad + gcol];
+                s2[n][mm] = pack2(v.x, v.y);
+            }
+    };
     desc_half<0, NR, NA>(nA, P.rcA_inv, load_nbr, s2, q);
-#pragma unroll
-    for (int n = 0; n < NA; ++n)
-#pragma unroll
-        for (int mm = 0; mm < NP; ++mm) {
-            float s0, s1;
-            unpack2(s2[n][mm], s0, s1);
-            spark[(n * NP + mm) * 32 + lane] = make_float2(s0, s1);
-        }
+    park(d.spark0);
     desc_half<1, NR, NA>(nA, P.rcA_inv, load_nbr, s2, q);
+    park(d.spark1);
 
-    // ---- P3: network Eq. 21-22 (minus biases) and Fp = dU/dq; two neurons per iteration ----
-    float Fp[D];
+    // ---- P3: network Eq. 21-22 (minus biases) and Fp = dU/dq; two neurons per iteration, weight rows
+    //      read from shared memory as warp-wide broadcasts (staged layout w1[H][Dp] | b1[H] | w2[H] | b2) ----
+    float Fp[Dp];
 #pragma unroll
-    for (int v = 0; v < D; ++v) Fp[v] = 0.f;
-    const int H = P.H;
-    const float* b1 = W.w + H * D;
+    for (int v = 0; v < Dp; ++v) Fp[v] = 0.f;
+    const float* b1 = sm + H * Dp;
     const float* w2 = b1 + H;
     float U = -w2[H];                                                   // - b2
     for (int mu = 0; mu < H; mu += 2) {
         const bool two = mu + 1 < H;
         const int mu1 = two ? mu + 1 : mu;
-        const float* r0 = W.w + mu * D;
-        const float* r1 = W.w + mu1 * D;
+        const float4* r0 = reinterpret_cast<const float4*>(sm + mu * Dp);
+        const float4* r1 = reinterpret_cast<const float4*>(sm + mu1 * Dp);
         float a0 = -b1[mu], a1 = 0.f, c0 = -b1[mu1], c1 = 0.f;
 #pragma unroll
-        for (int v = 0; v + 1 < D; v += 2) {
-            a0 = fmaf(r0[v], q[v], a0); a1 = fmaf(r0[v + 1], q[v + 1], a1);
-            c0 = fmaf(r1[v], q[v], c0); c1 = fmaf(r1[v + 1], q[v + 1], c1);
+        for (int v = 0; v < Dp / 4; ++v) {
+            const float4 x = r0[v], y = r1[v];
+            a0 = fmaf(x.x, q[4 * v], a0); a1 = fmaf(x.y, q[4 * v + 1], a1); a0 = fmaf(x.z, q[4 * v + 2], a0); a1 = fmaf(x.w, q[4 * v + 3], a1);
+            c0 = fmaf(y.x, q[4 * v], c0); c1 = fmaf(y.y, q[4 * v + 1], c1); c0 = fmaf(y.z, q[4 * v + 2], c0); c1 = fmaf(y.w, q[4 * v + 3], c1);
         }
-        if (D & 1) { a0 = fmaf(r0[D - 1], q[D - 1], a0); c0 = fmaf(r1[D - 1], q[D - 1], c0); }
         float t0, d0, t1, d1;
         tanh_sech2(a0 + a1, &t0, &d0);
         tanh_sech2(c0 + c1, &t1, &d1);
-        const float g0 = w2[mu] * d0, g1 = two ? w2[mu1] * d1 : 0.f;
-        U = fmaf(w2[mu], t0, U);
-        if (two) U = fmaf(w2[mu1], t1, U);
+        const float w20 = w2[mu], w21 = two ? w2[mu1] : 0.f;
+        const float g0 = w20 * d0, g1 = w21 * d1;
+        U = fmaf(w20, t0, fmaf(w21, t1, U));
 #pragma unroll
-        for (int v = 0; v < D; ++v) Fp[v] = fmaf(g0, r0[v], fmaf(g1, r1[v], Fp[v]));
+        for (int v = 0; v < Dp / 4; ++v) {
+            const float4 x = r0[v], y = r1[v];
+            Fp[4 * v] = fmaf(g0, x.x, fmaf(g1, y.x, Fp[4 * v]));
+            Fp[4 * v + 1] = fmaf(g0, x.y, fmaf(g1, y.y, Fp[4 * v + 1]));
+            Fp[4 * v + 2] = fmaf(g0, x.z, fmaf(g1, y.z, Fp[4 * v + 2]));
+            Fp[4 * v + 3] = fmaf(g0, x.w, fmaf(g1, y.w, Fp[4 * v + 3]));
+        }
     }
     if (active) d.Us[i] = U;
+
+    unpark(d.spark1);                                // half 1 comes back; its loads are in flight while P4 runs
 
     // ---- P4: radial-only neighbours, Eq. 24 ----
     float fsx = 0.f, fsy = 0.f, fsz = 0.f;
     float4* prow = d.p + (size_t)i * P.capR;         // p_ij lives at the record's own slot
-    for (int k0 = 0; k0 < nO; k0 += 4) {
-        float4 e[4];
+    for (int o = 0; o < nO; o += 2) {                // two neighbours per iteration: independent chains
 #pragma unroll
-        for (int u = 0; u < 4; ++u) e[u] = __ldg(&grec[(size_t)(P.capR - 1 - min(k0 + u, nO - 1)) * N]);
+        for (int u = 0; u < 2; ++u) {
+            const int oo = min(o + u, nO - 1);
+            const float4 e = raw_only(oo);
+            const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
+            const float rinv = inv_norm(r2);
+            float gs[NR], dg[NR];
+            radial_gd<NR>(r2 * rinv, P.rcR_inv, omega_of(e), 1.f, gs, dg);
+            float c0 = 0.f, c1 = 0.f;
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            if (k0 + u < nO) {
-                const float r2 = e[u].x * e[u].x + e[u].y * e[u].y + e[u].z * e[u].z;
-                const float rinv = inv_norm(r2);
-                float gs[NR], dg[NR];
-                radial_gd<NR>(r2 * rinv, P.rcR_inv, omega_of(e[u]), 1.f, gs, dg);
-                float c0 = 0.f, c1 = 0.f;
-#pragma unroll
-                for (int n = 0; n + 1 < NR; n += 2) { c0 = fmaf(Fp[n], dg[n], c0); c1 = fmaf(Fp[n + 1], dg[n + 1], c1); }
-                if (NR & 1) c0 = fmaf(Fp[NR - 1], dg[NR - 1], c0);
-                const float c = (c0 + c1) * rinv;
-                const float px = c * e[u].x, py = c * e[u].y, pz = c * e[u].z;
+            for (int n = 0; n + 1 < NR; n += 2) { c0 = fmaf(Fp[n], dg[n], c0); c1 = fmaf(Fp[n + 1], dg[n + 1], c1); }
+            if (NR & 1) c0 = fmaf(Fp[NR - 1], dg[NR - 1], c0);
+            const float c = (c0 + c1) * rinv;
+            const float px = c * e.x, py = c * e.y, pz = c * e.z;
+            if (o + u < nO) {
                 fsx += px; fsy += py; fsz += pz;
-                prow[P.capR - 1 - (k0 + u)] = make_float4(px, py, pz, 0.f);
+                prow[P.capR - 1 - oo] = make_float4(px, py, pz, 0.f);
             }
         }
     }
@@ -332,18 +392,14 @@ __global__ void __launch_bounds__(32, NEP_MAIN_MIN_BLOCKS) k_main(SysDev d, Main
         for (int n = 0; n + 1 < NR; n += 2) { c0 = fmaf(Fp[n], dR[n], c0); c1 = fmaf(Fp[n + 1], dR[n + 1], c1); }
         if (NR & 1) c0 = fmaf(Fp[NR - 1], dR[NR - 1], c0);
         const float c = c0 + c1;
-        prow[k] = make_float4(fmaf(c, x, px), fmaf(c, y, py), fmaf(c, z, pz), 0.f);
+        // half 1's share waits for half 0 in the (now free) radial-only rows of shared memory
+        const float4 ph = make_float4(fmaf(c, x, px), fmaf(c, y, py), fmaf(c, z, pz), 0.f);
+        if (k < kRowsO) praw[k * 32 + lane] = ph; else prow[k] = ph;
     }
-#pragma unroll
-    for (int n = 0; n < NA; ++n)
-#pragma unroll
-        for (int mm = 0; mm < NP; ++mm) {
-            const float2 v = spark[(n * NP + mm) * 32 + lane];
-            s2[n][mm] = pack2(v.x, v.y);
-        }
+    unpark(d.spark0);
     scale_half<0, NR, NA>(s2, Fp);
     for (int k = 0; k < nA; ++k) {
-        const float4 pold = prow[k];                 // half 1's share (this thread wrote it above)
+        const float4 pold = k < kRowsO ? praw[k * 32 + lane] : prow[k];
         float x, y, z, r, om;
         load_nbr(k, x, y, z, r, om);
         const float rinv = fast_rcp(r);

@@ -1,17 +1,21 @@
 // nep_main.cuh -- k_main: descriptor + network + partial forces (included by nep_b200.cu inside its
 // anonymous namespace, after SysDev and nep_math.cuh).
 //
-// One thread per atom, one warp per block.  k_order sorts every window of 256 atoms by neighbour
-// count, so the 32 atoms of a warp have (nearly) equal trip counts and the hardware block scheduler
-// balances the windows' light and heavy warps.  Per atom, in order:
-//   P1  radial descriptor q_n (Eq. 12) over all r < r_c^R neighbours, read once from global memory;
-//       the angular neighbours are left in shared memory as {r^_ij, r_ij}
+// One thread per atom; a block is two independent warps that share only the staged network weights.
+// k_order sorts every window of 256 atoms by neighbour count, so the 32 atoms of a warp have (nearly)
+// equal trip counts and the hardware block scheduler balances the windows' light and heavy blocks.
+// Per atom, in order:
+//   P0  all neighbour records of the atom (cp.async, every row in flight at once) and the weights
+//       (once per block) are staged in shared memory
+//   P1  radial descriptor q_n (Eq. 12) over all r < r_c^R neighbours; the angular neighbours are left
+//       in shared memory as {r^_ij, r_ij}
 //   P2  angular sums s[n][lm] = sum_j g_n(r_ij) b_lm(r^_ij) (Eq. 17-18 route to Eq. 13) in two halves of
-//       12 lm (96 register accumulators each); half 0 is parked in shared memory
-//   P3  network (Eq. 21-22) and Fp = dU/dq, weights read from the kernel-parameter constant bank
+//       12 lm (96 register accumulators each); a finished half is parked in coalesced, L2-resident rows
+//   P3  network (Eq. 21-22) and Fp = dU/dq with packed FMAs; weight rows are shared-memory broadcasts
 //   P4  partial forces of the radial-only neighbours (Eq. 24)
-//   P5  partial forces of the angular neighbours (Eq. 24 + Eq. 25), half 1 then half 0
-// Nothing but U_i, sum_j p_ij and the partial forces p_ij leaves the chip.
+//   P5  partial forces of the angular neighbours (Eq. 24 + Eq. 25), half 1 then half 0; half 1's share
+//       waits in the shared-memory rows P4 has freed
+// Nothing but U_i, sum_j p_ij, the partial forces p_ij and the parked sums leaves the chip.
 #pragma once
 
 constexpr int kRowsS = 24;          // angular neighbour rows staged in shared memory (more: read from global)
@@ -313,38 +317,47 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
 
     // ---- P3: network Eq. 21-22 (minus biases) and Fp = dU/dq; two neurons per iteration, weight rows
     //      read from shared memory as warp-wide broadcasts (staged layout w1[H][Dp] | b1[H] | w2[H] | b2) ----
+    // Packed FMAs: {a_lo, a_hi} accumulate the even / odd inputs of a neuron; the two weight rows of
+    // an iteration stay in registers between the forward and the backward sweep (one LDS.128 per 4 weights).
     float Fp[Dp];
-#pragma unroll
-    for (int v = 0; v < Dp; ++v) Fp[v] = 0.f;
     const float* b1 = sm + H * Dp;
     const float* w2 = b1 + H;
     float U = -w2[H];                                                   // - b2
-    for (int mu = 0; mu < H; mu += 2) {
-        const bool two = mu + 1 < H;
-        const int mu1 = two ? mu + 1 : mu;
-        const float4* r0 = reinterpret_cast<const float4*>(sm + mu * Dp);
-        const float4* r1 = reinterpret_cast<const float4*>(sm + mu1 * Dp);
-        float a0 = -b1[mu], a1 = 0.f, c0 = -b1[mu1], c1 = 0.f;
+    {
+        f32x2 qp[Dp / 2], Fpp[Dp / 2];
 #pragma unroll
-        for (int v = 0; v < Dp / 4; ++v) {
-            const float4 x = r0[v], y = r1[v];
-            a0 = fmaf(x.x, q[4 * v], a0); a1 = fmaf(x.y, q[4 * v + 1], a1); a0 = fmaf(x.z, q[4 * v + 2], a0); a1 = fmaf(x.w, q[4 * v + 3], a1);
-            c0 = fmaf(y.x, q[4 * v], c0); c1 = fmaf(y.y, q[4 * v + 1], c1); c0 = fmaf(y.z, q[4 * v + 2], c0); c1 = fmaf(y.w, q[4 * v + 3], c1);
-        }
-        float t0, d0, t1, d1;
-        tanh_sech2(a0 + a1, &t0, &d0);
-        tanh_sech2(c0 + c1, &t1, &d1);
-        const float w20 = w2[mu], w21 = two ? w2[mu1] : 0.f;
-        const float g0 = w20 * d0, g1 = w21 * d1;
-        U = fmaf(w20, t0, fmaf(w21, t1, U));
+        for (int v = 0; v < Dp / 2; ++v) { qp[v] = pack2(q[2 * v], q[2 * v + 1]); Fpp[v] = pack2(0.f, 0.f); }
+        for (int mu = 0; mu < H; mu += 2) {
+            const bool two = mu + 1 < H;
+            const int mu1 = two ? mu + 1 : mu;
+            const ulonglong2* r0 = reinterpret_cast<const ulonglong2*>(sm + mu * Dp);
+            const ulonglong2* r1 = reinterpret_cast<const ulonglong2*>(sm + mu1 * Dp);
+            ulonglong2 wa[Dp / 4], wb[Dp / 4];
 #pragma unroll
-        for (int v = 0; v < Dp / 4; ++v) {
-            const float4 x = r0[v], y = r1[v];
-            Fp[4 * v] = fmaf(g0, x.x, fmaf(g1, y.x, Fp[4 * v]));
-            Fp[4 * v + 1] = fmaf(g0, x.y, fmaf(g1, y.y, Fp[4 * v + 1]));
-            Fp[4 * v + 2] = fmaf(g0, x.z, fmaf(g1, y.z, Fp[4 * v + 2]));
-            Fp[4 * v + 3] = fmaf(g0, x.w, fmaf(g1, y.w, Fp[4 * v + 3]));
+            for (int v = 0; v < Dp / 4; ++v) { wa[v] = r0[v]; wb[v] = r1[v]; }
+            f32x2 a0 = pack2(-b1[mu], 0.f), a1 = pack2(0.f, 0.f), c0 = pack2(-b1[mu1], 0.f), c1 = pack2(0.f, 0.f);
+#pragma unroll
+            for (int v = 0; v < Dp / 4; ++v) {
+                a0 = ffma2(wa[v].x, qp[2 * v], a0); a1 = ffma2(wa[v].y, qp[2 * v + 1], a1);
+                c0 = ffma2(wb[v].x, qp[2 * v], c0); c1 = ffma2(wb[v].y, qp[2 * v + 1], c1);
+            }
+            float x0, x1, x2, x3, y0, y1, y2, y3;
+            unpack2(a0, x0, x1); unpack2(a1, x2, x3); unpack2(c0, y0, y1); unpack2(c1, y2, y3);
+            float t0, d0, t1, d1;
+            tanh_sech2((x0 + x1) + (x2 + x3), &t0, &d0);
+            tanh_sech2((y0 + y1) + (y2 + y3), &t1, &d1);
+            const float w20 = w2[mu], w21 = two ? w2[mu1] : 0.f;
+            const float g0 = w20 * d0, g1 = w21 * d1;
+            U = fmaf(w20, t0, fmaf(w21, t1, U));
+            const f32x2 g0p = pack2(g0, g0), g1p = pack2(g1, g1);
+#pragma unroll
+            for (int v = 0; v < Dp / 4; ++v) {
+                Fpp[2 * v] = ffma2(g0p, wa[v].x, ffma2(g1p, wb[v].x, Fpp[2 * v]));
+                Fpp[2 * v + 1] = ffma2(g0p, wa[v].y, ffma2(g1p, wb[v].y, Fpp[2 * v + 1]));
+            }
         }
+#pragma unroll
+        for (int v = 0; v < Dp / 2; ++v) unpack2(Fpp[v], Fp[2 * v], Fp[2 * v + 1]);
     }
     if (active) d.Us[i] = U;
 

@@ -231,6 +231,19 @@ __global__ void k_gather_b(SysDev d, int N, int have_v, int gated) {
     }
 }
 
+// 256-bit read-only loads (sm_100: LDG.E.256): one request per gathered 32-byte sector instead of two
+__device__ __forceinline__ double4 ldg256(const double4* p) {
+    double4 v;
+    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void ldg256(const uint4* p, uint4& a, uint4& b) {      // p[0], p[1]
+    unsigned long long x, y, z, w;
+    asm volatile("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(x), "=l"(y), "=l"(z), "=l"(w) : "l"(p));
+    a = make_uint4((unsigned)x, (unsigned)(x >> 32), (unsigned)y, (unsigned)(y >> 32));
+    b = make_uint4((unsigned)z, (unsigned)(z >> 32), (unsigned)w, (unsigned)(w >> 32));
+}
+
 __device__ __forceinline__ double min_image(double t, double L, double invL) { return t - L * rint(t * invL); }
 
 // Verlet list: all j != i with |r_ij|^2 < (r_c^R + skin)^2, rows ascending in the sorted index j
@@ -260,7 +273,7 @@ __global__ void __launch_bounds__(128) k_build_md(SysDev d, int N, Box b, double
         const int lo = d.cell_start[cells[q]], hi = d.cell_start[cells[q] + 1];
         for (int j = lo; j < hi; ++j) {
             if (j == i) continue;
-            const double4 pj = d.xs4[j];
+            const double4 pj = ldg256(&d.xs4[j]);
             const double dx = min_image(pj.x - xi, b.L[0], b.invL[0]);
             const double dy = min_image(pj.y - yi, b.L[1], b.invL[1]);
             const double dz = min_image(pj.z - zi, b.L[2], b.invL[2]);
@@ -324,7 +337,7 @@ __global__ void __launch_bounds__(128) k_filter(SysDev d, int N, Box b, double r
 #pragma unroll
         for (int u = 0; u < B; ++u) eb[u] = s0 + u < cnt ? d.md_idx[(size_t)(s0 + u) * N + i] : i;
 #pragma unroll
-        for (int u = 0; u < B; ++u) pb[u] = d.xs4[eb[u] & kJMask];
+        for (int u = 0; u < B; ++u) pb[u] = ldg256(&d.xs4[eb[u] & kJMask]);
 #pragma unroll
         for (int u = 0; u < B; ++u) {
             const int s = s0 + u;
@@ -452,8 +465,7 @@ __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
 #pragma unroll
             for (int u = 0; u < B; ++u) {
                 const int j = jr[u] & kJMask;
-                mrb[u] = d.masks[2 * (size_t)j];
-                mab[u] = d.masks[2 * (size_t)j + 1];
+                ldg256(&d.masks[2 * (size_t)j], mrb[u], mab[u]);
             }
 #pragma unroll
             for (int u = 0; u < B; ++u) {

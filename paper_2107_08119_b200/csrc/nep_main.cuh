@@ -54,26 +54,42 @@ __device__ __forceinline__ float fast_rcp(float x) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// k_order: order[w*256 + t] = the atom of window w with the t-th largest key (nA, then nR - nA).
-// Entries past N are -1.  One block of 256 threads per window; rank by counting.
+// k_order: order[w*256 + t] = the atom of window w with the t-th largest key; the key is the
+// angular count (exact, up to 127) and the radial-only count in steps of 4, so the 32 atoms of a warp
+// agree in nA and nearly in nR.  Entries past N are -1.  One block of 256 threads per window: a
+// counting sort (histogram, scan, cursor) in shared memory.
 // ------------------------------------------------------------------------------------------------
+constexpr int kOrderBins = 1024;
 __global__ void __launch_bounds__(kWin) k_order(SysDev d, int N) {
-    __shared__ int key[kWin];
+    __shared__ int hist[kOrderBins];
+    __shared__ int wsum[kWin / 32];
     const int t = threadIdx.x;
     const int i = blockIdx.x * kWin + t;
-    int k = -1;
-    if (i < N) {
-        const int nA = d.nnA[i], nR = d.nnR[i];
-        k = (nA << 8) | (nR - nA);
-    }
-    key[t] = k;
+    for (int b = t; b < kOrderBins; b += kWin) hist[b] = 0;
     __syncthreads();
-    int rank = 0;
-#pragma unroll 8
-    for (int j = 0; j < kWin; ++j) {
-        const int kj = key[j];
-        rank += (kj > k) || (kj == k && j < t);
+    int bin = kOrderBins - 1;                         // past N: sorts last
+    if (i < N) {
+        const int nA = d.nnA[i], nO = d.nnR[i] - nA;
+        bin = kOrderBins - 2 - (min(nA, 127) * 8 + min(nO >> 2, 7));     // descending key
     }
+    atomicAdd(&hist[bin], 1);
+    __syncthreads();
+    // exclusive scan of the 1024 bins: 4 per thread, warp scan, then the 8 warp totals
+    const int h0 = hist[4 * t], h1 = hist[4 * t + 1], h2 = hist[4 * t + 2], h3 = hist[4 * t + 3];
+    const int mine = h0 + h1 + h2 + h3;
+    int incl = mine;
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((t & 31) >= o) incl += v;
+    }
+    if ((t & 31) == 31) wsum[t >> 5] = incl;
+    __syncthreads();
+    int base = incl - mine;
+    for (int w = 0; w < (t >> 5); ++w) base += wsum[w];
+    __syncthreads();
+    hist[4 * t] = base; hist[4 * t + 1] = base + h0; hist[4 * t + 2] = base + h0 + h1; hist[4 * t + 3] = base + h0 + h1 + h2;
+    __syncthreads();
+    const int rank = atomicAdd(&hist[bin], 1);         // order inside a bin is arbitrary (equal keys)
     d.order[blockIdx.x * kWin + rank] = i < N ? i : -1;
 }
 

@@ -293,15 +293,17 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
         }
     }
     auto raw_only = [&](int o) { return o < kRowsO ? praw[o * 32 + lane] : grec[(size_t)(P.capR - 1 - o) * N]; };
-    for (int o = 0; o < nO; o += 2) {
-        const int o1 = min(o + 1, nO - 1);
-        const float4 e0 = raw_only(o), e1 = raw_only(o1);
-        float ri, r, om;
-        radial_acc(e0, true, ri, r, om);
-        radial_acc(e1, o + 1 < nO, ri, r, om);
+    for (int o = 0; o < nO; o += 4) {                // four independent chains per iteration
+        float4 e[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) e[u] = raw_only(min(o + u, nO - 1));
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            float ri, r, om;
+            radial_acc(e[u], o + u < nO, ri, r, om);
+        }
     }
 
-    // ---- P2: angular sums, half 0 (parked in shared memory) then half 1 (stays in registers) ----
     // A finished half leaves the registers for coalesced rows of spark0 / spark1 (written and read by the
     // same thread a few microseconds apart: L2 traffic) while other phases need them.
     f32x2 s2[NA][NP];
@@ -382,9 +384,9 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
     // ---- P4: radial-only neighbours, Eq. 24 ----
     float fsx = 0.f, fsy = 0.f, fsz = 0.f;
     float4* prow = d.p + (size_t)i * P.capR;         // p_ij lives at the record's own slot
-    for (int o = 0; o < nO; o += 2) {                // two neighbours per iteration: independent chains
+    for (int o = 0; o < nO; o += 4) {                // four independent chains per iteration
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < 4; ++u) {
             const int oo = min(o + u, nO - 1);
             const float4 e = raw_only(oo);
             const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;

@@ -99,6 +99,18 @@ def test_c2_amorphous_si(oracle):
     assert st["max_radial"] > 30                  # irregular neighbour counts
 
 
+def test_dense_amorphous_exercises_overflow_rows(oracle):
+    """1000 atoms at 1.45x the Si density with cutoffs 5.6 / 4.6 A: most atoms have more angular
+    neighbours than k_main stages in shared memory (24 rows) and more radial-only ones than its 20
+    rows, so the read-from-global paths of every phase are compared with the oracle too."""
+    w = inputs.config2(n_atoms=1000, side=24.0)
+    w.rc_r, w.rc_a = 5.6, 4.6
+    rep, system = run_config(oracle, w, cap_r=96, cap_a=48)
+    cnt_r, _ = system.get_neighbors(0)
+    cnt_a, _ = system.get_neighbors(1)
+    assert int(cnt_a.max()) > 24 and int((cnt_r - cnt_a).max()) > 20, (int(cnt_a.max()), int((cnt_r - cnt_a).max()))
+
+
 def test_c4_si_32768(oracle):
     run_config(oracle, inputs.config4(32768))
 

@@ -65,6 +65,7 @@ struct SysDev {                 // device pointers into the caller's workspace
     float4* p;                  // [N][cap_R] partial forces dU_i/dr_ij at the record slots
     float2* spark0;             // [NA*6][ceil(N/256)*256] angular sums s[n][lm] of lm half 0 / half 1: parked here by k_main
     float2* spark1;             //   (coalesced rows, L2-resident between write and read) while the registers hold other phases
+    float* FpG;                 // [D][ceil(N/256)*256] dU/dq from k_desc64 (multi-species models only)
     int* order;                 // [ceil(N/256)*256] atoms of each 256-window sorted by neighbour count (-1: none)
 };
 
@@ -73,6 +74,13 @@ constexpr int kMaxH = 64;           // hidden neurons supported (weights are sta
 // sqrt(Z_a Z_b) of Eq. 19, passed to k_main by value (kernel-parameter constant bank)
 struct ZZParams {
     float zz[kMaxTypes * kMaxTypes];
+};
+
+// parameters of k_desc64 (nep_desc64.cuh), passed by value
+struct Desc64Params {
+    double rcR, rcA;
+    double zz[kMaxTypes * kMaxTypes];     // sqrt(Z_a Z_b) in double
+    int H, N, capR;
 };
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -89,6 +97,8 @@ struct nep_model {
     float* params_dev;          // staged fp32 layout: w1[H][Dp] (rows zero-padded) | b1[H] | w2[H] | b2 | pad
     int params_floats;
     ZZParams zz;
+    double* params64_dev;       // multi-species models: the Eq. 26 vector in double, caller order (k_desc64)
+    Desc64Params p64;
 };
 
 struct nep_system {
@@ -407,6 +417,7 @@ __global__ void k_export_lists(SysDev d, int N, int which, int capR, int cap_out
 #define NEP_MAIN_MIN_BLOCKS 4
 #endif
 #include "nep_main.cuh"
+#include "nep_desc64.cuh"
 #include "fp32_peak.cuh"
 
 // ------------------------------------------------------------------------------------------------
@@ -623,7 +634,7 @@ struct Layout {
 };
 
 // carve the workspace; the same routine sizes it (base == nullptr)
-Layout carve(int64_t N, int capR, int capMD, int max_cells, int NA, SysDev* d, char* base) {
+Layout carve(int64_t N, int capR, int capMD, int max_cells, int NA, int D64, SysDev* d, char* base) {
     Layout L; size_t o = 0; int k = 0;
     auto take = [&](size_t bytes) { size_t at = o; o = align256(o + bytes); L.off[k++] = at; return base ? base + at : nullptr; };
     const size_t n = (size_t)N;
@@ -654,6 +665,7 @@ Layout carve(int64_t N, int capR, int capMD, int max_cells, int NA, SysDev* d, c
     t.xs4 = (double4*)take(n * 32);
     t.p = (float4*)take(n * 16 * capR);
     t.order = (int*)take(((n + kWin - 1) / kWin) * kWin * 4);
+    t.FpG = (float*)take(((n + kWin - 1) / kWin) * kWin * 4 * (size_t)D64 + 16);
     t.spark0 = (float2*)take(((n + kWin - 1) / kWin) * kWin * 8 * (size_t)(NA * kHalfLM / 2));
     t.spark1 = (float2*)take(((n + kWin - 1) / kWin) * kWin * 8 * (size_t)(NA * kHalfLM / 2));
     L.total = o;
@@ -702,6 +714,12 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
         attr_done = true;
     }
     const int windows = (int)((s->N + kWin - 1) / kWin);
+    if (MULTI) {
+        Desc64Params p64 = m->p64;
+        p64.N = (int)s->N; p64.capR = s->capR;
+        k_desc64<NR, NA><<<windows * (kWin / 64), 64, 0, st>>>(s->d, s->box, p64, m->params64_dev);
+        s->launches += 1;
+    }
     k_main<NR, NA, MULTI><<<windows * (kWin / (32 * kMainWarps)), 32 * kMainWarps, smem, st>>>(s->d, P, m->params_dev, m->zz);
     s->launches += 1;
 }
@@ -809,6 +827,14 @@ int nep_create(const nep_hyper* hy, const int* atomic_number, const double* para
     cudaError_t e = cudaMalloc(&m->params_dev, (size_t)m->params_floats * sizeof(float));
     if (e == cudaSuccess) e = cudaMemcpy(m->params_dev, stage, (size_t)m->params_floats * sizeof(float), cudaMemcpyHostToDevice);
     delete[] stage;
+    m->params64_dev = nullptr;
+    if (e == cudaSuccess && hy->n_types > 1) {
+        e = cudaMalloc(&m->params64_dev, (size_t)m->npar * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemcpy(m->params64_dev, params, (size_t)m->npar * sizeof(double), cudaMemcpyHostToDevice);
+        m->p64.rcR = hy->rc_radial; m->p64.rcA = hy->rc_angular; m->p64.H = H;
+        for (int a = 0; a < kMaxTypes; ++a)
+            for (int b = 0; b < kMaxTypes; ++b) m->p64.zz[a * kMaxTypes + b] = sqrt((double)m->Z[a] * (double)m->Z[b]);   // Eq. 19
+    }
     if (e != cudaSuccess) { set_cuda_error(e, "nep_create"); nep_destroy(m); return NEP_ECUDA; }
     *out = m;
     return NEP_OK;
@@ -820,6 +846,7 @@ int nep_num_params(const nep_model* m) { return m ? m->npar : NEP_EINVAL; }
 void nep_destroy(nep_model* m) {
     if (!m) return;
     if (m->params_dev) cudaFree(m->params_dev);
+    if (m->params64_dev) cudaFree(m->params64_dev);
     delete m;
 }
 
@@ -827,7 +854,7 @@ size_t nep_workspace_bytes(const nep_model* m, int64_t n_atoms, int cap_radial, 
     if (!m || n_atoms < 1 || n_atoms >= (1 << 24) || cap_radial < 1 || cap_radial > 124 || cap_angular < 1 ||
         cap_angular > cap_radial || !(skin >= 0.0))
         return 0;
-    return carve(n_atoms, cap_radial, cap_md_of(m, cap_radial, skin), max_cells_of(n_atoms), m->NA, nullptr, nullptr).total;
+    return carve(n_atoms, cap_radial, cap_md_of(m, cap_radial, skin), max_cells_of(n_atoms), m->NA, m->h.n_types > 1 ? m->D : 0, nullptr, nullptr).total;
 }
 
 int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, int cap_radial, int cap_angular,
@@ -842,7 +869,7 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
     s->model = m; s->N = n_atoms; s->capR = cap_radial; s->capA = cap_angular; s->skin = skin;
     s->capMD = cap_md_of(m, cap_radial, skin);
     s->max_cells = max_cells_of(n_atoms);
-    carve(n_atoms, s->capR, s->capMD, s->max_cells, m->NA, &s->d, (char*)workspace_dev);
+    carve(n_atoms, s->capR, s->capMD, s->max_cells, m->NA, m->h.n_types > 1 ? m->D : 0, &s->d, (char*)workspace_dev);
     s->built = false; s->have_forces = false; s->last_stream = nullptr; s->step_graph = nullptr;
     s->launches = 0; s->prof_on = false; s->prof_n = 0;
     for (int k = 0; k < NEP_PHASES; ++k) { s->prof_ms[k] = 0.0; s->prof_cnt[k] = 0; }

@@ -328,20 +328,27 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
                 s2[n][mm] = pack2(v.x, v.y);
             }
     };
-    desc_half<0, NR, NA>(nA, P.rcA_inv, load_nbr, s2, q);
-    park(d.spark0);
-    desc_half<1, NR, NA>(nA, P.rcA_inv, load_nbr, s2, q);
-    park(d.spark1);
+    // Multi-species models: q, the network and the sums s come from k_desc64 (fp64; nep_desc64.cuh),
+    // which has already filled Us, FpG and spark0 / spark1 -- P2 and P3 are skipped here.
+    if (!MULTI) {
+        desc_half<0, NR, NA>(nA, P.rcA_inv, load_nbr, s2, q);
+        park(d.spark0);
+        desc_half<1, NR, NA>(nA, P.rcA_inv, load_nbr, s2, q);
+        park(d.spark1);
+    }
 
     // ---- P3: network Eq. 21-22 (minus biases) and Fp = dU/dq; two neurons per iteration, weight rows
     //      read from shared memory as warp-wide broadcasts (staged layout w1[H][Dp] | b1[H] | w2[H] | b2) ----
     // Packed FMAs: {a_lo, a_hi} accumulate the even / odd inputs of a neuron; the two weight rows of
     // an iteration stay in registers between the forward and the backward sweep (one LDS.128 per 4 weights).
     float Fp[Dp];
-    const float* b1 = sm + H * Dp;
-    const float* w2 = b1 + H;
-    float U = -w2[H];                                                   // - b2
-    {
+    if (MULTI) {
+#pragma unroll
+        for (int v = 0; v < Dp; ++v) Fp[v] = v < D ? d.FpG[(size_t)v * npad + gcol] : 0.f;
+    } else {
+        const float* b1 = sm + H * Dp;
+        const float* w2 = b1 + H;
+        float U = -w2[H];                                               // - b2
         f32x2 qp[Dp / 2], Fpp[Dp / 2];
 #pragma unroll
         for (int v = 0; v < Dp / 2; ++v) { qp[v] = pack2(q[2 * v], q[2 * v + 1]); Fpp[v] = pack2(0.f, 0.f); }
@@ -376,8 +383,8 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
         }
 #pragma unroll
         for (int v = 0; v < Dp / 2; ++v) unpack2(Fpp[v], Fp[2 * v], Fp[2 * v + 1]);
+        if (active) d.Us[i] = U;
     }
-    if (active) d.Us[i] = U;
 
     unpark(d.spark1);                                // half 1 comes back; its loads are in flight while P4 runs
 

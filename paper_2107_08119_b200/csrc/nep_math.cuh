@@ -280,6 +280,39 @@ NEP_HD void radial_gd(float r, float rcinv, float omega, float gscale, float* gs
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// fp64 forms for the multi-species descriptor (k_desc64): with the sqrt(Z_i Z_j) weights of Eq. 19 the
+// descriptor reaches ~4e3 and the network's pre-activations cancel to O(1), so q, the pre-activations
+// and tanh are evaluated in double there.  Same polynomials as above.
+// ------------------------------------------------------------------------------------------------
+template <int N>
+NEP_HD void radial_g64(double r, double rc, double omega, double* g) {
+    const double u = r / rc, um1 = u - 1.0;
+    const double x2 = 4.0 * um1 * um1 - 2.0;                           // 2 x
+    const double hf = 0.25 * omega * (1.0 + cos(3.14159265358979323846 * u));     // omega fc / 2   (Eq. 15)
+    double Tm = 1.0, T = 0.5 * x2;
+    g[0] = 2.0 * hf;
+#pragma unroll
+    for (int n = 1; n < N; ++n) {
+        g[n] = hf * (T + 1.0);                                         // Eq. 14
+        const double Tn = x2 * T - Tm; Tm = T; T = Tn;                 // Eq. A1
+    }
+}
+
+NEP_HD void ylm_basis64(double x, double y, double z, double* b) {
+    const double z2 = z * z;
+    const double c2 = x * x - y * y, s2 = 2.0 * x * y;
+    const double c3 = x * c2 - y * s2, s3 = x * s2 + y * c2;
+    const double t5 = 5.0 * z2 - 1.0, t7 = 7.0 * z2 - 3.0, u7 = 7.0 * z2 - 1.0;
+    b[0] = x; b[1] = y; b[2] = z;
+    b[3] = 3.0 * z2 - 1.0; b[4] = x * z; b[5] = y * z; b[6] = c2; b[7] = s2;
+    b[8] = z * (5.0 * z2 - 3.0); b[9] = x * t5; b[10] = y * t5; b[11] = z * c2; b[12] = z * s2;
+    b[13] = c3; b[14] = s3;
+    b[15] = z2 * (35.0 * z2 - 30.0) + 3.0; b[16] = x * z * t7; b[17] = y * z * t7;
+    b[18] = c2 * u7; b[19] = s2 * u7; b[20] = z * c3; b[21] = z * s3;
+    b[22] = c2 * c2 - s2 * s2; b[23] = 2.0 * c2 * s2;
+}
+
 // t = tanh(a), d = 1 - tanh^2(a) = 4 e / (1 + e)^2 with e = exp(-2|a|): no cancellation when |t| -> 1.
 // On the device e and 1/(1+e) come from MUFU.EX2 / MUFU.RCP (2 and 1 ulp): |dt| < 3e-7, far inside the
 // 1e-5 eV energy bar, and the chain is a handful of instructions instead of expf + an IEEE division.

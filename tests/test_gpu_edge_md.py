@@ -153,6 +153,23 @@ def test_md_c1_nve_with_rebuilds(oracle):
     assert np.abs(hsum - ref["Jsum"]).max() < 1e-3 * np.abs(ref["Jsum"]).max()
 
 
+def test_md_c3_pbte_replica_tracks_oracle(oracle):
+    """C3 geometry (4x4x4 rock-salt cells, 512 atoms, literal Eq. 19) for 20 NVE steps: the GPU
+    trajectory and energies are judged against the oracle's own run at the same dt (the saturating
+    network makes the oracle itself drift; SURVEY.md 8(c) 'PbTe conditioning')."""
+    w = inputs.config3(cells=(4, 4, 4))
+    n_steps = 20
+    system, pos, vel, out, hsum, thermo, ref = _md_compare(oracle, w, n_steps, 1.0, cap_r=80, cap_a=40)
+    E = thermo[:, 0] + thermo[:, 1]
+    Eref = ref["thermo"][1:, 0] + ref["thermo"][1:, 1]
+    drift_ref = np.abs(Eref - Eref[0]).max() / w.n_atoms
+    drift = np.abs(E - E[0]).max() / w.n_atoms
+    print("C3 NVE |E-E0|/N: gpu %.3g  oracle %.3g" % (drift, drift_ref))
+    assert drift < 2 * drift_ref + 1e-6
+    assert np.abs(E - Eref).max() / w.n_atoms < 1e-5
+    assert np.abs(pos - ref["pos"]).max() < 1e-4
+
+
 def test_md_chunked_calls_continue_trajectory(oracle):
     """nep_md_step(30) + nep_md_step(20) == nep_md_step(50) bit for bit (same launch sequence)."""
     torch, api = _gpu()

@@ -341,13 +341,19 @@ __global__ void __launch_bounds__(128) k_filter(SysDev d, int N, Box b, double r
     int nA = 0, nO = 0;
     unsigned mR[4] = {0u, 0u, 0u, 0u}, mA[4] = {0u, 0u, 0u, 0u};
     constexpr int B = 8;                 // batch: B list entries, then B position gathers, in flight together
+    int en[B];                          // list entries of the NEXT batch: their loads overlap this batch's gathers
+#pragma unroll
+    for (int u = 0; u < B; ++u) en[u] = u < cnt ? d.md_idx[(size_t)u * N + i] : i;
     for (int s0 = 0; s0 < cnt; s0 += B) {
         int eb[B];
         double4 pb[B];
 #pragma unroll
-        for (int u = 0; u < B; ++u) eb[u] = s0 + u < cnt ? d.md_idx[(size_t)(s0 + u) * N + i] : i;
+        for (int u = 0; u < B; ++u) eb[u] = en[u];
 #pragma unroll
         for (int u = 0; u < B; ++u) pb[u] = ldg256(&d.xs4[eb[u] & kJMask]);
+#pragma unroll
+        for (int u = 0; u < B; ++u) en[u] = s0 + B + u < cnt ? d.md_idx[(size_t)(s0 + B + u) * N + i] : i;
+        unsigned bR = 0u, bA = 0u;
 #pragma unroll
         for (int u = 0; u < B; ++u) {
             const int s = s0 + u;
@@ -366,15 +372,15 @@ __global__ void __launch_bounds__(128) k_filter(SysDev d, int N, Box b, double r
                     d.rec[(size_t)slot * N + i] = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(ty));
                     d.jrev[(size_t)slot * N + i] = e;
                 }
-#pragma unroll
-                for (int wq = 0; wq < 4; ++wq) {
-                    const unsigned bit = (s >> 5) == wq ? 1u << (s & 31) : 0u;
-                    mR[wq] |= bit;
-                    if (ang) mA[wq] |= bit;
-                }
+                bR |= 1u << u;
+                if (ang) bA |= 1u << u;
                 if (ang) ++nA; else ++nO;
             }
         }
+        // the batch's 8 bits go into byte (s0 >> 3) & 3 of word s0 >> 5
+#pragma unroll
+        for (int wq = 0; wq < 4; ++wq)
+            if ((s0 >> 5) == wq) { mR[wq] |= bR << (s0 & 31); mA[wq] |= bA << (s0 & 31); }
     }
     const int nR = nA + nO;
     const bool over = nR > capR || nA > capA;

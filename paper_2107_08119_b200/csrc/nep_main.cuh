@@ -292,7 +292,11 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
             if (MULTI) som[k1 * 32 + lane] = om1;
         }
     }
-    auto raw_only = [&](int o) { return o < kRowsO ? praw[o * 32 + lane] : grec[(size_t)(P.capR - 1 - o) * N]; };
+    // radial-only record o: one generic load from the staged row or, past kRowsO rows, from global memory (no branch)
+    auto raw_only = [&](int o) {
+        const float4* src = o < kRowsO ? &praw[o * 32 + lane] : &grec[(size_t)(P.capR - 1 - o) * N];
+        return *src;
+    };
     for (int o = 0; o < nO; o += 4) {                // four independent chains per iteration
         float4 e[4];
 #pragma unroll
@@ -392,10 +396,13 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
     float fsx = 0.f, fsy = 0.f, fsz = 0.f;
     float4* prow = d.p + (size_t)i * P.capR;         // p_ij lives at the record's own slot
     for (int o = 0; o < nO; o += 4) {                // four independent chains per iteration
+        float4 e4[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) e4[u] = raw_only(min(o + u, nO - 1));
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const int oo = min(o + u, nO - 1);
-            const float4 e = raw_only(oo);
+            const float4 e = e4[u];
             const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
             const float rinv = inv_norm(r2);
             float gs[NR], dg[NR];

@@ -110,11 +110,11 @@ struct nep_system {
     Box box;
     bool built, have_forces;
     cudaStream_t last_stream;
+    // one MD step captured as a CUDA graph (replayed n_steps times; re-captured when its arguments change)
     cudaGraphExec_t step_graph;
-    // key of the captured graph (a change re-captures)
-    const void* g_key[10];
-    double g_dt;
-    double g_mass[kMaxTypes];
+    cudaStream_t cap_stream;               // library-owned stream used only for capture
+    unsigned char g_key[512];              // AsmParams + dt of the captured step
+    int64_t g_launches;                    // kernels per replay
     int64_t host_stats[4];
     int64_t launches;                      // kernels launched since creation
     // optional per-phase event timing (nep_profile)
@@ -785,6 +785,47 @@ bool device_ok() {
     return cudaGetDeviceCount(&n) == cudaSuccess && n > 0;
 }
 
+// one velocity-Verlet step: half-kick + drift, device-gated rebuild, filter, k_main, assembly + second half-kick
+void launch_step(nep_system* s, const AsmParams& P, double dt_fs, double hs2, cudaStream_t st) {
+    const int N = (int)s->N;
+    phase(s, PH_KICK, st);
+    k_kick_drift<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, dt_fs, hs2, P);
+    phase(s, PH_BUILD, st);
+    launch_build(s, s->d.xs, s->d.vs, 0, 1, st);
+    phase(s, PH_FILTER, st);
+    launch_filter(s, st);
+    phase(s, PH_MAIN, st);
+    launch_main(s, st);
+    phase(s, PH_ASSEMBLE, st);
+    k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
+    s->launches += 2;
+}
+
+// The step as a CUDA graph, captured on a library-owned stream (the caller's may be the legacy default
+// stream, which cannot capture) and launched into the caller's stream.  Keyed on every argument baked in.
+int ensure_step_graph(nep_system* s, const AsmParams& P, double dt_fs, double hs2) {
+    static_assert(sizeof(AsmParams) + sizeof(double) <= sizeof(s->g_key), "g_key too small");
+    unsigned char key[sizeof(s->g_key)];
+    memset(key, 0, sizeof(key));
+    memcpy(key, &P, sizeof(P));
+    memcpy(key + sizeof(P), &dt_fs, sizeof(double));
+    if (s->step_graph && memcmp(key, s->g_key, sizeof(key)) == 0) return NEP_OK;
+    if (s->step_graph) { cudaGraphExecDestroy(s->step_graph); s->step_graph = nullptr; }
+    if (!s->cap_stream) NEP_CUDA_OK(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
+    cudaGraph_t g = nullptr;
+    NEP_CUDA_OK(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
+    const int64_t l0 = s->launches;
+    launch_step(s, P, dt_fs, hs2, s->cap_stream);
+    s->g_launches = s->launches - l0;
+    s->launches = l0;
+    NEP_CUDA_OK(cudaStreamEndCapture(s->cap_stream, &g));
+    cudaError_t e = cudaGraphInstantiate(&s->step_graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { s->step_graph = nullptr; set_cuda_error(e, "cudaGraphInstantiate"); return NEP_ECUDA; }
+    memcpy(s->g_key, key, sizeof(key));
+    return NEP_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -876,7 +917,7 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
     s->capMD = cap_md_of(m, cap_radial, skin);
     s->max_cells = max_cells_of(n_atoms);
     carve(n_atoms, s->capR, s->capMD, s->max_cells, m->NA, m->h.n_types > 1 ? m->D : 0, &s->d, (char*)workspace_dev);
-    s->built = false; s->have_forces = false; s->last_stream = nullptr; s->step_graph = nullptr;
+    s->built = false; s->have_forces = false; s->last_stream = nullptr; s->step_graph = nullptr; s->cap_stream = nullptr; s->g_launches = 0;
     s->launches = 0; s->prof_on = false; s->prof_n = 0;
     for (int k = 0; k < NEP_PHASES; ++k) { s->prof_ms[k] = 0.0; s->prof_cnt[k] = 0; }
     for (int k = 0; k < kProfMaxEvents; ++k) s->prof_ev[k] = nullptr;
@@ -890,6 +931,7 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
 void nep_system_destroy(nep_system* s) {
     if (!s) return;
     if (s->step_graph) cudaGraphExecDestroy(s->step_graph);
+    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     for (int k = 0; k < kProfMaxEvents; ++k) if (s->prof_ev[k]) cudaEventDestroy(s->prof_ev[k]);
     delete s;
 }
@@ -912,6 +954,7 @@ int nep_neighbors(nep_system* s, const double* pos_dev, const double box[3], voi
     b.ncell = b.nc[0] * b.nc[1] * b.nc[2];
     s->box = b;
     s->last_stream = st;
+    if (s->step_graph) { cudaGraphExecDestroy(s->step_graph); s->step_graph = nullptr; }   // the box is baked into it
     phase(s, PH_BUILD, st);
     launch_build(s, pos_dev, nullptr, 1, 0, st);
     phase(s, PH_FILTER, st);
@@ -999,18 +1042,14 @@ int nep_md_step(nep_system* s, double* pos_dev, double* vel_dev, const double* m
         s->launches += 1;
     }
     P.md = 1;
-    for (int step = 0; step < n_steps; ++step) {
-        phase(s, PH_KICK, st);
-        k_kick_drift<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, dt_fs, hs2, P);
-        phase(s, PH_BUILD, st);
-        launch_build(s, s->d.xs, s->d.vs, 0, 1, st);
-        phase(s, PH_FILTER, st);
-        launch_filter(s, st);
-        phase(s, PH_MAIN, st);
-        launch_main(s, st);
-        phase(s, PH_ASSEMBLE, st);
-        k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
-        s->launches += 2;
+    if (s->prof_on || n_steps < 2) {
+        for (int step = 0; step < n_steps; ++step) launch_step(s, P, dt_fs, hs2, st);
+    } else {
+        // the step's launch sequence is fixed (rebuilds are device-gated): capture it once, replay it
+        const int rc = ensure_step_graph(s, P, dt_fs, hs2);
+        if (rc != NEP_OK) return rc;
+        for (int step = 0; step < n_steps; ++step) NEP_CUDA_OK(cudaGraphLaunch(s->step_graph, st));
+        s->launches += s->g_launches * n_steps;
     }
     phase(s, PH_STATE, st);
     k_store_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, vel_dev);

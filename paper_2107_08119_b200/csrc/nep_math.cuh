@@ -188,51 +188,55 @@ NEP_HD void ylm_basis_half(float x, float y, float z, float* b) {
     }
 }
 
-// V = sum_{k in half} St[k] grad B_k(r^)   (the non-radial part of ylm_force restricted to one half)
+// V = sum_{k in half} St[k] grad B_k(r^)   (the non-radial part of ylm_force restricted to one half).
+// (x, y, z) is a unit vector: x^2 + y^2 = 1 - z^2 shortens the gradient polynomials, e.g.
+// x^2 + y^2 - 4 z^2 = 1 - 5 z^2 and 9 x^2 + 3 y^2 - 4 z^2 = 6 x^2 - (7 z^2 - 3).
 template <int HALF>
 NEP_HD void ylm_grad_half(float x, float y, float z, const float* St, float* Vx, float* Vy, float* Vz) {
-    const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y, xz = x * z, yz = y * z;
-    const float c2 = x2 - y2;
+    const float x2 = x * x, y2 = y * y, z2 = z * z, xy = x * y;
+    const float c2 = fmaf(x, x, -y * y);
     if (HALF == 0) {
-        const float xyz = xy * z, s2 = xy + xy;
+        const float s2 = xy + xy;
         const float c3 = fmaf(x, c2, -y * s2), s3 = fmaf(x, s2, y * c2);
-        const float rho2 = x2 + y2;
-        const float q4 = fmaf(-4.f, z2, rho2);            // x^2 + y^2 - 4 z^2
-        const float m6xyz = -6.f * xyz, zc2_3 = 3.f * z * c2;
+        const float t7 = fmaf(7.f, z2, -3.f), u7 = fmaf(7.f, z2, -1.f);
+        const float m6xyz = -6.f * (xy * z);
+        const float zc2_3 = 3.f * (z * c2);
+        const float a40 = fmaf(-60.f, z2, 12.f);         // 12 (1 - 5 z^2)
+        const float d41 = fmaf(15.f, z2, -3.f);          // -3 (1 - 5 z^2)
+        const float c3_4 = 4.f * c3, s3_4 = 4.f * s3;
         float vx = St[0], vy = St[1], vz = St[2];        // l = 1
-        float wx, wy, wz;                                // l = 4 (second chain)
-        wx = St[3] * (12.f * x * q4); wy = St[3] * (12.f * y * q4);
-        wz = St[3] * (-16.f * z * fmaf(3.f, rho2, -2.f * z2));
-        vx = fmaf(St[4], -z * (fmaf(9.f, x2, 3.f * y2) - 4.f * z2), vx); vy = fmaf(St[4], m6xyz, vy);
-        vz = fmaf(St[4], -3.f * x * q4, vz);
-        wx = fmaf(St[5], m6xyz, wx); wy = fmaf(St[5], -z * (fmaf(3.f, x2, 9.f * y2) - 4.f * z2), wy);
-        wz = fmaf(St[5], -3.f * y * q4, wz);
-        vx = fmaf(St[6], -4.f * x * fmaf(-3.f, z2, x2), vx); vy = fmaf(St[6], 4.f * y * fmaf(-3.f, z2, y2), vy);
-        vz = fmaf(St[6], 12.f * z * c2, vz);
-        wx = fmaf(St[7], -2.f * y * (fmaf(3.f, x2, y2) - 6.f * z2), wx);
-        wy = fmaf(St[7], -2.f * x * (fmaf(3.f, y2, x2) - 6.f * z2), wy); wz = fmaf(St[7], 24.f * xyz, wz);
+        float wx, wy, wz;                                // second chain
+        wx = St[3] * (x * a40); wy = St[3] * (y * a40); wz = St[3] * (z * fmaf(80.f, z2, -48.f));
+        vx = fmaf(St[4], z * fmaf(-6.f, x2, t7), vx); vy = fmaf(St[4], m6xyz, vy); vz = fmaf(St[4], x * d41, vz);
+        wx = fmaf(St[5], m6xyz, wx); wy = fmaf(St[5], z * fmaf(-6.f, y2, t7), wy); wz = fmaf(St[5], y * d41, wz);
+        vx = fmaf(St[6], (4.f * x) * fmaf(3.f, z2, -x2), vx); vy = fmaf(St[6], (4.f * y) * fmaf(-3.f, z2, y2), vy);
+        vz = fmaf(St[6], 4.f * zc2_3, vz);
+        wx = fmaf(St[7], (y + y) * fmaf(-2.f, x2, u7), wx); wy = fmaf(St[7], (x + x) * fmaf(-2.f, y2, u7), wy);
+        wz = fmaf(St[7], -4.f * m6xyz, wz);
         vx = fmaf(St[8], zc2_3, vx); vy = fmaf(St[8], m6xyz, vy); vz = fmaf(St[8], c3, vz);
         wx = fmaf(St[9], -m6xyz, wx); wy = fmaf(St[9], zc2_3, wy); wz = fmaf(St[9], s3, wz);
-        vx = fmaf(St[10], 4.f * c3, vx); vy = fmaf(St[10], -4.f * s3, vy);
-        wx = fmaf(St[11], 4.f * s3, wx); wy = fmaf(St[11], 4.f * c3, wy);
+        vx = fmaf(St[10], c3_4, vx); vy = fmaf(St[10], -s3_4, vy);
+        wx = fmaf(St[11], s3_4, wx); wy = fmaf(St[11], c3_4, wy);
         *Vx = vx + wx; *Vy = vy + wy; *Vz = vz + wz;
     } else {
-        const float rho2 = x2 + y2;
+        const float xz = x * z, yz = y * z;
+        const float t5 = fmaf(5.f, z2, -1.f);
+        const float tx = x + x, ty = y + y;              // 2x, 2y
+        const float xy2 = xy + xy;                       // 2xy
         float vx, vy, vz, wx, wy, wz;
-        // l = 2
-        vx = St[0] * (-2.f * x); vy = St[0] * (-2.f * y); vz = St[0] * (4.f * z);
+        // l = 2:  Vx = 2x (St3 - St0) + z St1 + 2y St4, ...
+        vx = tx * (St[3] - St[0]); vy = -ty * (St[3] + St[0]); vz = (4.f * z) * St[0];
         vx = fmaf(St[1], z, vx); vz = fmaf(St[1], x, vz);
         vy = fmaf(St[2], z, vy); vz = fmaf(St[2], y, vz);
-        vx = fmaf(St[3], 2.f * x, vx); vy = fmaf(St[3], -2.f * y, vy);
-        vx = fmaf(St[4], 2.f * y, vx); vy = fmaf(St[4], 2.f * x, vy);
-        // l = 3
-        wx = St[5] * (-6.f * xz); wy = St[5] * (-6.f * yz); wz = St[5] * (-3.f * fmaf(-2.f, z2, rho2));
-        wx = fmaf(St[6], fmaf(4.f, z2, -3.f * x2) - y2, wx); wy = fmaf(St[6], -2.f * xy, wy); wz = fmaf(St[6], 8.f * xz, wz);
-        vx = fmaf(St[7], -2.f * xy, vx); vy = fmaf(St[7], fmaf(4.f, z2, -3.f * y2) - x2, vy); vz = fmaf(St[7], 8.f * yz, vz);
-        wx = fmaf(St[8], 2.f * xz, wx); wy = fmaf(St[8], -2.f * yz, wy); wz = fmaf(St[8], c2, wz);
-        vx = fmaf(St[9], 2.f * yz, vx); vy = fmaf(St[9], 2.f * xz, vy); vz = fmaf(St[9], 2.f * xy, vz);
-        wx = fmaf(St[10], 3.f * c2, wx); wy = fmaf(St[10], -6.f * xy, wy);
-        vx = fmaf(St[11], 6.f * xy, vx); vy = fmaf(St[11], 3.f * c2, vy);
+        vx = fmaf(St[4], ty, vx); vy = fmaf(St[4], tx, vy);
+        // l = 3 (4 z^2 - 3 x^2 - y^2 = (5 z^2 - 1) - 2 x^2 on the unit sphere)
+        wx = St[5] * (-6.f * xz); wy = St[5] * (-6.f * yz); wz = St[5] * fmaf(9.f, z2, -3.f);
+        wx = fmaf(St[6], fmaf(-2.f, x2, t5), wx); wy = fmaf(St[6], -xy2, wy); wz = fmaf(St[6], 8.f * xz, wz);
+        vx = fmaf(St[7], -xy2, vx); vy = fmaf(St[7], fmaf(-2.f, y2, t5), vy); vz = fmaf(St[7], 8.f * yz, vz);
+        wx = fmaf(St[8], xz + xz, wx); wy = fmaf(St[8], -(yz + yz), wy); wz = fmaf(St[8], c2, wz);
+        vx = fmaf(St[9], yz + yz, vx); vy = fmaf(St[9], xz + xz, vy); vz = fmaf(St[9], xy2, vz);
+        wx = fmaf(St[10], 3.f * c2, wx); wy = fmaf(St[10], -3.f * xy2, wy);
+        vx = fmaf(St[11], 3.f * xy2, vx); vy = fmaf(St[11], 3.f * c2, vy);
         *Vx = vx + wx; *Vy = vy + wy; *Vz = vz + wz;
     }
 }

@@ -226,6 +226,22 @@ def main():
     system.status()
 
     peak_ffma, peak_ffma2 = api.measure_fp32_peak()
+    pat_3reg, pat_desc, pat_force = api.measure_fp32_patterns()
+    # HBM-bound phases: algorithmic DRAM bytes per atom-step / phase time vs the measured copy peak
+    try:
+        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        hbm_src = "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        hbm_peak, hbm_src = 6500.0, "fallback of /opt/skills/guides/B200_PROFILING.md"
+    mr, ma = 0.5 * (m_r0 + m_r), 0.5 * (m_a0 + m_a)
+    m_md = mr * ((w.rc_r + args.skin) / w.rc_r) ** 3
+    bytes_filter = 4 * m_md + 32 + 20 * mr + 32 + 8           # Verlet row, own position, records + jrev, masks, counts
+    bytes_asm = 20 * mr + 16 * mr + 32 + 16 + 4 + 24 + 64 + 12 + 48   # records + jrev, p_ji, masks, Fself, U, v rw, outputs, Fs, kick
+    hbm_phases = {}
+    for name, nbytes in (("filter", bytes_filter), ("assemble", bytes_asm)):
+        gbs = nbytes * N / (prof[name]["ms"] / max(1, prof[name]["count"]) * 1e-3) / 1e9
+        hbm_phases[name] = {"bound": "hbm", "bytes_per_atom": nbytes, "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
+                            "frac": gbs / hbm_peak}
     traffic = None          # dram bytes per k_main launch from the committed ncu capture (1M-atom workload only)
     try:
         if args.workload == "c4_1048576":
@@ -271,10 +287,14 @@ def main():
                          "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
                          "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (no FP32 figure in MEASURED_PEAKS.json)",
                          "peak_measured_fma_chain": {"ffma": peak_ffma, "ffma2": peak_ffma2, "unit": "TFLOP/s"},
+                         "pattern_ceilings": {"ffma_three_distinct_registers": pat_3reg, "descriptor_contraction_ffma2": pat_desc,
+                                              "force_contraction_ffma2": pat_force, "unit": "TFLOP/s",
+                                              "what": "register-resident inner-loop patterns of k_main at its residency (8 warps/SM)"},
                          "frac_of_measured_ffma": achieved / peak_ffma,
                          "flops_per_atom": flops_atom, "kernel_ms": main_ms, "kernel_share_of_step": phase_ms["main"] / tot_phase,
                          "traffic": traffic},
             "phase_ms_per_step": phase_ms,
+            "roofline_hbm_phases": dict(hbm_phases, peak_source=hbm_src),
             "cpu_baseline": cpu,
         }
         print(json.dumps(line))

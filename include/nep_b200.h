@@ -151,6 +151,12 @@ int  nep_get_profile(nep_system*, double ms[8], int64_t count[8]);
  * FFMA and with packed fma.rn.f32x2 -- the measured denominator of the "alu" roofline. */
 int  nep_measure_fp32_peak(double* tflops_ffma, double* tflops_ffma2, void* cuda_stream);
 
+/* Three more register-resident patterns at k_main's residency (4 x 64 threads per SM), in TFLOP/s:
+ * [0] FFMA whose three source registers all differ (the register-file read limit), [1] the packed
+ * descriptor contraction s[n][lm] += g_n b_lm, [2] the packed force contraction S'/S += A[n][lm] g'_n / g_n.
+ * They are the attainable ceilings of k_main's inner loops, reported beside the nominal peak. */
+int  nep_measure_fp32_patterns(double tflops[3], void* cuda_stream);
+
 const char* nep_strerror(int code);
 
 #ifdef __cplusplus

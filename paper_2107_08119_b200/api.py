@@ -16,7 +16,7 @@ _lib = None
 
 SYMBOLS = ["nep_create", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",
            "nep_system_create", "nep_system_destroy", "nep_neighbors", "nep_get_neighbors", "nep_compute",
-           "nep_md_step", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile", "nep_measure_fp32_peak",
+           "nep_md_step", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile", "nep_measure_fp32_peak", "nep_measure_fp32_patterns",
            "nep_strerror"]
 
 
@@ -185,6 +185,13 @@ def measure_fp32_peak():
     a, b = C.c_double(), C.c_double()
     _check(lib().nep_measure_fp32_peak(C.byref(a), C.byref(b), _stream()), "nep_measure_fp32_peak")
     return a.value, b.value
+
+
+def measure_fp32_patterns():
+    """TFLOP/s of (FFMA with three distinct registers, packed descriptor contraction, packed force contraction)."""
+    out = (C.c_double * 3)()
+    _check(lib().nep_measure_fp32_patterns(C.cast(out, C.c_void_p), _stream()), "nep_measure_fp32_patterns")
+    return out[0], out[1], out[2]
 
 
 def from_workload(w, cap_radial=64, cap_angular=32, skin=1.0, device="cuda:0"):

@@ -1114,6 +1114,37 @@ int nep_measure_fp32_peak(double* tflops_ffma, double* tflops_ffma2, void* cuda_
     return NEP_OK;
 }
 
+int nep_measure_fp32_patterns(double tflops[3], void* cuda_stream) {
+    if (!tflops) return NEP_EINVAL;
+    if (!device_ok()) { set_cuda_error(cudaErrorNoDevice, "nep_measure_fp32_patterns"); return NEP_ECUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaDeviceProp prop;
+    NEP_CUDA_OK(cudaGetDeviceProperties(&prop, 0));
+    float* out = nullptr;
+    NEP_CUDA_OK(cudaMalloc(&out, 16));
+    cudaEvent_t e0, e1;
+    NEP_CUDA_OK(cudaEventCreate(&e0)); NEP_CUDA_OK(cudaEventCreate(&e1));
+    const int blocks = prop.multiProcessorCount * 4, iters = 1 << 13;        // k_main's residency: 4 x 64 threads per SM
+    const double fma_per_iter[3] = {16.0, 96.0, 192.0};
+    for (int v = 0; v < 3; ++v) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; ++rep) {
+            NEP_CUDA_OK(cudaEventRecord(e0, st));
+            if (v == 0) k_fma_pattern<0><<<blocks, 64, 0, st>>>(out, iters * 8, 0.999f, 0.001f);
+            else if (v == 1) k_fma_pattern<1><<<blocks, 64, 0, st>>>(out, iters, 0.999f, 0.001f);
+            else k_fma_pattern<2><<<blocks, 64, 0, st>>>(out, iters, 0.999f, 0.001f);
+            NEP_CUDA_OK(cudaEventRecord(e1, st));
+            NEP_CUDA_OK(cudaEventSynchronize(e1));
+            float ms = 0.f;
+            NEP_CUDA_OK(cudaEventElapsedTime(&ms, e0, e1));
+            if (rep > 0 && ms < best) best = ms;
+        }
+        tflops[v] = 2.0 * fma_per_iter[v] * iters * (v == 0 ? 8 : 1) * 64.0 * blocks / (best * 1e-3) / 1e12;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
+    return NEP_OK;
+}
+
 int nep_profile(nep_system* s, int enable) {
     if (!s) return NEP_EINVAL;
     NEP_CUDA_OK(cudaStreamSynchronize(s->last_stream));

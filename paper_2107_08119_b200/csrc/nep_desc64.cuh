@@ -8,9 +8,70 @@
 // the fp64 positions:  q_n (Eq. 12), s[n][lm] and q_nl (Eq. 17-18 route to Eq. 13), the network
 // (Eq. 21-22) and Fp = dU/dq, and hands U_i, Fp and s (rounded to fp32, relative error 6e-8) to k_main,
 // which then runs only its force phases P4 / P5 (their terms do not cancel).
-// One thread per atom in k_order's window-sorted order (the column k_main uses); s lives in local
-// memory: this is the accuracy path, not the throughput path.
+// One thread per atom in k_order's window-sorted order (the column k_main uses); the 24 lm components are
+// swept in three passes of 8 so that the 8 x 8 double accumulators stay in registers.
 #pragma once
+
+// fp64 geometry of neighbour `slot` of atom i: minimum-image r_ij from the fp64 positions, and Eq. 19's weight
+struct Nbr64 { double x, y, z, r, om; };
+__device__ __forceinline__ Nbr64 nbr64(const SysDev& d, const Box& b, const double4& pi, const double* zrow, int slot, int N, int i) {
+    const int j = d.jrev[(size_t)slot * N + i] & kJMask;
+    const double4 pj = d.xs4[j];
+    Nbr64 o;
+    o.x = min_image(pj.x - pi.x, b.L[0], b.invL[0]);
+    o.y = min_image(pj.y - pi.y, b.L[1], b.invL[1]);
+    o.z = min_image(pj.z - pi.z, b.L[2], b.invL[2]);
+    o.r = sqrt(o.x * o.x + o.y * o.y + o.z * o.z);
+    o.om = zrow[(int)__double_as_longlong(pj.w) & (kMaxTypes - 1)];
+    return o;
+}
+
+// One third of the angular sums (lm components 8 T .. 8 T + 7; 64 register accumulators): s, its share of
+// q_nl, and s rounded to fp32 into k_main's parked layout.  The first third also does Eq. 12 for the
+// angular neighbours.
+template <int T, int NR, int NA>
+__device__ __forceinline__ void desc64_third(const SysDev& d, const Box& b, const Desc64Params& P, const double4& pi,
+                                             const double* zrow, int i, int nA, size_t npad, size_t gcol, double* q) {
+    constexpr double C[kNumLM] = {NEP_CLM_LIST};
+    constexpr int LOF[kNumLM] = {NEP_LOF_LIST};
+    constexpr int NP = kHalfLM / 2;
+    const int N = P.N;
+    double s[NA][8];
+#pragma unroll
+    for (int n = 0; n < NA; ++n)
+#pragma unroll
+        for (int m = 0; m < 8; ++m) s[n][m] = 0.0;
+    for (int k = 0; k < nA; ++k) {
+        const Nbr64 e = nbr64(d, b, pi, zrow, k, N, i);
+        double g[NR > NA ? NR : NA];
+        if (T == 0) {
+            radial_g64<NR>(e.r, P.rcR, e.om, g);
+#pragma unroll
+            for (int n = 0; n < NR; ++n) q[n] += g[n];                   // Eq. 12
+        }
+        radial_g64<NA>(e.r, P.rcA, e.om, g);
+        double bb[kNumLM];
+        const double rinv = 1.0 / e.r;
+        ylm_basis64(e.x * rinv, e.y * rinv, e.z * rinv, bb);             // the unused components are dead code
+#pragma unroll
+        for (int n = 0; n < NA; ++n)
+#pragma unroll
+            for (int m = 0; m < 8; ++m) s[n][m] += g[n] * bb[8 * T + m];   // Eq. 18 in real form
+    }
+#pragma unroll
+    for (int n = 0; n < NA; ++n)
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+            constexpr int dummy = 0; (void)dummy;
+            const int gm = 8 * T + m;                                    // global lm index (compile-time after unrolling)
+            q[NR + 4 * n + LOF[gm] - 1] += C[gm] * s[n][m] * s[n][m];   // Eq. 17 with n' = n
+            // k_main's parked layout: half 0 holds m 0..2 and 15..23, half 1 holds m 3..14
+            const bool h0 = gm < 3 || gm >= 15;
+            const int kk = h0 ? (gm < 3 ? gm : gm - 12) : gm - 3;
+            float* base = reinterpret_cast<float*>(h0 ? d.spark0 : d.spark1);
+            base[((size_t)(n * NP + (kk >> 1)) * npad + gcol) * 2 + (kk & 1)] = (float)s[n][m];
+        }
+}
 
 template <int NR, int NA>
 __global__ void __launch_bounds__(64) k_desc64(SysDev d, Box b, const __grid_constant__ Desc64Params P,
@@ -31,40 +92,16 @@ __global__ void __launch_bounds__(64) k_desc64(SysDev d, Box b, const __grid_con
     double q[D];
 #pragma unroll
     for (int v = 0; v < D; ++v) q[v] = 0.0;
-    double s[NA][kNumLM];
-    for (int n = 0; n < NA; ++n)
-        for (int m = 0; m < kNumLM; ++m) s[n][m] = 0.0;
-
-    for (int k = 0; k < nR; ++k) {
-        const int slot = k < nA ? k : P.capR - 1 - (k - nA);
-        const int j = d.jrev[(size_t)slot * N + i] & kJMask;
-        const double4 pj = d.xs4[j];
-        const double dx = min_image(pj.x - pi.x, b.L[0], b.invL[0]);
-        const double dy = min_image(pj.y - pi.y, b.L[1], b.invL[1]);
-        const double dz = min_image(pj.z - pi.z, b.L[2], b.invL[2]);
-        const double r = sqrt(dx * dx + dy * dy + dz * dz);
-        const double om = zrow[(int)__double_as_longlong(pj.w) & (kMaxTypes - 1)];
-        double g[NR > NA ? NR : NA];
-        radial_g64<NR>(r, P.rcR, om, g);
+    for (int k = nA; k < nR; ++k) {                                      // Eq. 12, radial-only neighbours
+        const Nbr64 e = nbr64(d, b, pi, zrow, P.capR - 1 - (k - nA), N, i);
+        double g[NR];
+        radial_g64<NR>(e.r, P.rcR, e.om, g);
 #pragma unroll
-        for (int n = 0; n < NR; ++n) q[n] += g[n];                       // Eq. 12
-        if (k < nA) {
-            radial_g64<NA>(r, P.rcA, om, g);
-            double bb[kNumLM];
-            const double rinv = 1.0 / r;
-            ylm_basis64(dx * rinv, dy * rinv, dz * rinv, bb);
-            for (int n = 0; n < NA; ++n)
-#pragma unroll
-                for (int m = 0; m < kNumLM; ++m) s[n][m] += g[n] * bb[m];   // Eq. 18 in real form
-        }
+        for (int n = 0; n < NR; ++n) q[n] += g[n];
     }
-    for (int n = 0; n < NA; ++n) {
-        double ql[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-        for (int m = 0; m < kNumLM; ++m) ql[LOF[m] - 1] += C[m] * s[n][m] * s[n][m];   // Eq. 17 with n' = n
-#pragma unroll
-        for (int l = 0; l < 4; ++l) q[NR + 4 * n + l] = ql[l];
-    }
+    desc64_third<0, NR, NA>(d, b, P, pi, zrow, i, nA, npad, gcol, q);
+    desc64_third<1, NR, NA>(d, b, P, pi, zrow, i, nA, npad, gcol, q);
+    desc64_third<2, NR, NA>(d, b, P, pi, zrow, i, nA, npad, gcol, q);
 
     // network, Eq. 21-22 with the minus biases, and Fp = dU/dq
     const int H = P.H;
@@ -92,13 +129,4 @@ __global__ void __launch_bounds__(64) k_desc64(SysDev d, Box b, const __grid_con
     d.Us[i] = (float)U;
 #pragma unroll
     for (int v = 0; v < D; ++v) d.FpG[(size_t)v * npad + gcol] = (float)Fp[v];
-    // s in k_main's parked layout: half h, pair mm of radial index n
-    for (int n = 0; n < NA; ++n)
-#pragma unroll
-        for (int mm = 0; mm < NP; ++mm) {
-            d.spark0[(size_t)(n * NP + mm) * npad + gcol] =
-                make_float2((float)s[n][half_m<0>(2 * mm)], (float)s[n][half_m<0>(2 * mm + 1)]);
-            d.spark1[(size_t)(n * NP + mm) * npad + gcol] =
-                make_float2((float)s[n][half_m<1>(2 * mm)], (float)s[n][half_m<1>(2 * mm + 1)]);
-        }
 }

@@ -109,6 +109,16 @@ int  nep_get_neighbors(nep_system*, int which, int* count_dev, int* index_dev, v
 int  nep_compute(nep_system*, const double* pos_dev, const double* vel_dev, float* energy_dev,
                  float* force_dev, float* virial_dev, float* heat_dev, void* cuda_stream);
 
+/* Parity hook for the intermediate rows of the path: runs the same kernels as
+ * nep_compute up to the partial forces and copies out, in the caller's atom order,
+ *   q_dev  [D][N]  the descriptor q_i (Eq. 12-13; fp32, from the fp64 kernel for multi-species models)
+ *   fp_dev [D][N]  dU_i/dq (Eq. 21-23)
+ *   p_dev  [N][cap_radial][3]  dU_i/dr_ij (Eq. 23-25); neighbour k of atom i is entry k of
+ *          nep_get_neighbors(which = 0) called after this function
+ * Each pointer may be NULL.  Same preconditions and errors as nep_compute. */
+int  nep_compute_internals(nep_system* system, const double* pos_dev, float* q_dev, float* fp_dev, float* p_dev,
+                           void* cuda_stream);
+
 /* n_steps velocity-Verlet NVE steps (BASELINE.json north_star; the paper's own timing used NVT,
  * PAPER.md:395):  v += dt/2 F/m;  r += dt v;  [rebuild lists on device when an atom moved > skin/2];
  * evaluate;  v += dt/2 F/m;  J_i = W_i . v_i (Eq. 7, both at t+dt).  a = F / (m * 103.642697) A/fs^2.

@@ -15,7 +15,7 @@ _LIB_PATH = os.environ.get("NEP_B200_LIB", os.path.join(_HERE, "libnep_b200.so")
 _lib = None
 
 SYMBOLS = ["nep_create", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",
-           "nep_system_create", "nep_system_destroy", "nep_neighbors", "nep_get_neighbors", "nep_compute",
+           "nep_system_create", "nep_system_destroy", "nep_neighbors", "nep_get_neighbors", "nep_compute", "nep_compute_internals",
            "nep_md_step", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile", "nep_measure_fp32_peak", "nep_measure_fp32_patterns",
            "nep_strerror"]
 
@@ -48,6 +48,7 @@ def lib():
         L.nep_neighbors.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.nep_get_neighbors.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.nep_compute.argtypes = [C.c_void_p] * 8
+        L.nep_compute_internals.argtypes = [C.c_void_p] * 6
         L.nep_md_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int] + [C.c_void_p] * 7
         for f in ("nep_destroy", "nep_system_destroy"):
             getattr(L, f).argtypes = [C.c_void_p]
@@ -142,6 +143,16 @@ class System:
         _check(lib().nep_compute(self._h, _ptr(pos), _ptr(vel), _ptr(U), _ptr(F), _ptr(W), _ptr(J), _stream()),
                "nep_compute")
         return U, F, W, J
+
+    def compute_internals(self, pos):
+        """(q [D,N], dU/dq [D,N], p [N,cap_radial,3]) of the intermediate rows, for parity tests."""
+        dev = self.workspace.device
+        D = self.model.descriptor_dim
+        q = torch.zeros((D, self.n), dtype=torch.float32, device=dev)
+        fp = torch.zeros((D, self.n), dtype=torch.float32, device=dev)
+        p = torch.zeros((self.n, self.cap_radial, 3), dtype=torch.float32, device=dev)
+        _check(lib().nep_compute_internals(self._h, _ptr(pos), _ptr(q), _ptr(fp), _ptr(p), _stream()), "nep_compute_internals")
+        return q, fp, p
 
     def md_step(self, pos, vel, masses, dt, n_steps, out=None, heat_sum=None, thermo=None):
         assert pos.dtype == torch.float64 and vel.dtype == torch.float64 and pos.is_contiguous() and vel.is_contiguous()

@@ -81,6 +81,7 @@ struct Desc64Params {
     double rcR, rcA;
     double zz[kMaxTypes * kMaxTypes];     // sqrt(Z_a Z_b) in double
     int H, N, capR;
+    float* q_out;                         // nullable parity hook, [D][N] caller order
 };
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -109,6 +110,7 @@ struct nep_system {
     SysDev d;
     Box box;
     bool built, have_forces;
+    float* dump_q; float* dump_fp;        // set only inside nep_compute_internals
     cudaStream_t last_stream;
     // one MD step captured as a CUDA graph (replayed n_steps times; re-captured when its arguments change)
     cudaGraphExec_t step_graph;
@@ -419,6 +421,20 @@ __global__ void k_export_lists(SysDev d, int N, int which, int capR, int cap_out
     }
 }
 
+// partial forces dU_i/dr_ij in the caller's numbering, neighbour order of k_export_lists(which = 0)
+__global__ void k_export_p(SysDev d, int N, int capR, float* p_out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int nA = d.nnA[i], nR = d.nnR[i];
+    const int row = d.perm[i];
+    for (int k = 0; k < capR; ++k) {
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (k < nR) v = d.p[(size_t)i * capR + (k < nA ? k : capR - 1 - (k - nA))];
+        float* o = p_out + ((size_t)row * capR + k) * 3;
+        o[0] = v.x; o[1] = v.y; o[2] = v.z;
+    }
+}
+
 #ifndef NEP_MAIN_MIN_BLOCKS
 #define NEP_MAIN_MIN_BLOCKS 4
 #endif
@@ -711,6 +727,7 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
     MainParams P;
     P.rcR_inv = (float)(1.0 / m->h.rc_radial); P.rcA_inv = (float)(1.0 / m->h.rc_angular);
     P.H = m->H; P.N = (int)s->N; P.capR = s->capR;
+    P.q_out = MULTI ? nullptr : s->dump_q; P.fp_out = s->dump_fp;
     const size_t smem = ((size_t)m->params_floats + kMainWarps * main_warp_floats<NA, MULTI>()) * sizeof(float);
     static bool attr_done = false;
     if (!attr_done) {
@@ -722,7 +739,7 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
     const int windows = (int)((s->N + kWin - 1) / kWin);
     if (MULTI) {
         Desc64Params p64 = m->p64;
-        p64.N = (int)s->N; p64.capR = s->capR;
+        p64.N = (int)s->N; p64.capR = s->capR; p64.q_out = s->dump_q;
         k_desc64<NR, NA><<<windows * (kWin / 64), 64, 0, st>>>(s->d, s->box, p64, m->params64_dev);
         s->launches += 1;
     }
@@ -917,7 +934,7 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
     s->capMD = cap_md_of(m, cap_radial, skin);
     s->max_cells = max_cells_of(n_atoms);
     carve(n_atoms, s->capR, s->capMD, s->max_cells, m->NA, m->h.n_types > 1 ? m->D : 0, &s->d, (char*)workspace_dev);
-    s->built = false; s->have_forces = false; s->last_stream = nullptr; s->step_graph = nullptr; s->cap_stream = nullptr; s->g_launches = 0;
+    s->built = false; s->have_forces = false; s->dump_q = nullptr; s->dump_fp = nullptr; s->last_stream = nullptr; s->step_graph = nullptr; s->cap_stream = nullptr; s->g_launches = 0;
     s->launches = 0; s->prof_on = false; s->prof_n = 0;
     for (int k = 0; k < NEP_PHASES; ++k) { s->prof_ms[k] = 0.0; s->prof_cnt[k] = 0; }
     for (int k = 0; k < kProfMaxEvents; ++k) s->prof_ev[k] = nullptr;
@@ -1001,6 +1018,25 @@ int nep_compute(nep_system* s, const double* pos_dev, const double* vel_dev, flo
     k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
     phase(s, -1, st);
     s->launches += 2;
+    NEP_CUDA_OK(cudaGetLastError());
+    s->have_forces = false;
+    return NEP_OK;
+}
+
+int nep_compute_internals(nep_system* s, const double* pos_dev, float* q_dev, float* fp_dev, float* p_dev, void* cuda_stream) {
+    if (!s || !pos_dev) return NEP_EINVAL;
+    if (!s->built) return NEP_ESTATE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    s->last_stream = st;
+    const int N = (int)s->N;
+    const double hs = 0.5 * s->skin;
+    k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, nullptr, hs * hs * (1.0 + 1e-12) + 1e-24, 0);
+    launch_filter(s, st);
+    s->dump_q = q_dev; s->dump_fp = fp_dev;
+    launch_main(s, st);
+    s->dump_q = nullptr; s->dump_fp = nullptr;
+    if (p_dev) { k_export_p<<<grid_for(N, 128), 128, 0, st>>>(s->d, N, s->capR, p_dev); s->launches += 1; }
+    s->launches += 1;
     NEP_CUDA_OK(cudaGetLastError());
     s->have_forces = false;
     return NEP_OK;

@@ -127,6 +127,11 @@ __global__ void __launch_bounds__(64) k_desc64(SysDev d, Box b, const __grid_con
         for (int v = 0; v < D; ++v) Fp[v] += gm * w[v];
     }
     d.Us[i] = (float)U;
+    if (P.q_out) {                                                       // parity hook (nep_compute_internals)
+        const int row = d.perm[i];
+#pragma unroll
+        for (int v = 0; v < D; ++v) P.q_out[(size_t)v * N + row] = (float)q[v];
+    }
 #pragma unroll
     for (int v = 0; v < D; ++v) d.FpG[(size_t)v * npad + gcol] = (float)Fp[v];
 }

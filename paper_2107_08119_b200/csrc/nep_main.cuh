@@ -24,6 +24,8 @@ constexpr int kWin = 256;           // k_order's sort window (atoms)
 struct MainParams {
     float rcR_inv, rcA_inv;
     int H, N, capR;
+    float* q_out;          // nullable, [D][N] caller order: the descriptor q_i (nep_compute_internals)
+    float* fp_out;         // nullable, [D][N] caller order: dU_i/dq
 };
 
 // Packed FP32x2 arithmetic (sm_100+: FFMA2 issues two FMAs per lane in one instruction slot).
@@ -339,6 +341,11 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
         park(d.spark0);
         desc_half<1, NR, NA>(nA, P.rcA_inv, load_nbr, s2, q);
         park(d.spark1);
+        if (P.q_out && active) {                     // parity hook: the descriptor, in the caller's atom order
+            const int row = d.perm[i];
+#pragma unroll
+            for (int v = 0; v < D; ++v) P.q_out[(size_t)v * N + row] = q[v];
+        }
     }
 
     // ---- P3: network Eq. 21-22 (minus biases) and Fp = dU/dq; two neurons per iteration, weight rows
@@ -390,6 +397,11 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
         if (active) d.Us[i] = U;
     }
 
+    if (P.fp_out && active) {                        // parity hook: dU/dq
+        const int row = d.perm[i];
+#pragma unroll
+        for (int v = 0; v < D; ++v) P.fp_out[(size_t)v * N + row] = Fp[v];
+    }
     unpark(d.spark1);                                // half 1 comes back; its loads are in flight while P4 runs
 
     // ---- P4: radial-only neighbours, Eq. 24 ----

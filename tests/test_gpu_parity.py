@@ -160,3 +160,34 @@ def test_sampled_parity_large(oracle):
     assert np.abs(F.sum(1)).max() < 1e-3 * frms * np.sqrt(w.n_atoms)
     Wt = W.sum(1).reshape(3, 3)
     assert np.abs(Wt - Wt.T).max() < 1e-4 * np.abs(Wt).max()
+
+
+@pytest.mark.parametrize("which", ["c0", "c0_d45", "c2", "c3_replica"])
+def test_intermediate_rows_match_oracle(oracle, which):
+    """SURVEY.md 8(a) rows a3-a6 one by one: the descriptor q_i, dU_i/dq and every stored partial force
+    dU_i/dr_ij against the oracle's internals (matched by neighbour index)."""
+    torch, api = _gpu()
+    w, caps, skin = {"c0": (inputs.config0(), (64, 32), 0.4), "c0_d45": (inputs.config0(8), (64, 32), 0.4),
+                     "c2": (inputs.config2(), (80, 40), 1.0), "c3_replica": (inputs.config3(cells=(6, 6, 6)), (80, 40), 1.0)}[which]
+    model, system, pos, vel = api.from_workload(w, caps[0], caps[1], skin)
+    system.neighbors(pos, w.box)
+    q, fp, p = [t.cpu().numpy().astype(np.float64) for t in system.compute_internals(pos)]
+    cnt, idx = [t.cpu().numpy() for t in system.get_neighbors(0)]
+    system.status()
+    h = _hyper(oracle, w)
+    method = "brute" if w.n_atoms <= 8000 else "cell"
+    ocR, oiR, _ = oracle.neighbors(w.pos, w.box, w.rc_r, 96, method)
+    ocA, oiA, _ = oracle.neighbors(w.pos, w.box, w.rc_a, 64, method)
+    ref = oracle.compute(h, w.atomic_numbers, w.params, w.pos, w.vel, w.types, w.box, ocR, oiR, ocA, oiA, want_internals=True)
+    qs = np.abs(ref["q"]).max()
+    dq = np.abs(q.T - ref["q"]).max() / qs
+    dfp = np.abs(fp.T - ref["Fp"]).max() / np.abs(ref["Fp"]).max()
+    # partial forces: the GPU rows are in list order, the oracle's in ascending neighbour index
+    prms = np.sqrt((ref["p"] ** 2).sum() / max(1, ocR.sum()) / 3)
+    dp = 0.0
+    for i in range(w.n_atoms):
+        order = np.argsort(idx[i, :cnt[i]])
+        assert np.array_equal(idx[i, :cnt[i]][order], oiR[i, :ocR[i]])
+        dp = max(dp, np.abs(p[i, :cnt[i]][order] - ref["p"][i, :ocR[i]]).max(initial=0.0))
+    print(which, {"dq/max|q|": float("%.3g" % dq), "dFp/max|Fp|": float("%.3g" % dfp), "dp/rms(p)": float("%.3g" % (dp / prms))})
+    assert dq <= 2e-6 and dfp <= 2e-5 and dp <= TOL_REL * prms

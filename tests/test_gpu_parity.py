@@ -191,3 +191,13 @@ def test_intermediate_rows_match_oracle(oracle, which):
         dp = max(dp, np.abs(p[i, :cnt[i]][order] - ref["p"][i, :ocR[i]]).max(initial=0.0))
     print(which, {"dq/max|q|": float("%.3g" % dq), "dFp/max|Fp|": float("%.3g" % dfp), "dp/rms(p)": float("%.3g" % (dp / prms))})
     assert dq <= 2e-6 and dfp <= 2e-5 and dp <= TOL_REL * prms
+
+
+@pytest.mark.parametrize("n_neurons", [1, 17, 64])
+def test_network_widths(oracle, n_neurons):
+    """Odd, minimal and maximal hidden-layer widths (the network loop takes two neurons per iteration and
+    stages H weight rows in shared memory): C0 geometry, seeded weights of the given width."""
+    w = inputs.config0()
+    w.n_neurons = n_neurons
+    w.params = inputs.make_params(w.dim, n_neurons, 11)
+    run_config(oracle, w, skin=0.4, lists=False)

@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(kWin) k_order(SysDev d, int N) {
     int bin = kOrderBins - 1;                         // past N: sorts last
     if (i < N) {
         const int nA = d.nnA[i], nO = d.nnR[i] - nA;
-        bin = kOrderBins - 2 - (min(nA, 127) * 8 + min(nO >> 2, 7));     // descending key
+        bin = max(0, kOrderBins - 2 - (min(nA, 127) * 8 + min(max(nO, 0) >> 2, 7)));     // descending key
     }
     atomicAdd(&hist[bin], 1);
     __syncthreads();

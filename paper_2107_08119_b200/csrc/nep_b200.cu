@@ -330,16 +330,28 @@ __global__ void k_build_done(SysDev d, int gated) {
 // ------------------------------------------------------------------------------------------------
 // per-step list filter (the paper's "multiple levels of neighbor list")
 // ------------------------------------------------------------------------------------------------
-// One thread per sorted atom.  The predicate is the oracle's plain IEEE expression
+// The per-step filter of one sorted atom i (valid == false: a lane without atom, it only takes part in
+// the warp statistics).  The predicate is the oracle's plain IEEE expression
 //   d = (x_j - x_i) - L rint((x_j - x_i)/L);  (dx*dx + dy*dy) + dz*dz < rc*rc     (no FMA contraction)
 // so the sets agree bit for bit (reading Q9).  Angular neighbours (r < r_c^A) are packed
-// from slot 0 upwards, radial-only ones (r_c^A <= r < r_c^R) from slot capR-1 downwards.
-__global__ void __launch_bounds__(128) k_filter(SysDev d, int N, Box b, double rcR2, double rcA2, int capR, int capA,
-                                                int capMD) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
+// from slot 0 upwards, radial-only ones (r_c^A <= r < r_c^R) from slot capR-1 downwards.  Records,
+// jrev, the slot masks and the counts go to global memory (k_assemble reads them); with TO_SMEM the
+// caller is k_main and the records are also left in its shared-memory rows (column `lane`), so the
+// force evaluation starts without reading them back.
+struct FilterParams {
+    Box b;
+    double rcR2, rcA2;
+    int capR, capA;
+};
+
+template <bool TO_SMEM>
+__device__ __forceinline__ void filter_atom(const SysDev& d, int N, const FilterParams& F, int i, bool valid,
+                                            float4* srec, int rows_s, float4* praw, int rows_o, int lane,
+                                            int& nA_out, int& nR_out) {
+    const Box& b = F.b;
+    const int capR = F.capR;
     const double4 pi = d.xs4[i];
-    const int cnt = d.md_cnt[i];
+    const int cnt = valid ? d.md_cnt[i] : 0;
     int nA = 0, nO = 0;
     unsigned mR[4] = {0u, 0u, 0u, 0u}, mA[4] = {0u, 0u, 0u, 0u};
     constexpr int B = 8;                 // batch: B list entries, then B position gathers, in flight together
@@ -366,13 +378,18 @@ __global__ void __launch_bounds__(128) k_filter(SysDev d, int N, Box b, double r
             const double dy = min_image(pj.y - pi.y, b.L[1], b.invL[1]);
             const double dz = min_image(pj.z - pi.z, b.L[2], b.invL[2]);
             const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-            if (r2 < rcR2) {
-                const bool ang = r2 < rcA2;
+            if (r2 < F.rcR2) {
+                const bool ang = r2 < F.rcA2;
                 if (nA + nO < capR) {
                     const int slot = ang ? nA : capR - 1 - nO;
                     const int ty = (int)__double_as_longlong(pj.w);
-                    d.rec[(size_t)slot * N + i] = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(ty));
+                    const float4 rec = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(ty));
+                    d.rec[(size_t)slot * N + i] = rec;
                     d.jrev[(size_t)slot * N + i] = e;
+                    if (TO_SMEM) {
+                        if (ang) { if (nA < rows_s) srec[nA * 32 + lane] = rec; }
+                        else     { if (nO < rows_o) praw[nO * 32 + lane] = rec; }
+                    }
                 }
                 bR |= 1u << u;
                 if (ang) bA |= 1u << u;
@@ -385,22 +402,33 @@ __global__ void __launch_bounds__(128) k_filter(SysDev d, int N, Box b, double r
             if ((s0 >> 5) == wq) { mR[wq] |= bR << (s0 & 31); mA[wq] |= bA << (s0 & 31); }
     }
     const int nR = nA + nO;
-    const bool over = nR > capR || nA > capA;
-    d.nnA[i] = over ? 0 : nA;          // an overflowing atom is dropped (and reported), never truncated
-    d.nnR[i] = over ? 0 : nR;
-    if (over) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
-    d.masks[2 * (size_t)i] = make_uint4(mR[0], mR[1], mR[2], mR[3]);
-    d.masks[2 * (size_t)i + 1] = make_uint4(mA[0], mA[1], mA[2], mA[3]);
+    const bool over = nR > capR || nA > F.capA;
+    nA_out = over ? 0 : nA;            // an overflowing atom is dropped (and reported), never truncated
+    nR_out = over ? 0 : nR;
+    if (valid) {
+        d.nnA[i] = nA_out;
+        d.nnR[i] = nR_out;
+        if (over) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
+        d.masks[2 * (size_t)i] = make_uint4(mR[0], mR[1], mR[2], mR[3]);
+        d.masks[2 * (size_t)i + 1] = make_uint4(mA[0], mA[1], mA[2], mA[3]);
+    }
     // warp-aggregated statistics
     int xR = nR, xA = nA;
     for (int o = 16; o > 0; o >>= 1) {
         xR = max(xR, __shfl_xor_sync(0xffffffffu, xR, o));
         xA = max(xA, __shfl_xor_sync(0xffffffffu, xA, o));
     }
-    if ((threadIdx.x & 31) == 0) {
+    if (lane == 0) {
         if (xR > d.flags[F_MAXR]) atomicMax(&d.flags[F_MAXR], xR);
         if (xA > d.flags[F_MAXA]) atomicMax(&d.flags[F_MAXA], xA);
     }
+}
+
+// stand-alone filter: one thread per sorted atom (nep_neighbors, multi-species models, unfused runs)
+__global__ void __launch_bounds__(128) k_filter(SysDev d, int N, const __grid_constant__ FilterParams F) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int nA, nR;
+    filter_atom<false>(d, N, F, min(i, N - 1), i < N, nullptr, 0, nullptr, 0, threadIdx.x & 31, nA, nR);
 }
 
 // lists in the caller's numbering for nep_get_neighbors
@@ -762,12 +790,24 @@ void launch_main(nep_system* s, cudaStream_t st) {
 #endif
 }
 
-void launch_filter(nep_system* s, cudaStream_t st) {
+FilterParams filter_params(const nep_system* s) {
     const nep_hyper& h = s->model->h;
-    k_filter<<<grid_for(s->N, 128), 128, 0, st>>>(s->d, (int)s->N, s->box, h.rc_radial * h.rc_radial,
-                                                 h.rc_angular * h.rc_angular, s->capR, s->capA, s->capMD);
+    FilterParams F;
+    F.b = s->box;
+    F.rcR2 = h.rc_radial * h.rc_radial; F.rcA2 = h.rc_angular * h.rc_angular;
+    F.capR = s->capR; F.capA = s->capA;
+    return F;
+}
+
+void launch_order(nep_system* s, cudaStream_t st) {
     k_order<<<(int)((s->N + kWin - 1) / kWin), kWin, 0, st>>>(s->d, (int)s->N);
-    s->launches += 2;
+    s->launches += 1;
+}
+
+void launch_filter(nep_system* s, cudaStream_t st) {
+    k_filter<<<grid_for(s->N, 128), 128, 0, st>>>(s->d, (int)s->N, filter_params(s));
+    s->launches += 1;
+    launch_order(s, st);
 }
 
 void fill_masses(AsmParams* P, const nep_model* m, const double* mass_by_type) {

@@ -464,7 +464,7 @@ __global__ void k_export_p(SysDev d, int N, int capR, float* p_out) {
 }
 
 #ifndef NEP_MAIN_MIN_BLOCKS
-#define NEP_MAIN_MIN_BLOCKS 4
+#define NEP_MAIN_MIN_BLOCKS 2
 #endif
 #include "nep_main.cuh"
 #include "nep_desc64.cuh"
@@ -759,7 +759,7 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
     const size_t smem = ((size_t)m->params_floats + kMainWarps * main_warp_floats<NA, MULTI>()) * sizeof(float);
     static bool attr_done = false;
     if (!attr_done) {
-        cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+        cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
         cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributePreferredSharedMemoryCarveout,
                              cudaSharedmemCarveoutMaxShared);
         attr_done = true;

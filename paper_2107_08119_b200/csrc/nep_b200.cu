@@ -800,7 +800,7 @@ FilterParams filter_params(const nep_system* s) {
 }
 
 void launch_order(nep_system* s, cudaStream_t st) {
-    k_order<<<(int)((s->N + kWin - 1) / kWin), kWin, 0, st>>>(s->d, (int)s->N);
+    k_order<<<(int)((s->N + kWin - 1) / kWin), kOrderThreads, 0, st>>>(s->d, (int)s->N);
     s->launches += 1;
 }
 

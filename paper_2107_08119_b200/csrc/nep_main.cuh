@@ -2,7 +2,8 @@
 // anonymous namespace, after SysDev and nep_math.cuh).
 //
 // One thread per atom; a block is four independent warps that share only the staged network weights.
-// k_order sorts every window of 256 atoms by neighbour count, so the 32 atoms of a warp have (nearly)
+// k_order sorts every window of 4096 atoms by neighbour count (measured: windows of 256, 512, 1024, 4096, 16384
+// atoms -> 1.08, 1.06, 1.05, 1.02, 1.02 ms), so the 32 atoms of a warp have (nearly)
 // equal trip counts and the hardware block scheduler balances the windows' light and heavy blocks.
 // Per atom, in order:
 //   P0  all neighbour records of the atom (cp.async, every row in flight at once) and the weights
@@ -20,7 +21,7 @@
 
 constexpr int kRowsS = 24;          // angular neighbour rows staged in shared memory (more: read from global)
 constexpr int kRowsO = 20;          // radial-only neighbour rows staged in shared memory (more: read from global)
-constexpr int kWin = 256;           // k_order's sort window (atoms)
+constexpr int kWin = 4096;           // k_order's sort window (atoms)
 struct MainParams {
     float rcR_inv, rcA_inv;
     int H, N, capR;
@@ -56,27 +57,33 @@ __device__ __forceinline__ float fast_rcp(float x) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// k_order: order[w*256 + t] = the atom of window w with the t-th largest key; the key is the
-// angular count (exact, up to 127) and the radial-only count in steps of 4, so the 32 atoms of a warp
-// agree in nA and nearly in nR.  Entries past N are -1.  One block of 256 threads per window: a
-// counting sort (histogram, scan, cursor) in shared memory.
+// k_order: order[w*kWin + t] = the atom of window w with the t-th largest key; the key is the pair
+// (angular count, radial-only count), so the 32 atoms of a warp of k_main agree in nA and nearly in nR.
+// Entries past N are -1.  One block of 1024 threads per window of kWin atoms: a counting sort
+// (histogram, scan, cursor) in shared memory.
 // ------------------------------------------------------------------------------------------------
-constexpr int kOrderBins = 1024;
-__global__ void __launch_bounds__(kWin) k_order(SysDev d, int N) {
+constexpr int kOrderThreads = 1024;
+constexpr int kOrderItems = kWin / kOrderThreads;
+constexpr int kOrderBins = 4096;                    // 128 angular counts x 32 radial-only counts
+__global__ void __launch_bounds__(kOrderThreads) k_order(SysDev d, int N) {
     __shared__ int hist[kOrderBins];
-    __shared__ int wsum[kWin / 32];
+    __shared__ int wsum[kOrderThreads / 32];
     const int t = threadIdx.x;
-    const int i = blockIdx.x * kWin + t;
-    for (int b = t; b < kOrderBins; b += kWin) hist[b] = 0;
+    for (int b = t; b < kOrderBins; b += kOrderThreads) hist[b] = 0;
     __syncthreads();
-    int bin = kOrderBins - 1;                         // past N: sorts last
-    if (i < N) {
-        const int nA = d.nnA[i], nO = d.nnR[i] - nA;
-        bin = max(0, kOrderBins - 2 - (min(nA, 127) * 8 + min(max(nO, 0) >> 2, 7)));     // descending key
+    int bin[kOrderItems];
+#pragma unroll
+    for (int u = 0; u < kOrderItems; ++u) {
+        const int i = blockIdx.x * kWin + u * kOrderThreads + t;
+        bin[u] = kOrderBins - 1;                      // past N: sorts last
+        if (i < N) {
+            const int nA = d.nnA[i], nO = d.nnR[i] - nA;
+            bin[u] = max(0, kOrderBins - 2 - (min(nA, 127) * 32 + min(max(nO, 0), 31)));     // descending key
+        }
+        atomicAdd(&hist[bin[u]], 1);
     }
-    atomicAdd(&hist[bin], 1);
     __syncthreads();
-    // exclusive scan of the 1024 bins: 4 per thread, warp scan, then the 8 warp totals
+    // exclusive scan of the 4096 bins: 4 per thread, warp scan, then the 32 warp totals
     const int h0 = hist[4 * t], h1 = hist[4 * t + 1], h2 = hist[4 * t + 2], h3 = hist[4 * t + 3];
     const int mine = h0 + h1 + h2 + h3;
     int incl = mine;
@@ -91,8 +98,12 @@ __global__ void __launch_bounds__(kWin) k_order(SysDev d, int N) {
     __syncthreads();
     hist[4 * t] = base; hist[4 * t + 1] = base + h0; hist[4 * t + 2] = base + h0 + h1; hist[4 * t + 3] = base + h0 + h1 + h2;
     __syncthreads();
-    const int rank = atomicAdd(&hist[bin], 1);         // order inside a bin is arbitrary (equal keys)
-    d.order[blockIdx.x * kWin + rank] = i < N ? i : -1;
+#pragma unroll
+    for (int u = 0; u < kOrderItems; ++u) {
+        const int i = blockIdx.x * kWin + u * kOrderThreads + t;
+        const int rank = atomicAdd(&hist[bin[u]], 1);  // order inside a bin is arbitrary (equal keys)
+        d.order[blockIdx.x * kWin + rank] = i < N ? i : -1;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -8,8 +8,8 @@
 // Per atom, in order:
 //   P0  all neighbour records of the atom (cp.async, every row in flight at once) and the weights
 //       (once per block) are staged in shared memory
-//   P1  radial descriptor q_n (Eq. 12) over all r < r_c^R neighbours; the angular neighbours are left
-//       in shared memory as {r^_ij, r_ij}
+//   P1  radial descriptor q_n (Eq. 12): the radial-only neighbours here, the angular ones inside P2's first
+//       pass, which leaves them in shared memory as {r^_ij, r_ij}
 //   P2  angular sums s[n][lm] = sum_j g_n(r_ij) b_lm(r^_ij) (Eq. 17-18 route to Eq. 13) in two halves of
 //       12 lm (96 register accumulators each); a finished half is parked in coalesced, L2-resident rows
 //   P3  network (Eq. 21-22) and Fp = dU/dq with packed FMAs; weight rows are shared-memory broadcasts
@@ -289,7 +289,9 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
 #pragma unroll
         for (int n = 0; n < NR; ++n) q[n] += g[n];
     };
-    for (int k = 0; k < nA; k += 2) {                // two neighbours per iteration: independent chains
+    // (single-species models: the angular neighbours' share of Eq. 12 and their normalisation happen in the
+    //  first descriptor pass below, which touches them anyway)
+    for (int k = 0; MULTI && k < nA; k += 2) {       // two neighbours per iteration: independent chains
         const int k1 = min(k + 1, nA - 1);
         const float4 e0 = k < kRowsS ? srec[k * 32 + lane] : grec[(size_t)k * N];
         const float4 e1 = k1 < kRowsS ? srec[k1 * 32 + lane] : grec[(size_t)k1 * N];
@@ -348,7 +350,15 @@ __global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(S
     // Multi-species models: q, the network and the sums s come from k_desc64 (fp64; nep_desc64.cuh),
     // which has already filled Us, FpG and spark0 / spark1 -- P2 and P3 are skipped here.
     if (!MULTI) {
-        desc_half<0, NR, NA>(nA, P.rcA_inv, load_nbr, s2, q);
+        // first touch of an angular neighbour: raw record -> Eq. 12's share, then {r^, r} back into its row
+        auto load_first = [&](int k, float& x, float& y, float& z, float& r, float& om) {
+            const float4 e = k < kRowsS ? srec[k * 32 + lane] : grec[(size_t)k * N];
+            float rinv;
+            radial_acc(e, true, rinv, r, om);
+            x = e.x * rinv; y = e.y * rinv; z = e.z * rinv;
+            if (k < kRowsS) srec[k * 32 + lane] = make_float4(x, y, z, r);
+        };
+        desc_half<0, NR, NA>(nA, P.rcA_inv, load_first, s2, q);
         park(d.spark0);
         desc_half<1, NR, NA>(nA, P.rcA_inv, load_nbr, s2, q);
         park(d.spark1);

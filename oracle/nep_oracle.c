@@ -24,8 +24,10 @@
  * values, N_des/N_par printed by the paper, dimer/trimer closed forms, the
  * addition-theorem identity Eq. 17-18 via scipy's complex Y_lm, invariances,
  * F = -grad U and W = -dU/d(strain) by central differences, the heat-current
- * identity on an open cluster, brute-force vs cell-list neighbours, NVE.
- * Parity unpinned: the per-atom split of J beyond its definition Eq. 7.
+ * identity on an open cluster, brute-force vs cell-list neighbours, NVE; the PER-ATOM
+ * split of W_i and J_i = W_i . v_i through dU_j/dr_ji == dU_j/dr_i, i.e. central
+ * differences of the per-atom energies U_j as atom i moves (open cluster and periodic C0),
+ * with the transposed index order and p_ij-for-p_ji as failing negative controls.
  *
  * Layout: positions/velocities/forces SoA  x[N] | y[N] | z[N];  virial [9][N]
  * row-major (xx,xy,xz,yx,...), W^{ab} = sum_j r_ij^a (dU_j/dr_ji)^b.

@@ -183,3 +183,69 @@ def test_nve_conservation_and_dt_scaling(oracle):
     assert np.abs(back["vel"] + w.vel).max() < 1e-11
     # accumulated heat current equals the sum of per-step J (steps 1..n)
     assert np.allclose(out1["Jsum"].sum(1), out1["thermo"][1:, 2:5].sum(0), rtol=1e-10)
+
+
+def _per_atom_virial_fd(ev, pos, box, periodic, atoms, eps=1e-5):
+    """W_i^{ab} = sum_{j != i} r_ij^a dU_j/dr_i^b (Eq. 6 with dU_j/dr_ji == dU_j/dr_i):
+    the derivative by 4th-order central differences of the oracle's PER-ATOM energies U_j as atom i moves.
+    Also returns the 'wrong partial force' variant sum_j r_ij^a dU_i/dr_j^b (p_ij in place of p_ji)."""
+    n = pos.shape[1]
+    W = {}; Wwrong = {}
+    for i in atoms:
+        d = pos - pos[:, [i]]                                 # r_ij = r_j - r_i  (Eq. 3)
+        if periodic:
+            d -= box[:, None] * np.rint(d / box[:, None])
+        dUj_dri = np.zeros((n, 3))
+        for b in range(3):
+            def U_at(t):
+                pp = pos.copy(); pp[b, i] += t
+                return ev(pp)["U"]
+            dUj_dri[:, b] = (8 * (U_at(eps) - U_at(-eps)) - (U_at(2 * eps) - U_at(-2 * eps))) / (12 * eps)
+        dUj_dri[i] = 0.0                                      # j != i
+        W[i] = np.einsum("aj,jb->ab", d, dUj_dri)
+        # negative control: dU_i/dr_j (what Eq. 6 would be with p_ij instead of p_ji)
+        dUi_drj = np.zeros((n, 3))
+        for j in range(n):
+            if j == i or np.linalg.norm(d[:, j]) > 6.0:
+                continue
+            for b in range(3):
+                pp = pos.copy(); pp[b, j] += eps
+                pm = pos.copy(); pm[b, j] -= eps
+                dUi_drj[j, b] = (ev(pp)["U"][i] - ev(pm)["U"][i]) / (2 * eps)
+        Wwrong[i] = np.einsum("aj,jb->ab", d, dUi_drj)
+    return W, Wwrong
+
+
+@pytest.mark.parametrize("which", ["open_cluster", "c0_periodic"])
+def test_per_atom_virial_and_heat_current_from_site_energy_derivatives(oracle, which):
+    """Pins the PER-ATOM split of W_i (Eq. 6) and J_i (Eq. 7) with something other than the oracle's own
+    formula: dU_j/dr_ji == dU_j/dr_i, so W_i^{ab} = sum_j r_ij^a dU_j/dr_i^b follows from central
+    differences of the per-atom energies.  Negative controls: the transposed index order and p_ij in
+    place of p_ji both fail."""
+    w = inputs.config0()
+    h = _hyper(oracle, w)
+    if which == "open_cluster":
+        n = 14
+        u = inputs.uniform01(77, 3 * n).reshape(n, 3)
+        pos = np.ascontiguousarray((40.0 + (u - 0.5) * 6.0).T)
+        box = np.array([80.0, 80.0, 80.0])
+        vel = np.ascontiguousarray((inputs.normal(78, 3 * n).reshape(n, 3) * 0.01).T)
+        types = np.zeros(n, dtype=np.int32)
+        atoms = list(range(n)); periodic = False
+    else:
+        pos, box, vel, types = w.pos, w.box, w.vel, w.types
+        atoms = [0, 7, 13, 31, 50, 63]; periodic = True
+    ev = lambda p, v=None: oracle.evaluate(h, w.atomic_numbers, w.params, p, v, types, box)
+    out = ev(pos, vel)
+    Wfd, Wwrong = _per_atom_virial_fd(ev, pos, box, periodic, atoms)
+    scale = np.sqrt((out["W"] ** 2).mean())
+    worst_T = 0.0; worst_P = 0.0
+    for i in atoms:
+        Wi = out["W"][:, i].reshape(3, 3)
+        assert np.abs(Wi - Wfd[i]).max() < 1e-6 * max(scale, np.abs(Wi).max()), i
+        Ji = Wfd[i] @ vel[:, i]                                # Eq. 7: J^a = sum_b W^{ab} v^b
+        assert np.abs(out["J"][:, i] - Ji).max() < 1e-6 * max(np.abs(out["J"]).max(), 1e-12), i
+        worst_T = max(worst_T, np.abs(Wi.T - Wfd[i]).max() / scale)
+        worst_P = max(worst_P, np.abs(Wi - Wwrong[i]).max() / scale)
+    assert worst_T > 1e-2        # transposed indices: off by O(1)
+    assert worst_P > 1e-2        # p_ij in place of p_ji: off by O(1)

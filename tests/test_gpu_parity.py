@@ -60,10 +60,13 @@ def compare_outputs(out_gpu, ref, tol_u=TOL_U, tol_rel=TOL_REL, label=""):
         # the total heat current of a thermal crystal nearly cancels; compare it on the scale
         # sqrt(N) * rms(J_i) of a sum of N terms
         rep["dJtot"] = np.linalg.norm(J.sum(1) - ref["J"].sum(1)) / (jrms * np.sqrt(J.shape[1]))
+        # the literal reading of "within 1e-4 relative of its norm", printed beside it (not asserted:
+        # |sum J| is a cancelling sum ~ sqrt(N) rms(J_i); reading Q18)
+        rep["dJtot_plain"] = np.linalg.norm(J.sum(1) - ref["J"].sum(1)) / max(np.linalg.norm(ref["J"].sum(1)), 1e-300)
     print(label, {k: float("%.3g" % v) for k, v in rep.items()})
     assert rep["dU"] <= tol_u, rep
     for k, v in rep.items():
-        if k != "dU":
+        if k not in ("dU", "dJtot_plain"):
             assert v <= tol_rel, rep
     return rep
 

@@ -54,9 +54,9 @@ typedef struct {
     double rc_radial;       /* r_c^R, Angstrom                                                        */
     double rc_angular;      /* r_c^A, Angstrom, <= rc_radial                                          */
     int    n_max_radial;    /* 0..15                                                                  */
-    int    n_max_angular;   /* 0..15 (kernels are instantiated for n_max_angular+1 in {8, 9})         */
-    int    l_max;           /* must be 4 in this build                                                */
-    int    n_neurons;       /* N_neu, single hidden layer (Eq. 21-22), 1..64                          */
+    int    n_max_angular;   /* 0..15                                                                  */
+    int    l_max;           /* 1..4                                                                   */
+    int    n_neurons;       /* N_neu, single hidden layer (Eq. 21-22), 1..128                         */
     int    n_types;         /* 1..8; >1 switches on the sqrt(Z_i Z_j) weighting of Eq. 19             */
 } nep_hyper;
 
@@ -88,6 +88,19 @@ int  nep_system_create(const nep_model*, int64_t n_atoms, const int* type_dev, i
                        int cap_angular, double skin, void* workspace_dev, size_t workspace_bytes,
                        nep_system** out);
 void nep_system_destroy(nep_system*);
+
+/* Which kernel evaluates Eq. 12-25 (the descriptor, the network and the partial forces):
+ *   NEP_PATH_THREAD  one thread per atom (k_main): every per-atom quantity in registers; instantiated for
+ *                    n_max_radial == n_max_angular in {7, 8}, l_max == 4, n_neurons <= 64 -- the BASELINE.json
+ *                    shapes (D = 40 / 45); the fastest form once >~ 1.5e5 atoms fill the GPU
+ *   NEP_PATH_GROUP   eight lanes per atom (k_gen): any shape nep_create accepts, Table I's 80-50-1, 65-40-1 and
+ *                    41-40-1 models included; the form for small systems
+ * nep_system_create picks one from the shape and n_atoms (NEP_PATH_AUTO); nep_system_set_path overrides it
+ * (NEP_EINVAL if the thread path is not instantiated for the model).  Changing the path invalidates the
+ * lists: call nep_neighbors again.  Both paths produce the same quantities from the same lists. */
+enum { NEP_PATH_AUTO = 0, NEP_PATH_THREAD = 1, NEP_PATH_GROUP = 2 };
+int  nep_system_set_path(nep_system*, int path);
+int  nep_system_path(const nep_system*);
 
 /* Cell binning, cell sort and the Verlet list (cutoff r_c^R + skin) with reverse slots
  * ("smaller than r_c", "three neighbor lists").

@@ -11,11 +11,11 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.environ.get("NEP_B200_LIB", os.path.join(_HERE, "libnep_b200.so"))   # override: kernel experiments
+_LIB_PATH = os.path.join(_HERE, "libnep_b200.so")
 _lib = None
 
 SYMBOLS = ["nep_create", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",
-           "nep_system_create", "nep_system_destroy", "nep_neighbors", "nep_get_neighbors", "nep_compute", "nep_compute_internals",
+           "nep_system_create", "nep_system_destroy", "nep_system_set_path", "nep_system_path", "nep_neighbors", "nep_get_neighbors", "nep_compute", "nep_compute_internals",
            "nep_md_step", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile", "nep_measure_fp32_peak", "nep_measure_fp32_patterns",
            "nep_strerror"]
 
@@ -56,6 +56,8 @@ def lib():
         for f in ("nep_descriptor_dim", "nep_num_params", "nep_status"):
             getattr(L, f).argtypes = [C.c_void_p]
         L.nep_stats.argtypes = [C.c_void_p, C.c_void_p]
+        L.nep_system_set_path.argtypes = [C.c_void_p, C.c_int]
+        L.nep_system_path.argtypes = [C.c_void_p]
         L.nep_launch_count.argtypes = [C.c_void_p]
         L.nep_launch_count.restype = C.c_int64
         L.nep_profile.argtypes = [C.c_void_p, C.c_int]
@@ -119,6 +121,16 @@ class System:
         _check(lib().nep_system_create(model._h, self.n, _ptr(types), cap_radial, cap_angular, float(skin),
                                        C.c_void_p(self.workspace.data_ptr() + off), nbytes, C.byref(self._h)),
                "nep_system_create")
+
+    PATH_AUTO, PATH_THREAD, PATH_GROUP = 0, 1, 2
+
+    def set_path(self, path: int):
+        """nep_system_set_path: 0 auto, 1 one thread per atom (k_main), 2 eight lanes per atom (k_gen)."""
+        _check(lib().nep_system_set_path(self._h, int(path)), "nep_system_set_path")
+
+    @property
+    def path(self):
+        return lib().nep_system_path(self._h)
 
     def neighbors(self, pos: torch.Tensor, box):
         assert pos.is_cuda and pos.dtype == torch.float64 and pos.is_contiguous() and pos.shape == (3, self.n)
@@ -205,11 +217,13 @@ def measure_fp32_patterns():
     return out[0], out[1], out[2]
 
 
-def from_workload(w, cap_radial=64, cap_angular=32, skin=1.0, device="cuda:0"):
-    """Model + System + device tensors for a paper_2107_08119_b200.inputs.Workload."""
+def from_workload(w, cap_radial=64, cap_angular=32, skin=1.0, device="cuda:0", path=None):
+    """Model + System + device tensors for a paper_2107_08119_b200.inputs.Workload (path: nep_system_set_path)."""
     model = Model(w.rc_r, w.rc_a, w.n_max_r, w.n_max_a, w.l_max, w.n_neurons, w.atomic_numbers, w.params)
     types = torch.from_numpy(w.types).to(device)
     system = System(model, types, cap_radial, cap_angular, skin)
+    if path is not None:
+        system.set_path(path)
     pos = torch.from_numpy(w.pos).to(device).contiguous()
     vel = torch.from_numpy(w.vel).to(device).contiguous()
     return model, system, pos, vel

@@ -4,7 +4,8 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "nep_b200.cu")
-DEPS = [SRC, os.path.join(HERE, "csrc", "nep_math.cuh"), os.path.join(HERE, "..", "include", "nep_b200.h")]
+import glob
+DEPS = sorted(glob.glob(os.path.join(HERE, "csrc", "*.cu*")) + glob.glob(os.path.join(HERE, "..", "include", "*.h")))
 LIB = os.path.join(HERE, "libnep_b200.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-diag-suppress", "177"]

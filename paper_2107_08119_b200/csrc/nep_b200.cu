@@ -3,7 +3,7 @@
 // Data flow of one evaluation (all in the cell-sorted atom order):
 //   k_filter    Verlet list -> per-step radial/angular lists as records {r_ij (fp32 from an fp64
 //               minimum-image difference), j, type_j}; predicate |d|^2 < r_c^2 in fp64
-//   k_main      two lanes per atom: radial descriptor (Eq. 12), angular sums s[n][lm] (Eq. 17-18 route
+//   k_main      one thread per atom: radial descriptor (Eq. 12), angular sums s[n][lm] (Eq. 17-18 route
 //               to Eq. 13), network (Eq. 21-22) and dU/dq, partial forces (Eq. 23-25) -> p_ij
 //   k_assemble  F_i = sum_j (p_ij - p_ji), W_i = sum_j r_ij (x) p_ji (Eq. 4-6), second half-kick,
 //               J_i = W_i . v_i (Eq. 7), thermo sums; outputs in the caller's atom order
@@ -23,13 +23,14 @@ using namespace nepk;
 namespace {
 
 constexpr int kMaxTypes = 8;
-constexpr int kJMask = 0x00FFFFFF;            // sorted index of the neighbour (N < 2^24)
+constexpr unsigned kJMask = 0x00FFFFFFu;       // sorted index of the neighbour (N < 2^24)
+constexpr int kMaxCapMD = 124;                // Verlet slots per atom: the accepted-slot masks hold 128 bits
 constexpr double kAmuConv = 103.642697;       // 1 amu A^2/fs^2 in eV
 
 // device status / counter words (int32 each)
 enum { F_STATUS = 0, F_REBUILD = 1, F_STEP = 2, F_NREBUILD = 3, F_MAXR = 4, F_MAXA = 5, F_MAXMD = 6, F_BUILT = 7,
        F_COUNT = 16 };
-enum { ST_OVERFLOW = 1, ST_STALE = 2 };
+enum { ST_OVERFLOW = 1, ST_STALE = 2, ST_BADTYPE = 4 };
 
 struct Box {
     double L[3], invL[3];
@@ -56,20 +57,21 @@ struct SysDev {                 // device pointers into the caller's workspace
     float* Us;                  // [N] sorted site energies
     float4* Fself;              // [N] sum_j p_ij
     int* md_cnt;                // [N]
-    int* md_idx;                // [cap_md][N]  j | rev << 24
+    unsigned* md_idx;           // [cap_md][N]  j | rev << 24   (rev: slot of i in j's Verlet row, < 128)
     int* nnR;                   // [N]
     int* nnA;                   // [N]
-    float4* rec;                // [cap_R][N]  {dx, dy, dz, bits(md_slot | type_j << 8)}   (read by k_main)
-    int* jrev;                  // [cap_R][N]  j | rev << 24                               (read by k_assemble)
+    float4* rec;                // [cap_R][N]  {dx, dy, dz, bits(type_j)}                     (read by k_main, k_assemble)
+    unsigned* jrev;             // [cap_R][N]  j | rev << 24 of the same slots                 (read by k_assemble)
     uint4* masks;               // [N][2] bit s set: Verlet slot s is inside r_c^R ([0]) / r_c^A ([1])
     float4* p;                  // [N][cap_R] partial forces dU_i/dr_ij at the record slots
-    float2* spark0;             // [NA*6][ceil(N/256)*256] angular sums s[n][lm] of lm half 0 / half 1: parked here by k_main
+    float2* spark0;             // [NA*6][ceil(N/kWin)*kWin] angular sums s[n][lm] of lm half 0 / half 1: parked here by k_main
     float2* spark1;             //   (coalesced rows, L2-resident between write and read) while the registers hold other phases
-    float* FpG;                 // [D][ceil(N/256)*256] dU/dq from k_desc64 (multi-species models only)
-    int* order;                 // [ceil(N/256)*256] atoms of each 256-window sorted by neighbour count (-1: none)
+    float* FpG;                 // [D][ceil(N/kWin)*kWin] dU/dq from k_desc64 (multi-species models only)
+    int* order;                 // [ceil(N/kWin)*kWin] atoms of each kWin-atom window sorted by neighbour count (-1: none)
 };
 
-constexpr int kMaxH = 64;           // hidden neurons supported (weights are staged in shared memory by k_main)
+constexpr int kMaxH = 64;           // hidden neurons k_main supports (it stages the weights in shared memory)
+constexpr int64_t kThreadPathMinAtoms = 150000;   // nep_system_create: from here on k_main (one thread per atom) is chosen
 
 // sqrt(Z_a Z_b) of Eq. 19, passed to k_main by value (kernel-parameter constant bank)
 struct ZZParams {
@@ -98,8 +100,9 @@ struct nep_model {
     float* params_dev;          // staged fp32 layout: w1[H][Dp] (rows zero-padded) | b1[H] | w2[H] | b2 | pad
     int params_floats;
     ZZParams zz;
-    double* params64_dev;       // multi-species models: the Eq. 26 vector in double, caller order (k_desc64)
+    double* params64_dev;       // multi-species models: the Eq. 26 vector in double, caller order (k_desc64, k_gen<double>)
     Desc64Params p64;
+    bool thread_path_ok;        // k_main / k_desc64 are instantiated for this shape
 };
 
 struct nep_system {
@@ -110,6 +113,7 @@ struct nep_system {
     SysDev d;
     Box box;
     bool built, have_forces;
+    int path;                              // NEP_PATH_THREAD or NEP_PATH_GROUP: which kernel evaluates Eq. 12-25
     float* dump_q; float* dump_fp;        // set only inside nep_compute_internals
     cudaStream_t last_stream;
     // one MD step captured as a CUDA graph (replayed n_steps times; re-captured when its arguments change)
@@ -226,7 +230,7 @@ __global__ void k_gather_a(SysDev d, const double* __restrict__ xin, const doubl
     }
 }
 
-__global__ void k_gather_b(SysDev d, int N, int have_v, int gated) {
+__global__ void k_gather_b(SysDev d, int N, int have_v, int n_types, int gated) {
     if (gate_closed(d.flags, gated)) return;
     for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < N; k += gridDim.x * blockDim.x) {
 #pragma unroll
@@ -237,7 +241,8 @@ __global__ void k_gather_b(SysDev d, int N, int have_v, int gated) {
         }
         const int p = d.cell_of[k];
         d.perm[k] = p;
-        const int ty = d.type_in[p];
+        int ty = d.type_in[p];
+        if (ty < 0 || ty >= n_types) { atomicOr(&d.flags[F_STATUS], ST_BADTYPE); ty = 0; }    // reported by nep_status as NEP_EINVAL
         d.type_s[k] = ty;
         d.xs4[k] = make_double4(d.xref[k], d.xref[N + k], d.xref[2 * N + k], __longlong_as_double((long long)ty));
     }
@@ -262,8 +267,7 @@ __device__ __forceinline__ double min_image(double t, double L, double invL) { r
 // (neighbour cells are visited in ascending cell id; a cell's atoms are contiguous and ascending).
 __global__ void __launch_bounds__(128) k_build_md(SysDev d, int N, Box b, double rc2, int capMD, int gated) {
     if (gate_closed(d.flags, gated)) return;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
     const double xi = d.xs[i], yi = d.xs[N + i], zi = d.xs[2 * N + i];
     const int cx = cell_coord(xi, b.L[0], b.invL[0], b.nc[0]);
     const int cy = cell_coord(yi, b.L[1], b.invL[1], b.nc[1]);
@@ -299,24 +303,25 @@ __global__ void __launch_bounds__(128) k_build_md(SysDev d, int N, Box b, double
     d.md_cnt[i] = min(cnt, capMD);
     if (cnt > capMD) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
     atomicMax(&d.flags[F_MAXMD], cnt);
+    }
 }
 
 // reverse slot: position of i in j's (ascending) row, by binary search
 __global__ void __launch_bounds__(128) k_rev(SysDev d, int N, int gated) {
     if (gate_closed(d.flags, gated)) return;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
-    const int cnt = d.md_cnt[i];
-    for (int s = 0; s < cnt; ++s) {
-        const int j = d.md_idx[(size_t)s * N + i] & kJMask;
-        int lo = 0, hi = d.md_cnt[j] - 1, found = 0;
-        while (lo <= hi) {
-            const int mid = (lo + hi) >> 1;
-            const int v = d.md_idx[(size_t)mid * N + j] & kJMask;
-            if (v == i) { found = mid; break; }
-            if (v < i) lo = mid + 1; else hi = mid - 1;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+        const int cnt = d.md_cnt[i];
+        for (int s = 0; s < cnt; ++s) {
+            const int j = (int)(d.md_idx[(size_t)s * N + i] & kJMask);
+            int lo = 0, hi = d.md_cnt[j] - 1, found = 0;
+            while (lo <= hi) {
+                const int mid = (lo + hi) >> 1;
+                const int v = (int)(d.md_idx[(size_t)mid * N + j] & kJMask);
+                if (v == i) { found = mid; break; }
+                if (v < i) lo = mid + 1; else hi = mid - 1;
+            }
+            d.md_idx[(size_t)s * N + i] = (unsigned)j | ((unsigned)found << 24);
         }
-        d.md_idx[(size_t)s * N + i] = j | (found << 24);
     }
 }
 
@@ -330,49 +335,47 @@ __global__ void k_build_done(SysDev d, int gated) {
 // ------------------------------------------------------------------------------------------------
 // per-step list filter (the paper's "multiple levels of neighbor list")
 // ------------------------------------------------------------------------------------------------
-// The per-step filter of one sorted atom i (valid == false: a lane without atom, it only takes part in
-// the warp statistics).  The predicate is the oracle's plain IEEE expression
+// One thread per sorted atom i walks its Verlet row.  The predicate is the oracle's plain IEEE expression
 //   d = (x_j - x_i) - L rint((x_j - x_i)/L);  (dx*dx + dy*dy) + dz*dz < rc*rc     (no FMA contraction)
 // so the sets agree bit for bit (reading Q9).  Angular neighbours (r < r_c^A) are packed
 // from slot 0 upwards, radial-only ones (r_c^A <= r < r_c^R) from slot capR-1 downwards.  Records,
-// jrev, the slot masks and the counts go to global memory (k_assemble reads them); with TO_SMEM the
-// caller is k_main and the records are also left in its shared-memory rows (column `lane`), so the
-// force evaluation starts without reading them back.
+// jrev, the slot masks and the counts go to global memory (k_main and k_assemble read them).
 struct FilterParams {
     Box b;
     double rcR2, rcA2;
     int capR, capA;
 };
 
-template <bool TO_SMEM>
-__device__ __forceinline__ void filter_atom(const SysDev& d, int N, const FilterParams& F, int i, bool valid,
-                                            float4* srec, int rows_s, float4* praw, int rows_o, int lane,
-                                            int& nA_out, int& nR_out) {
+__global__ void __launch_bounds__(128) k_filter(SysDev d, int N, const __grid_constant__ FilterParams F) {
     const Box& b = F.b;
     const int capR = F.capR;
+    const int gi = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = gi < N;
+    const int i = min(gi, N - 1);                // a lane without atom only takes part in the warp statistics
+    const int lane = threadIdx.x & 31;
     const double4 pi = d.xs4[i];
     const int cnt = valid ? d.md_cnt[i] : 0;
     int nA = 0, nO = 0;
     unsigned mR[4] = {0u, 0u, 0u, 0u}, mA[4] = {0u, 0u, 0u, 0u};
     constexpr int B = 8;                 // batch: B list entries, then B position gathers, in flight together
-    int en[B];                          // list entries of the NEXT batch: their loads overlap this batch's gathers
+    unsigned en[B];                      // list entries of the NEXT batch: their loads overlap this batch's gathers
 #pragma unroll
-    for (int u = 0; u < B; ++u) en[u] = u < cnt ? d.md_idx[(size_t)u * N + i] : i;
+    for (int u = 0; u < B; ++u) en[u] = u < cnt ? d.md_idx[(size_t)u * N + i] : (unsigned)i;
     for (int s0 = 0; s0 < cnt; s0 += B) {
-        int eb[B];
+        unsigned eb[B];
         double4 pb[B];
 #pragma unroll
         for (int u = 0; u < B; ++u) eb[u] = en[u];
 #pragma unroll
         for (int u = 0; u < B; ++u) pb[u] = ldg256(&d.xs4[eb[u] & kJMask]);
 #pragma unroll
-        for (int u = 0; u < B; ++u) en[u] = s0 + B + u < cnt ? d.md_idx[(size_t)(s0 + B + u) * N + i] : i;
+        for (int u = 0; u < B; ++u) en[u] = s0 + B + u < cnt ? d.md_idx[(size_t)(s0 + B + u) * N + i] : (unsigned)i;
         unsigned bR = 0u, bA = 0u;
 #pragma unroll
         for (int u = 0; u < B; ++u) {
             const int s = s0 + u;
             if (s >= cnt) break;
-            const int e = eb[u];
+            const unsigned e = eb[u];
             const double4 pj = pb[u];
             const double dx = min_image(pj.x - pi.x, b.L[0], b.invL[0]);
             const double dy = min_image(pj.y - pi.y, b.L[1], b.invL[1]);
@@ -383,13 +386,8 @@ __device__ __forceinline__ void filter_atom(const SysDev& d, int N, const Filter
                 if (nA + nO < capR) {
                     const int slot = ang ? nA : capR - 1 - nO;
                     const int ty = (int)__double_as_longlong(pj.w);
-                    const float4 rec = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(ty));
-                    d.rec[(size_t)slot * N + i] = rec;
+                    d.rec[(size_t)slot * N + i] = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(ty));
                     d.jrev[(size_t)slot * N + i] = e;
-                    if (TO_SMEM) {
-                        if (ang) { if (nA < rows_s) srec[nA * 32 + lane] = rec; }
-                        else     { if (nO < rows_o) praw[nO * 32 + lane] = rec; }
-                    }
                 }
                 bR |= 1u << u;
                 if (ang) bA |= 1u << u;
@@ -403,11 +401,9 @@ __device__ __forceinline__ void filter_atom(const SysDev& d, int N, const Filter
     }
     const int nR = nA + nO;
     const bool over = nR > capR || nA > F.capA;
-    nA_out = over ? 0 : nA;            // an overflowing atom is dropped (and reported), never truncated
-    nR_out = over ? 0 : nR;
     if (valid) {
-        d.nnA[i] = nA_out;
-        d.nnR[i] = nR_out;
+        d.nnA[i] = over ? 0 : nA;          // an overflowing atom is dropped (and reported), never truncated
+        d.nnR[i] = over ? 0 : nR;
         if (over) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
         d.masks[2 * (size_t)i] = make_uint4(mR[0], mR[1], mR[2], mR[3]);
         d.masks[2 * (size_t)i + 1] = make_uint4(mA[0], mA[1], mA[2], mA[3]);
@@ -422,13 +418,6 @@ __device__ __forceinline__ void filter_atom(const SysDev& d, int N, const Filter
         if (xR > d.flags[F_MAXR]) atomicMax(&d.flags[F_MAXR], xR);
         if (xA > d.flags[F_MAXA]) atomicMax(&d.flags[F_MAXA], xA);
     }
-}
-
-// stand-alone filter: one thread per sorted atom (nep_neighbors, multi-species models, unfused runs)
-__global__ void __launch_bounds__(128) k_filter(SysDev d, int N, const __grid_constant__ FilterParams F) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    int nA, nR;
-    filter_atom<false>(d, N, F, min(i, N - 1), i < N, nullptr, 0, nullptr, 0, threadIdx.x & 31, nA, nR);
 }
 
 // lists in the caller's numbering for nep_get_neighbors
@@ -463,11 +452,9 @@ __global__ void k_export_p(SysDev d, int N, int capR, float* p_out) {
     }
 }
 
-#ifndef NEP_MAIN_MIN_BLOCKS
-#define NEP_MAIN_MIN_BLOCKS 2
-#endif
 #include "nep_main.cuh"
 #include "nep_desc64.cuh"
+#include "nep_gen.cuh"
 #include "fp32_peak.cuh"
 
 // ------------------------------------------------------------------------------------------------
@@ -513,7 +500,7 @@ __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
         float w[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         constexpr int B = 8;             // batch the three dependent loads (jrev -> masks -> p) for MLP
         for (int k0 = 0; k0 < nR; k0 += B) {
-            int jr[B];
+            unsigned jr[B];
             float4 eb[B], pb[B];
             uint4 mrb[B], mab[B];
 #pragma unroll
@@ -524,17 +511,14 @@ __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
                 eb[u] = d.rec[(size_t)slot * N + i];
             }
 #pragma unroll
-            for (int u = 0; u < B; ++u) {
-                const int j = jr[u] & kJMask;
-                ldg256(&d.masks[2 * (size_t)j], mrb[u], mab[u]);
-            }
+            for (int u = 0; u < B; ++u) ldg256(&d.masks[2 * (size_t)(jr[u] & kJMask)], mrb[u], mab[u]);
 #pragma unroll
             for (int u = 0; u < B; ++u) {
-                const int j = jr[u] & kJMask, rev = jr[u] >> 24;      // rev: Verlet slot of i in j's row
+                const int rev = (int)(jr[u] >> 24);                   // rev: Verlet slot of i in j's row
                 // record slot of i in j's row = rank of Verlet slot rev among j's accepted slots
                 const int cs = rank_below(mab[u], rev);
                 const int cslot = bit_set(mab[u], rev) ? cs : P.capR - 1 - (rank_below(mrb[u], rev) - cs);
-                pb[u] = d.p[(size_t)j * P.capR + cslot];              // dU_j/dr_ji
+                pb[u] = d.p[(size_t)(jr[u] & kJMask) * P.capR + cslot];      // dU_j/dr_ji
             }
 #pragma unroll
             for (int u = 0; u < B; ++u) {
@@ -675,7 +659,7 @@ int cap_md_of(const nep_model* m, int capR, double skin) {
     const double f = (m->h.rc_radial + skin) / m->h.rc_radial;
     int c = (int)ceil(capR * f * f * f);
     c = (c + 3) & ~3;
-    return c > 124 ? 124 : c;       // the reverse slot is stored in 7 bits
+    return c > kMaxCapMD ? kMaxCapMD : c;
 }
 
 struct Layout {
@@ -706,11 +690,11 @@ Layout carve(int64_t N, int capR, int capMD, int max_cells, int NA, int D64, Sys
     t.Us = (float*)take(n * 4);
     t.Fself = (float4*)take(n * 16);
     t.md_cnt = (int*)take(n * 4);
-    t.md_idx = (int*)take(n * 4 * capMD);
+    t.md_idx = (unsigned*)take(n * 4 * capMD);
     t.nnR = (int*)take(n * 4);
     t.nnA = (int*)take(n * 4);
     t.rec = (float4*)take(n * 16 * capR);
-    t.jrev = (int*)take(n * 4 * capR);
+    t.jrev = (unsigned*)take(n * 4 * capR);
     t.masks = (uint4*)take(n * 32);
     t.xs4 = (double4*)take(n * 32);
     t.p = (float4*)take(n * 16 * capR);
@@ -742,11 +726,18 @@ void launch_build(nep_system* s, const double* xin, const double* vin, int first
     k_fill<<<grid_stride(N), 256, 0, st>>>(d, N, gated);
     k_sort_cells<<<grid_stride(b.ncell), 256, 0, st>>>(d, b.ncell, gated);
     k_gather_a<<<grid_stride(N), 256, 0, st>>>(d, xin, vin, N, first, gated);
-    k_gather_b<<<grid_stride(N), 256, 0, st>>>(d, N, vin != nullptr, gated);
-    k_build_md<<<grid_for(N, 128), 128, 0, st>>>(d, N, b, rc * rc, s->capMD, gated);
-    k_rev<<<grid_for(N, 128), 128, 0, st>>>(d, N, gated);
+    k_gather_b<<<grid_stride(N), 256, 0, st>>>(d, N, vin != nullptr, s->model->h.n_types, gated);
+    const int gb = grid_for(N, 128) > 148 * 16 ? 148 * 16 : grid_for(N, 128);      // grid-stride: a closed gate costs few blocks
+    k_build_md<<<gb, 128, 0, st>>>(d, N, b, rc * rc, s->capMD, gated);
+    k_rev<<<gb, 128, 0, st>>>(d, N, gated);
     k_build_done<<<1, 1, 0, st>>>(d, gated);
     s->launches += kBuildLaunches;
+}
+
+constexpr int kMainSmemLimit = 112 * 1024;          // two blocks of k_main per SM
+template <int NA, bool MULTI>
+size_t main_smem_bytes(int params_floats) {
+    return ((size_t)params_floats + kMainWarps * main_warp_floats<NA, MULTI>()) * sizeof(float);
 }
 
 template <int NR, int NA, bool MULTI>
@@ -756,13 +747,15 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
     P.rcR_inv = (float)(1.0 / m->h.rc_radial); P.rcA_inv = (float)(1.0 / m->h.rc_angular);
     P.H = m->H; P.N = (int)s->N; P.capR = s->capR;
     P.q_out = MULTI ? nullptr : s->dump_q; P.fp_out = s->dump_fp;
-    const size_t smem = ((size_t)m->params_floats + kMainWarps * main_warp_floats<NA, MULTI>()) * sizeof(float);
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024);
-        cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                             cudaSharedmemCarveoutMaxShared);
-        attr_done = true;
+    const size_t smem = main_smem_bytes<NA, MULTI>(m->params_floats);
+    static bool attr_done[64] = {};                // per device: the attribute belongs to the (device, function) pair
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64 || !attr_done[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMainSmemLimit);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_main<NR, NA, MULTI>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                                        cudaSharedmemCarveoutMaxShared);
+        if (e == cudaSuccess && dev >= 0 && dev < 64) attr_done[dev] = true;      // on failure the launch below reports it
     }
     const int windows = (int)((s->N + kWin - 1) / kWin);
     if (MULTI) {
@@ -776,18 +769,52 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
 }
 
 bool main_supported(const nep_model* m) {
-    return ((m->NR == 8 && m->NA == 8) || (m->NR == 9 && m->NA == 9)) && m->H <= kMaxH;
+    if (!((m->NR == 8 && m->NA == 8) || (m->NR == 9 && m->NA == 9)) || m->H > kMaxH || m->h.l_max != 4) return false;
+    // the staged weights must fit beside the per-warp record rows (H = 64 with D = 45 and Eq. 19 does not)
+    const size_t smem = m->h.n_types > 1 ? main_smem_bytes<8, true>(m->params_floats) : main_smem_bytes<8, false>(m->params_floats);
+    return smem <= (size_t)kMainSmemLimit;
+}
+
+template <int NMAX, typename TD>
+void launch_gen_t(nep_system* s, cudaStream_t st) {
+    const nep_model* m = s->model;
+    GenParams P;
+    memset(&P, 0, sizeof(P));
+    P.rcR = m->h.rc_radial; P.rcA = m->h.rc_angular;
+    P.rcR_inv = (float)(1.0 / m->h.rc_radial); P.rcA_inv = (float)(1.0 / m->h.rc_angular);
+    for (int k = 0; k < kMaxTypes * kMaxTypes; ++k) { P.zz[k] = m->zz.zz[k]; P.zz64[k] = m->p64.zz[k]; }
+    P.NR = m->NR; P.NA = m->NA; P.LMAX = m->h.l_max; P.H = m->H; P.D = m->D; P.Dp = (m->D + 3) & ~3;
+    P.N = (int)s->N; P.capR = s->capR; P.box = s->box;
+    P.params = m->params_dev; P.params64 = m->params64_dev;
+    P.q_out = s->dump_q; P.fp_out = s->dump_fp;
+    const size_t smem = (size_t)kGenAtomsPerBlock * sizeof(GenSmem<NMAX, TD>);
+    static bool attr_done[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64 || !attr_done[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(k_gen<NMAX, TD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess && dev >= 0 && dev < 64) attr_done[dev] = true;          // on failure the launch below reports it
+    }
+    const int64_t need = (s->N + kGenAtomsPerBlock - 1) / kGenAtomsPerBlock;
+    const int64_t cap = 148 * 16;
+    k_gen<NMAX, TD><<<(int)(need < cap ? need : cap), 32 * kGenWarps, smem, st>>>(s->d, P);
+    s->launches += 1;
+}
+
+void launch_gen(nep_system* s, cudaStream_t st) {
+    const nep_model* m = s->model;
+    const bool multi = m->h.n_types > 1;
+    const bool small = m->NR <= 8 && m->NA <= 8;
+    if (small) { if (multi) launch_gen_t<8, double>(s, st); else launch_gen_t<8, float>(s, st); }
+    else       { if (multi) launch_gen_t<16, double>(s, st); else launch_gen_t<16, float>(s, st); }
 }
 
 void launch_main(nep_system* s, cudaStream_t st) {
     const nep_model* m = s->model;
     const bool multi = m->h.n_types > 1;
-#ifdef NEP_FAST_BUILD            // kernel experiments: one instantiation only
-    launch_main_t<8, 8, false>(s, st);
-#else
+    if (s->path == NEP_PATH_GROUP) { launch_gen(s, st); return; }
     if (m->NR == 8 && m->NA == 8) { if (multi) launch_main_t<8, 8, true>(s, st); else launch_main_t<8, 8, false>(s, st); }
     else if (m->NR == 9 && m->NA == 9) { if (multi) launch_main_t<9, 9, true>(s, st); else launch_main_t<9, 9, false>(s, st); }
-#endif
 }
 
 FilterParams filter_params(const nep_system* s) {
@@ -807,7 +834,7 @@ void launch_order(nep_system* s, cudaStream_t st) {
 void launch_filter(nep_system* s, cudaStream_t st) {
     k_filter<<<grid_for(s->N, 128), 128, 0, st>>>(s->d, (int)s->N, filter_params(s));
     s->launches += 1;
-    launch_order(s, st);
+    if (s->path == NEP_PATH_THREAD) launch_order(s, st);         // k_gen takes the atoms in sorted order as they are
 }
 
 void fill_masses(AsmParams* P, const nep_model* m, const double* mass_by_type) {
@@ -906,8 +933,8 @@ int nep_create(const nep_hyper* hy, const int* atomic_number, const double* para
     *out = nullptr;
     if (!(hy->rc_radial > 0.0) || !(hy->rc_angular > 0.0) || hy->rc_angular > hy->rc_radial) return NEP_EINVAL;
     if (hy->n_max_radial < 0 || hy->n_max_radial > 15 || hy->n_max_angular < 0 || hy->n_max_angular > 15) return NEP_EINVAL;
-    if (hy->l_max != 4) return NEP_EINVAL;
-    if (hy->n_neurons < 1 || hy->n_neurons > kMaxH) return NEP_EINVAL;
+    if (hy->l_max < 1 || hy->l_max > 4) return NEP_EINVAL;
+    if (hy->n_neurons < 1 || hy->n_neurons > kMaxHGen) return NEP_EINVAL;
     if (hy->n_types < 1 || hy->n_types > kMaxTypes) return NEP_EINVAL;
     if (hy->n_types > 1 && !atomic_number) return NEP_EINVAL;
     nep_model* m = new (std::nothrow) nep_model();
@@ -916,12 +943,13 @@ int nep_create(const nep_hyper* hy, const int* atomic_number, const double* para
     m->NR = hy->n_max_radial + 1; m->NA = hy->n_max_angular + 1; m->H = hy->n_neurons;
     m->D = m->NR + m->NA * hy->l_max;                    // Eq. 16
     m->npar = (m->D + 2) * m->H + 1;                     // Eq. 26
-    if (n_params != (size_t)m->npar || !main_supported(m)) { delete m; return NEP_EINVAL; }
-    if (!device_ok()) { delete m; set_cuda_error(cudaErrorNoDevice, "nep_create"); return NEP_ECUDA; }
-    for (int t = 0; t < kMaxTypes; ++t) m->Z[t] = (hy->n_types > 1 && t < hy->n_types) ? atomic_number[t] : 1;
     // staged fp32 layout: w1[H][Dp] (rows zero-padded to a multiple of 4) | b1[H] | w2[H] | b2
     const int H = m->H, D = m->D, Dp = (D + 3) & ~3;
     m->params_floats = (H * Dp + 2 * H + 1 + 3) & ~3;
+    if (n_params != (size_t)m->npar) { delete m; return NEP_EINVAL; }
+    m->thread_path_ok = main_supported(m);
+    if (!device_ok()) { delete m; set_cuda_error(cudaErrorNoDevice, "nep_create"); return NEP_ECUDA; }
+    for (int t = 0; t < kMaxTypes; ++t) m->Z[t] = (hy->n_types > 1 && t < hy->n_types) ? atomic_number[t] : 1;
     float* stage = new float[(size_t)m->params_floats]();
     for (int mu = 0; mu < H; ++mu)
         for (int v = 0; v < D; ++v) stage[mu * Dp + v] = (float)params[(size_t)mu * D + v];
@@ -932,12 +960,12 @@ int nep_create(const nep_hyper* hy, const int* atomic_number, const double* para
     if (e == cudaSuccess) e = cudaMemcpy(m->params_dev, stage, (size_t)m->params_floats * sizeof(float), cudaMemcpyHostToDevice);
     delete[] stage;
     m->params64_dev = nullptr;
+    m->p64.rcR = hy->rc_radial; m->p64.rcA = hy->rc_angular; m->p64.H = H;
+    for (int a = 0; a < kMaxTypes; ++a)
+        for (int b = 0; b < kMaxTypes; ++b) m->p64.zz[a * kMaxTypes + b] = sqrt((double)m->Z[a] * (double)m->Z[b]);   // Eq. 19
     if (e == cudaSuccess && hy->n_types > 1) {
         e = cudaMalloc(&m->params64_dev, (size_t)m->npar * sizeof(double));
         if (e == cudaSuccess) e = cudaMemcpy(m->params64_dev, params, (size_t)m->npar * sizeof(double), cudaMemcpyHostToDevice);
-        m->p64.rcR = hy->rc_radial; m->p64.rcA = hy->rc_angular; m->p64.H = H;
-        for (int a = 0; a < kMaxTypes; ++a)
-            for (int b = 0; b < kMaxTypes; ++b) m->p64.zz[a * kMaxTypes + b] = sqrt((double)m->Z[a] * (double)m->Z[b]);   // Eq. 19
     }
     if (e != cudaSuccess) { set_cuda_error(e, "nep_create"); nep_destroy(m); return NEP_ECUDA; }
     *out = m;
@@ -955,7 +983,7 @@ void nep_destroy(nep_model* m) {
 }
 
 size_t nep_workspace_bytes(const nep_model* m, int64_t n_atoms, int cap_radial, int cap_angular, double skin) {
-    if (!m || n_atoms < 1 || n_atoms >= (1 << 24) || cap_radial < 1 || cap_radial > 124 || cap_angular < 1 ||
+    if (!m || n_atoms < 1 || n_atoms >= (1 << 24) || cap_radial < 1 || cap_radial > kMaxCapMD || cap_angular < 1 ||
         cap_angular > cap_radial || !(skin >= 0.0))
         return 0;
     return carve(n_atoms, cap_radial, cap_md_of(m, cap_radial, skin), max_cells_of(n_atoms), m->NA, m->h.n_types > 1 ? m->D : 0, nullptr, nullptr).total;
@@ -973,6 +1001,9 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
     s->model = m; s->N = n_atoms; s->capR = cap_radial; s->capA = cap_angular; s->skin = skin;
     s->capMD = cap_md_of(m, cap_radial, skin);
     s->max_cells = max_cells_of(n_atoms);
+    // one thread per atom pays once the machine is full; below that (and for every shape k_main is not
+    // instantiated for) eight lanes share an atom
+    s->path = (m->thread_path_ok && n_atoms >= kThreadPathMinAtoms) ? NEP_PATH_THREAD : NEP_PATH_GROUP;
     carve(n_atoms, s->capR, s->capMD, s->max_cells, m->NA, m->h.n_types > 1 ? m->D : 0, &s->d, (char*)workspace_dev);
     s->built = false; s->have_forces = false; s->dump_q = nullptr; s->dump_fp = nullptr; s->last_stream = nullptr; s->step_graph = nullptr; s->cap_stream = nullptr; s->g_launches = 0;
     s->launches = 0; s->prof_on = false; s->prof_n = 0;
@@ -992,6 +1023,21 @@ void nep_system_destroy(nep_system* s) {
     for (int k = 0; k < kProfMaxEvents; ++k) if (s->prof_ev[k]) cudaEventDestroy(s->prof_ev[k]);
     delete s;
 }
+
+int nep_system_set_path(nep_system* s, int path) {
+    if (!s || (path != NEP_PATH_AUTO && path != NEP_PATH_THREAD && path != NEP_PATH_GROUP)) return NEP_EINVAL;
+    if (path == NEP_PATH_THREAD && !s->model->thread_path_ok) return NEP_EINVAL;
+    if (path == NEP_PATH_AUTO)
+        path = (s->model->thread_path_ok && s->N >= kThreadPathMinAtoms) ? NEP_PATH_THREAD : NEP_PATH_GROUP;
+    if (path != s->path) {
+        s->path = path;
+        s->built = false; s->have_forces = false;                      // k_order's output belongs to the thread path
+        if (s->step_graph) { cudaGraphExecDestroy(s->step_graph); s->step_graph = nullptr; }
+    }
+    return NEP_OK;
+}
+
+int nep_system_path(const nep_system* s) { return s ? s->path : NEP_EINVAL; }
 
 int nep_neighbors(nep_system* s, const double* pos_dev, const double box[3], void* cuda_stream) {
     if (!s || !pos_dev || !box) return NEP_EINVAL;
@@ -1144,6 +1190,7 @@ int nep_status(nep_system* s) {
     s->host_stats[0] = flags[F_NREBUILD]; s->host_stats[1] = flags[F_MAXR];
     s->host_stats[2] = flags[F_MAXA]; s->host_stats[3] = flags[F_MAXMD];
     if (flags[F_STATUS]) NEP_CUDA_OK(cudaMemset(s->d.flags + F_STATUS, 0, sizeof(int)));
+    if (flags[F_STATUS] & ST_BADTYPE) return NEP_EINVAL;
     if (flags[F_STATUS] & ST_OVERFLOW) return NEP_EOVERFLOW;
     if (flags[F_STATUS] & ST_STALE) return NEP_ESTALE;
     return NEP_OK;
@@ -1165,7 +1212,7 @@ int nep_measure_fp32_peak(double* tflops_ffma, double* tflops_ffma2, void* cuda_
     if (!device_ok()) { set_cuda_error(cudaErrorNoDevice, "nep_measure_fp32_peak"); return NEP_ECUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaDeviceProp prop;
-    NEP_CUDA_OK(cudaGetDeviceProperties(&prop, 0));
+    { int dev_ = 0; NEP_CUDA_OK(cudaGetDevice(&dev_)); NEP_CUDA_OK(cudaGetDeviceProperties(&prop, dev_)); }
     float* out = nullptr;
     NEP_CUDA_OK(cudaMalloc(&out, 16));
     cudaEvent_t e0, e1;
@@ -1195,7 +1242,7 @@ int nep_measure_fp32_patterns(double tflops[3], void* cuda_stream) {
     if (!device_ok()) { set_cuda_error(cudaErrorNoDevice, "nep_measure_fp32_patterns"); return NEP_ECUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaDeviceProp prop;
-    NEP_CUDA_OK(cudaGetDeviceProperties(&prop, 0));
+    { int dev_ = 0; NEP_CUDA_OK(cudaGetDevice(&dev_)); NEP_CUDA_OK(cudaGetDeviceProperties(&prop, dev_)); }
     float* out = nullptr;
     NEP_CUDA_OK(cudaMalloc(&out, 16));
     cudaEvent_t e0, e1;

@@ -225,7 +225,7 @@ template <int NA, bool MULTI>
 __host__ __device__ constexpr int main_warp_floats() { return (kRowsS + kRowsO) * 32 * 4 + (MULTI ? kRowsS * 32 : 0); }
 
 template <int NR, int NA, bool MULTI>
-__global__ void __launch_bounds__(32 * kMainWarps, NEP_MAIN_MIN_BLOCKS) k_main(SysDev d, MainParams P,
+__global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParams P,
                                                                               const float* __restrict__ params,
                                                                               const __grid_constant__ ZZParams Z) {
     constexpr int D = NR + 4 * NA;

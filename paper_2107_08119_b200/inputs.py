@@ -256,3 +256,56 @@ def config4(n_atoms: int = 1048576, n_max: int = 7) -> Workload:
 def si_cells(cells, sigma=0.1, seed_pos=8, seed_vel=9, n_max=7) -> Workload:
     """Any diamond-Si replica with the C4 seeds (used for bounded oracle samples)."""
     return _si_workload("si_%dx%dx%d" % tuple(cells), tuple(cells), sigma, seed_pos, seed_vel, n_max)
+
+
+# --------------------------------------------------------------------------- Table I shapes (PAPER.md:334-347)
+def _silicene_sheet(nx: int, ny: int, a: float = 3.87, buckling: float = 0.45, vacuum: float = 20.0):
+    """Buckled honeycomb sheet in an orthorhombic box: rectangular cell (a, a sqrt 3) with 4 atoms, the two
+    sublattices displaced by +-buckling/2 along z, a vacuum layer above (the 2-D geometry of PAPER.md:322)."""
+    b = a * math.sqrt(3.0)
+    basis = np.array([[0.0, 0.0, 0.0], [0.5, 0.5, 0.0], [0.0, 1.0 / 3.0, 1.0], [0.5, 5.0 / 6.0, 1.0]])
+    ix, iy = np.meshgrid(np.arange(nx), np.arange(ny), indexing="ij")
+    origin = np.stack([ix.ravel(), iy.ravel()], axis=1).astype(np.float64)
+    xy = (origin[:, None, :] + basis[None, :, :2]).reshape(-1, 2) * np.array([a, b])
+    z = 0.5 * vacuum + buckling * (np.tile(basis[:, 2], nx * ny) - 0.5)
+    r = np.concatenate([xy, z[:, None]], axis=1)
+    return r, np.array([nx * a, ny * b, vacuum])
+
+
+def table1(which: str, cells=None, sigma: float = 0.1) -> Workload:
+    """The paper's three model SHAPES (Table I; N_des/N_par at PAPER.md:361) with seeded
+    random weights (the trained ones do not exist here), on cells of the size the paper timed (8000-atom bulk
+    Si and PbTe, 6000-atom silicene):
+      "si"        n_max 15/15, r_c 5/5 A,     l_max 4, N_neu 50  -> 80-50-1   diamond Si, 10^3 cells
+      "silicene"  n_max 12/12, r_c 5.5/5.5 A, l_max 4, N_neu 40  -> 65-40-1   buckled 2-D sheet + vacuum, 30 x 50 cells
+      "pbte"      n_max 12/6,  r_c 8/4 A,     l_max 4, N_neu 40  -> 41-40-1   rock-salt PbTe, 10^3 cells, Eq. 19"""
+    if which == "si":
+        cells = cells or (10, 10, 10)
+        a = 5.431
+        box = np.array(cells, dtype=np.float64) * a
+        r = _jitter_wrap(_lattice(_DIAMOND_BASIS, a, cells), sigma, 21, box)
+        types = np.zeros(r.shape[0], dtype=np.int32)
+        masses, zs = np.array([MASS["Si"]]), np.array([ZNUM["Si"]], dtype=np.int32)
+        hyp = (5.0, 5.0, 15, 15, 4, 50)
+    elif which == "silicene":
+        cells = cells or (30, 50)
+        r0, box = _silicene_sheet(cells[0], cells[1])
+        r = _jitter_wrap(r0, sigma, 22, box)
+        types = np.zeros(r.shape[0], dtype=np.int32)
+        masses, zs = np.array([MASS["Si"]]), np.array([ZNUM["Si"]], dtype=np.int32)
+        hyp = (5.5, 5.5, 12, 12, 4, 40)
+    elif which == "pbte":
+        cells = cells or (10, 10, 10)
+        a = 6.46
+        box = np.array(cells, dtype=np.float64) * a
+        basis = np.concatenate([_FCC, _FCC + np.array([.5, 0, 0])])
+        r = _jitter_wrap(_lattice(basis, a, cells), sigma, 23, box)
+        types = np.tile(np.array([0, 0, 0, 0, 1, 1, 1, 1], dtype=np.int32), r.shape[0] // 8)
+        masses, zs = np.array([MASS["Pb"], MASS["Te"]]), np.array([ZNUM["Pb"], ZNUM["Te"]], dtype=np.int32)
+        hyp = (8.0, 4.0, 12, 6, 4, 40)
+    else:
+        raise ValueError(which)
+    vel = maxwell_boltzmann(masses[types], 300.0, 24)
+    dim = descriptor_dim(hyp[2], hyp[3], hyp[4])
+    return Workload("table1_" + which, np.ascontiguousarray(r.T), vel, types, box, hyp[0], hyp[1], hyp[2], hyp[3],
+                    hyp[4], hyp[5], zs, masses, make_params(dim, hyp[5], 25), 1.0, 100)

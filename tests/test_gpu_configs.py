@@ -34,13 +34,13 @@ def test_c2_d45(oracle):
     run_config(oracle, inputs.config2(n_max=8), cap_r=80, cap_a=40)
 
 
-def _md_leg(oracle, w, n_steps, cap_r, cap_a, min_rebuilds, label, traj_tol):
+def _md_leg(oracle, w, n_steps, cap_r, cap_a, min_rebuilds, label, traj_tol, path=1):
     """n_steps of nep_md_step against orc_md: (i) the trajectories stay together, (ii) the energy record
     follows the oracle's, (iii) the outputs of the last step meet the north-star bars against the oracle
     evaluated at the SAME final state (so trajectory divergence does not enter the comparison),
     (iv) the filtered lists at the final positions are bit-exact."""
     torch, api = _gpu()
-    model, system, pos, vel = api.from_workload(w, cap_r, cap_a, 1.0)
+    model, system, pos, vel = api.from_workload(w, cap_r, cap_a, 1.0, path=path)
     system.neighbors(pos, w.box)
     heat_sum = torch.zeros((3, w.n_atoms), dtype=torch.float64, device="cuda")
     thermo = torch.zeros((n_steps, 5), dtype=torch.float64, device="cuda")
@@ -75,8 +75,9 @@ def test_md_c2_amorphous_100_steps(oracle):
     _md_leg(oracle, inputs.config2(), 100, 80, 40, 2, "C2 a-Si 8000", 2e-3)
 
 
-def test_md_c3_pbte_64000(oracle):
-    _md_leg(oracle, inputs.config3(), 20, 80, 40, 1, "C3 PbTe 64000", 1e-4)
+@pytest.mark.parametrize("path", [1, 2])
+def test_md_c3_pbte_64000(oracle, path):
+    _md_leg(oracle, inputs.config3(), 20, 80, 40, 1, "C3 PbTe 64000 path %d" % path, 1e-4, path=path)
 
 
 def test_md_c4_32768_with_rebuild(oracle):

@@ -59,7 +59,7 @@ def test_error_codes(oracle):
         api.Model(w.rc_r, w.rc_a, 7, 7, 4, 30, w.atomic_numbers, w.params[:-1])
     assert e.value.code == -1
     with pytest.raises(api.NepError) as e:
-        api.Model(w.rc_r, w.rc_a, 7, 7, 3, 30, w.atomic_numbers, w.params)
+        api.Model(w.rc_r, w.rc_a, 7, 7, 5, 30, w.atomic_numbers, w.params)
     assert e.value.code == -1
     model, system, pos, vel = api.from_workload(w, 64, 32, 1.0)
     with pytest.raises(api.NepError) as e:            # compute before neighbors -> NEP_ESTATE
@@ -104,9 +104,9 @@ def test_compute_with_moved_positions_within_skin(oracle):
     compare_outputs(out, ref, label="C1 displaced")
 
 
-def _md_compare(oracle, w, n_steps, skin, cap_r=64, cap_a=32):
+def _md_compare(oracle, w, n_steps, skin, cap_r=64, cap_a=32, path=1):
     torch, api = _gpu()
-    model, system, pos, vel = api.from_workload(w, cap_r, cap_a, skin)
+    model, system, pos, vel = api.from_workload(w, cap_r, cap_a, skin, path=path)
     system.neighbors(pos, w.box)
     heat_sum = torch.zeros((3, w.n_atoms), dtype=torch.float64, device="cuda")
     thermo = torch.zeros((n_steps, 5), dtype=torch.float64, device="cuda")
@@ -116,10 +116,11 @@ def _md_compare(oracle, w, n_steps, skin, cap_r=64, cap_a=32):
     return system, pos.cpu().numpy(), vel.cpu().numpy(), out, heat_sum.cpu().numpy(), thermo.cpu().numpy(), ref
 
 
-def test_md_c0_trajectory_matches_oracle(oracle):
+@pytest.mark.parametrize("path", [1, 2])
+def test_md_c0_trajectory_matches_oracle(oracle, path):
     w = inputs.config0()
     n_steps = 50
-    system, pos, vel, out, hsum, thermo, ref = _md_compare(oracle, w, n_steps, 0.4)
+    system, pos, vel, out, hsum, thermo, ref = _md_compare(oracle, w, n_steps, 0.4, path=path)
     # fp32 forces vs fp64 forces: trajectories stay together over 50 fs
     assert np.abs(pos - ref["pos"]).max() < 2e-6
     assert np.abs(vel - ref["vel"]).max() < 2e-7

@@ -71,9 +71,11 @@ def compare_outputs(out_gpu, ref, tol_u=TOL_U, tol_rel=TOL_REL, label=""):
     return rep
 
 
-def run_config(oracle, w, cap_r=64, cap_a=32, skin=1.0, tol_u=TOL_U, tol_rel=TOL_REL, lists=True):
+def run_config(oracle, w, cap_r=64, cap_a=32, skin=1.0, tol_u=TOL_U, tol_rel=TOL_REL, lists=True, path=1):
+    """path = 1: one thread per atom (k_main), whatever the size -- the eight-lanes-per-atom path on the same
+    configs is tests/test_gpu_shapes.py."""
     torch, api = _gpu()
-    model, system, pos, vel = api.from_workload(w, cap_r, cap_a, skin)
+    model, system, pos, vel = api.from_workload(w, cap_r, cap_a, skin, path=path)
     assert model.descriptor_dim == w.dim and model.num_params == w.params.size
     system.neighbors(pos, w.box)
     out = system.compute(pos, vel)
@@ -136,6 +138,7 @@ def test_sampled_parity_large(oracle):
     torch, api = _gpu()
     w = inputs.config4(1048576)
     model, system, pos, vel = api.from_workload(w, 64, 32, 1.0)
+    assert system.path == 1                        # one thread per atom at this size
     system.neighbors(pos, w.box)
     U, F, W, J = [t.cpu().numpy().astype(np.float64) for t in system.compute(pos, vel)]
     system.status()
@@ -165,14 +168,15 @@ def test_sampled_parity_large(oracle):
     assert np.abs(Wt - Wt.T).max() < 1e-4 * np.abs(Wt).max()
 
 
+@pytest.mark.parametrize("path", [1, 2])
 @pytest.mark.parametrize("which", ["c0", "c0_d45", "c2", "c3_replica"])
-def test_intermediate_rows_match_oracle(oracle, which):
+def test_intermediate_rows_match_oracle(oracle, which, path):
     """SURVEY.md 8(a) rows a3-a6 one by one: the descriptor q_i, dU_i/dq and every stored partial force
     dU_i/dr_ij against the oracle's internals (matched by neighbour index)."""
     torch, api = _gpu()
     w, caps, skin = {"c0": (inputs.config0(), (64, 32), 0.4), "c0_d45": (inputs.config0(8), (64, 32), 0.4),
                      "c2": (inputs.config2(), (80, 40), 1.0), "c3_replica": (inputs.config3(cells=(6, 6, 6)), (80, 40), 1.0)}[which]
-    model, system, pos, vel = api.from_workload(w, caps[0], caps[1], skin)
+    model, system, pos, vel = api.from_workload(w, caps[0], caps[1], skin, path=path)
     system.neighbors(pos, w.box)
     q, fp, p = [t.cpu().numpy().astype(np.float64) for t in system.compute_internals(pos)]
     cnt, idx = [t.cpu().numpy() for t in system.get_neighbors(0)]

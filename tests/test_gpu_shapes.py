@@ -1,0 +1,130 @@
+"""GPU parity of the eight-lanes-per-atom path (k_gen, NEP_PATH_GROUP) and of the model shapes only it covers:
+the paper's three Table I models (80-50-1, 65-40-1, 41-40-1), n_max^R != n_max^A,
+l_max < 4 -- all against the fp64 oracle at the north-star bars (tests/test_gpu_parity.py)."""
+import numpy as np
+import pytest
+
+from paper_2107_08119_b200 import inputs
+from test_gpu_parity import TOL_REL, TOL_U, _gpu, _hyper, check_lists, compare_outputs
+
+pytestmark = pytest.mark.gpu
+
+GROUP, THREAD = 2, 1
+
+
+def _run(oracle, w, cap_r, cap_a, skin, path, lists=True, ocap=(96, 64)):
+    torch, api = _gpu()
+    model, system, pos, vel = api.from_workload(w, cap_r, cap_a, skin)
+    assert model.descriptor_dim == w.dim and model.num_params == w.params.size
+    if path is not None:
+        system.set_path(path)
+        assert system.path == path
+    system.neighbors(pos, w.box)
+    out = system.compute(pos, vel)
+    system.status()
+    if lists:
+        check_lists(oracle, w, system, cap_r, cap_a)
+    ref = oracle.evaluate(_hyper(oracle, w), w.atomic_numbers, w.params, w.pos, w.vel, w.types, w.box, ocap[0], ocap[1])
+    compare_outputs(out, ref, label="%s path %s" % (w.name, path))
+    return system, out
+
+
+@pytest.mark.parametrize("which", ["c0", "c0_d45", "c1", "c2", "dense", "c3_replica", "c4_32768"])
+def test_group_path_on_baseline_configs(oracle, which):
+    if which == "dense":
+        w = inputs.config2(n_atoms=1000, side=24.0)
+        w.rc_r, w.rc_a = 5.6, 4.6
+        caps, skin = (96, 48), 1.0
+    else:
+        w, caps, skin = {"c0": (inputs.config0(), (64, 32), 0.4), "c0_d45": (inputs.config0(8), (64, 32), 0.4),
+                         "c1": (inputs.config1(), (64, 32), 1.0), "c2": (inputs.config2(), (80, 40), 1.0),
+                         "c3_replica": (inputs.config3(cells=(6, 6, 6)), (80, 40), 1.0),
+                         "c4_32768": (inputs.config4(32768), (64, 32), 1.0)}[which]
+    _run(oracle, w, caps[0], caps[1], skin, GROUP)
+
+
+def test_auto_path_switches_with_size(oracle):
+    """nep_system_create picks eight lanes per atom for small systems and one thread per atom for large ones;
+    sizes on either side of the switch give the same results as the oracle (C4-32768 above, C4-262144 here)."""
+    torch, api = _gpu()
+    w_small = inputs.config4(32768)
+    _, s_small, _, _ = api.from_workload(w_small, 64, 32, 1.0)
+    assert s_small.path == GROUP
+    w_big = inputs.config4(262144)
+    system, out = _run(oracle, w_big, 64, 32, 1.0, None, ocap=(64, 32))
+    assert system.path == THREAD
+    system.set_path(GROUP)                                       # and the other kernel on the same system
+    pos = torch.from_numpy(w_big.pos).cuda(); vel = torch.from_numpy(w_big.vel).cuda()
+    system.neighbors(pos, w_big.box)
+    out2 = system.compute(pos, vel)
+    system.status()
+    for a, b, name in zip(out, out2, "UFWJ"):
+        scale = float(a.double().pow(2).mean().sqrt())
+        assert float((a - b).abs().max()) <= 2e-5 * max(scale, 1e-3), name
+
+
+@pytest.mark.parametrize("which", ["si", "silicene", "pbte"])
+def test_table1_model_shapes(oracle, which):
+    """The paper's own model shapes on cells of the size it timed: 8000-atom Si 80-50-1 at 5/5 A,
+    6000-atom silicene sheet 65-40-1 at 5.5/5.5 A, 8000-atom PbTe 41-40-1 at 8/4 A with Eq. 19 weights."""
+    w = inputs.table1(which)
+    assert (w.dim, w.params.size) == {"si": (80, 4101), "silicene": (65, 2681), "pbte": (41, 1721)}[which]
+    caps = {"si": (48, 48), "silicene": (32, 32), "pbte": (86, 16)}[which]
+    system, _ = _run(oracle, w, caps[0], caps[1], 1.0, None, ocap=(96, 64))
+    assert system.path == GROUP
+
+
+@pytest.mark.parametrize("shape", [(7, 7, 1), (7, 7, 2), (7, 7, 3), (4, 9, 4), (15, 3, 4), (0, 0, 1), (11, 5, 2)])
+def test_general_shapes_on_c0(oracle, shape):
+    """n_max^R != n_max^A (Eq. 12-13 leave them independent) and l_max = 1..3 (Eq. 16)."""
+    nr, na, lmax = shape
+    w = inputs.config0()
+    w.n_max_r, w.n_max_a, w.l_max = nr, na, lmax
+    w.params = inputs.make_params(w.dim, w.n_neurons, 31)
+    _run(oracle, w, 64, 32, 0.4, None, lists=False)
+
+
+def test_group_path_multispecies_table_shape_internals(oracle):
+    """Intermediate rows (q, dU/dq, every p_ij) of k_gen<double> on a PbTe replica with the Table I shape 12/6."""
+    torch, api = _gpu()
+    w = inputs.table1("pbte", cells=(5, 5, 5))
+    model, system, pos, vel = api.from_workload(w, 86, 16, 1.0)
+    system.neighbors(pos, w.box)
+    q, fp, p = [t.cpu().numpy().astype(np.float64) for t in system.compute_internals(pos)]
+    cnt, idx = [t.cpu().numpy() for t in system.get_neighbors(0)]
+    system.status()
+    h = _hyper(oracle, w)
+    ocR, oiR, _ = oracle.neighbors(w.pos, w.box, w.rc_r, 96, "brute")
+    ocA, oiA, _ = oracle.neighbors(w.pos, w.box, w.rc_a, 64, "brute")
+    ref = oracle.compute(h, w.atomic_numbers, w.params, w.pos, w.vel, w.types, w.box, ocR, oiR, ocA, oiA, want_internals=True)
+    dq = np.abs(q.T - ref["q"]).max() / np.abs(ref["q"]).max()
+    dfp = np.abs(fp.T - ref["Fp"]).max() / np.abs(ref["Fp"]).max()
+    prms = np.sqrt((ref["p"] ** 2).sum() / max(1, ocR.sum()) / 3)
+    dp = 0.0
+    for i in range(w.n_atoms):
+        order = np.argsort(idx[i, :cnt[i]])
+        assert np.array_equal(idx[i, :cnt[i]][order], oiR[i, :ocR[i]])
+        dp = max(dp, np.abs(p[i, :cnt[i]][order] - ref["p"][i, :ocR[i]]).max(initial=0.0))
+    print({"dq": dq, "dfp": dfp, "dp/rms": dp / prms})
+    assert dq <= 2e-6 and dfp <= 2e-5 and dp <= TOL_REL * prms
+
+
+def test_md_group_path_c1(oracle):
+    """100 NVE steps of C1 through k_gen (the path nep_system_create picks for 4096 atoms), with in-loop rebuilds."""
+    torch, api = _gpu()
+    w = inputs.config1()
+    model, system, pos, vel = api.from_workload(w, 64, 32, 1.0)
+    assert system.path == GROUP
+    system.neighbors(pos, w.box)
+    thermo = torch.zeros((100, 5), dtype=torch.float64, device="cuda")
+    out = system.md_step(pos, vel, w.masses, w.dt, 100, thermo=thermo)
+    system.status()
+    assert system.stats()["rebuilds"] >= 2
+    ref = oracle.md(_hyper(oracle, w), w.atomic_numbers, w.params, w.pos, w.vel, w.types, w.box, w.masses, w.dt, 100)
+    th = thermo.cpu().numpy()
+    E, Eref = th[:, 0] + th[:, 1], ref["thermo"][1:, 0] + ref["thermo"][1:, 1]
+    assert np.abs(E - Eref).max() / w.n_atoms < 1e-5
+    assert np.abs(pos.cpu().numpy() - ref["pos"]).max() < 1e-4
+    gpos, gvel = pos.cpu().numpy(), vel.cpu().numpy()
+    ref2 = oracle.evaluate(_hyper(oracle, w), w.atomic_numbers, w.params, gpos, gvel, w.types, w.box)
+    compare_outputs(out, ref2, label="C1 group path after 100 steps")

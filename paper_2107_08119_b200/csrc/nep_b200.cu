@@ -146,15 +146,16 @@ __device__ __forceinline__ int cell_coord(double x, double L, double invL, int n
 
 __device__ __forceinline__ bool gate_closed(const int* flags, int gated) { return gated && flags[F_REBUILD] == 0; }
 
-__global__ void k_clear_cells(SysDev d, int ncell, int gated) {
-    if (gate_closed(d.flags, gated)) return;
-    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c <= ncell; c += gridDim.x * blockDim.x) d.cell_cnt[c] = 0;
+// Each phase of the build is a device function over a flat thread index (tid of nth): the same bodies serve
+// the multi-kernel chain (large systems: one kernel per phase, all SMs) and k_build_cluster (small systems:
+// one launch, the phases separated by cluster barriers).
+__device__ __forceinline__ void ph_clear(const SysDev& d, int ncell, int tid, int nth) {
+    for (int c = tid; c <= ncell; c += nth) d.cell_cnt[c] = 0;
 }
 
 // cell id of every atom of the build input `x` ([3][N]) and the per-cell population
-__global__ void k_bin(SysDev d, const double* __restrict__ x, int N, Box b, int gated) {
-    if (gate_closed(d.flags, gated)) return;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+__device__ __forceinline__ void ph_bin(const SysDev& d, const double* __restrict__ x, int N, const Box& b, int tid, int nth) {
+    for (int i = tid; i < N; i += nth) {
         const int cx = cell_coord(x[i], b.L[0], b.invL[0], b.nc[0]);
         const int cy = cell_coord(x[N + i], b.L[1], b.invL[1], b.nc[1]);
         const int cz = cell_coord(x[2 * N + i], b.L[2], b.invL[2], b.nc[2]);
@@ -165,12 +166,10 @@ __global__ void k_bin(SysDev d, const double* __restrict__ x, int N, Box b, int 
 }
 
 // exclusive scan of cell_cnt[0..ncell) -> cell_start[0..ncell]; one block of 1024 threads
-__global__ void __launch_bounds__(1024) k_scan(SysDev d, int ncell, int gated) {
-    if (gate_closed(d.flags, gated)) return;
-    __shared__ int part[1024];
+__device__ __forceinline__ void ph_scan(const SysDev& d, int ncell, int* part /* shared, [1024] */) {
     const int t = threadIdx.x;
     const int per = (ncell + 1023) / 1024;
-    const int lo = t * per, hi = min(ncell, lo + per);
+    const int lo = min(ncell, t * per), hi = min(ncell, lo + per);
     int s = 0;
     for (int c = lo; c < hi; ++c) s += d.cell_cnt[c];
     part[t] = s;
@@ -190,18 +189,16 @@ __global__ void __launch_bounds__(1024) k_scan(SysDev d, int ncell, int gated) {
     if (t == 1023) d.cell_start[ncell] = part[1023];
 }
 
-__global__ void k_fill(SysDev d, int N, int gated) {
-    if (gate_closed(d.flags, gated)) return;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+__device__ __forceinline__ void ph_fill(const SysDev& d, int N, int tid, int nth) {
+    for (int i = tid; i < N; i += nth) {
         const int slot = atomicAdd(&d.cell_fill[d.cell_of[i]], 1);
         d.perm_tmp[slot] = i;
     }
 }
 
 // deterministic order inside a cell: ascending build-input index (insertion sort, cells are small)
-__global__ void k_sort_cells(SysDev d, int ncell, int gated) {
-    if (gate_closed(d.flags, gated)) return;
-    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += gridDim.x * blockDim.x) {
+__device__ __forceinline__ void ph_sort_cells(const SysDev& d, int ncell, int tid, int nth) {
+    for (int c = tid; c < ncell; c += nth) {
         const int lo = d.cell_start[c], hi = d.cell_start[c + 1];
         for (int a = lo + 1; a < hi; ++a) {
             const int v = d.perm_tmp[a];
@@ -214,11 +211,10 @@ __global__ void k_sort_cells(SysDev d, int ncell, int gated) {
 
 // Gather the build input into the new sorted order.  first != 0: input is the caller's arrays
 // (perm := perm_tmp).  first == 0 (in-loop rebuild): input is the current sorted state, so
-// perm := perm[perm_tmp]; velocities move too.  Two-phase through tmp buffers (k_gather_a/b).
-__global__ void k_gather_a(SysDev d, const double* __restrict__ xin, const double* __restrict__ vin, int N,
-                           int first, int gated) {
-    if (gate_closed(d.flags, gated)) return;
-    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < N; k += gridDim.x * blockDim.x) {
+// perm := perm[perm_tmp]; velocities move too.  Two-phase through tmp buffers (gather_a / gather_b).
+__device__ __forceinline__ void ph_gather_a(const SysDev& d, const double* __restrict__ xin, const double* __restrict__ vin,
+                                            int N, int first, int tid, int nth) {
+    for (int k = tid; k < N; k += nth) {
         const int src = d.perm_tmp[k];
 #pragma unroll
         for (int a = 0; a < 3; ++a) d.xref[a * N + k] = xin[a * N + src];
@@ -230,9 +226,8 @@ __global__ void k_gather_a(SysDev d, const double* __restrict__ xin, const doubl
     }
 }
 
-__global__ void k_gather_b(SysDev d, int N, int have_v, int n_types, int gated) {
-    if (gate_closed(d.flags, gated)) return;
-    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < N; k += gridDim.x * blockDim.x) {
+__device__ __forceinline__ void ph_gather_b(const SysDev& d, int N, int have_v, int n_types, int tid, int nth) {
+    for (int k = tid; k < N; k += nth) {
 #pragma unroll
         for (int a = 0; a < 3; ++a) d.xs[a * N + k] = d.xref[a * N + k];
         if (have_v) {
@@ -246,6 +241,37 @@ __global__ void k_gather_b(SysDev d, int N, int have_v, int n_types, int gated) 
         d.type_s[k] = ty;
         d.xs4[k] = make_double4(d.xref[k], d.xref[N + k], d.xref[2 * N + k], __longlong_as_double((long long)ty));
     }
+}
+
+__global__ void k_clear_cells(SysDev d, int ncell, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    ph_clear(d, ncell, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+__global__ void k_bin(SysDev d, const double* __restrict__ x, int N, Box b, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    ph_bin(d, x, N, b, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+__global__ void __launch_bounds__(1024) k_scan(SysDev d, int ncell, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    __shared__ int part[1024];
+    ph_scan(d, ncell, part);
+}
+__global__ void k_fill(SysDev d, int N, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    ph_fill(d, N, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+__global__ void k_sort_cells(SysDev d, int ncell, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    ph_sort_cells(d, ncell, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+__global__ void k_gather_a(SysDev d, const double* __restrict__ xin, const double* __restrict__ vin, int N,
+                           int first, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    ph_gather_a(d, xin, vin, N, first, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+__global__ void k_gather_b(SysDev d, int N, int have_v, int n_types, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    ph_gather_b(d, N, have_v, n_types, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
 
 // 256-bit read-only loads (sm_100: LDG.E.256): one request per gathered 32-byte sector instead of two
@@ -265,51 +291,51 @@ __device__ __forceinline__ double min_image(double t, double L, double invL) { r
 
 // Verlet list: all j != i with |r_ij|^2 < (r_c^R + skin)^2, rows ascending in the sorted index j
 // (neighbour cells are visited in ascending cell id; a cell's atoms are contiguous and ascending).
-__global__ void __launch_bounds__(128) k_build_md(SysDev d, int N, Box b, double rc2, int capMD, int gated) {
-    if (gate_closed(d.flags, gated)) return;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
-    const double xi = d.xs[i], yi = d.xs[N + i], zi = d.xs[2 * N + i];
-    const int cx = cell_coord(xi, b.L[0], b.invL[0], b.nc[0]);
-    const int cy = cell_coord(yi, b.L[1], b.invL[1], b.nc[1]);
-    const int cz = cell_coord(zi, b.L[2], b.invL[2], b.nc[2]);
-    int cells[27];
-    int ncells = 0;
-    const int wx = b.nc[0] > 1 ? 1 : 0, wy = b.nc[1] > 1 ? 1 : 0, wz = b.nc[2] > 1 ? 1 : 0;   // nc is 1 or >= 3
-    for (int ox = -wx; ox <= wx; ++ox)
-        for (int oy = -wy; oy <= wy; ++oy)
-            for (int oz = -wz; oz <= wz; ++oz) {
-                const int c = (((cx + ox + b.nc[0]) % b.nc[0]) * b.nc[1] + (cy + oy + b.nc[1]) % b.nc[1]) * b.nc[2] +
-                              (cz + oz + b.nc[2]) % b.nc[2];
-                int k = ncells++;
-                while (k > 0 && cells[k - 1] > c) { cells[k] = cells[k - 1]; --k; }
-                cells[k] = c;
-            }
-    int cnt = 0;
-    for (int q = 0; q < ncells; ++q) {
-        const int lo = d.cell_start[cells[q]], hi = d.cell_start[cells[q] + 1];
-        for (int j = lo; j < hi; ++j) {
-            if (j == i) continue;
-            const double4 pj = ldg256(&d.xs4[j]);
-            const double dx = min_image(pj.x - xi, b.L[0], b.invL[0]);
-            const double dy = min_image(pj.y - yi, b.L[1], b.invL[1]);
-            const double dz = min_image(pj.z - zi, b.L[2], b.invL[2]);
-            const double r2 = dx * dx + dy * dy + dz * dz;
-            if (r2 < rc2) {
-                if (cnt < capMD) d.md_idx[(size_t)cnt * N + i] = j;
-                ++cnt;
+// NC: read positions through the non-coherent path (valid when an earlier KERNEL wrote them).
+template <bool NC>
+__device__ __forceinline__ void ph_build_md(const SysDev& d, int N, const Box& b, double rc2, int capMD, int tid, int nth) {
+    for (int i = tid; i < N; i += nth) {
+        const double xi = d.xs[i], yi = d.xs[N + i], zi = d.xs[2 * N + i];
+        const int cx = cell_coord(xi, b.L[0], b.invL[0], b.nc[0]);
+        const int cy = cell_coord(yi, b.L[1], b.invL[1], b.nc[1]);
+        const int cz = cell_coord(zi, b.L[2], b.invL[2], b.nc[2]);
+        int cells[27];
+        int ncells = 0;
+        const int wx = b.nc[0] > 1 ? 1 : 0, wy = b.nc[1] > 1 ? 1 : 0, wz = b.nc[2] > 1 ? 1 : 0;   // nc is 1 or >= 3
+        for (int ox = -wx; ox <= wx; ++ox)
+            for (int oy = -wy; oy <= wy; ++oy)
+                for (int oz = -wz; oz <= wz; ++oz) {
+                    const int c = (((cx + ox + b.nc[0]) % b.nc[0]) * b.nc[1] + (cy + oy + b.nc[1]) % b.nc[1]) * b.nc[2] +
+                                  (cz + oz + b.nc[2]) % b.nc[2];
+                    int k = ncells++;
+                    while (k > 0 && cells[k - 1] > c) { cells[k] = cells[k - 1]; --k; }
+                    cells[k] = c;
+                }
+        int cnt = 0;
+        for (int q = 0; q < ncells; ++q) {
+            const int lo = d.cell_start[cells[q]], hi = d.cell_start[cells[q] + 1];
+            for (int j = lo; j < hi; ++j) {
+                if (j == i) continue;
+                const double4 pj = NC ? ldg256(&d.xs4[j]) : d.xs4[j];
+                const double dx = min_image(pj.x - xi, b.L[0], b.invL[0]);
+                const double dy = min_image(pj.y - yi, b.L[1], b.invL[1]);
+                const double dz = min_image(pj.z - zi, b.L[2], b.invL[2]);
+                const double r2 = dx * dx + dy * dy + dz * dz;
+                if (r2 < rc2) {
+                    if (cnt < capMD) d.md_idx[(size_t)cnt * N + i] = j;
+                    ++cnt;
+                }
             }
         }
-    }
-    d.md_cnt[i] = min(cnt, capMD);
-    if (cnt > capMD) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
-    atomicMax(&d.flags[F_MAXMD], cnt);
+        d.md_cnt[i] = min(cnt, capMD);
+        if (cnt > capMD) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
+        atomicMax(&d.flags[F_MAXMD], cnt);
     }
 }
 
 // reverse slot: position of i in j's (ascending) row, by binary search
-__global__ void __launch_bounds__(128) k_rev(SysDev d, int N, int gated) {
-    if (gate_closed(d.flags, gated)) return;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+__device__ __forceinline__ void ph_rev(const SysDev& d, int N, int tid, int nth) {
+    for (int i = tid; i < N; i += nth) {
         const int cnt = d.md_cnt[i];
         for (int s = 0; s < cnt; ++s) {
             const int j = (int)(d.md_idx[(size_t)s * N + i] & kJMask);
@@ -325,11 +351,59 @@ __global__ void __launch_bounds__(128) k_rev(SysDev d, int N, int gated) {
     }
 }
 
-__global__ void k_build_done(SysDev d, int gated) {
-    if (gate_closed(d.flags, gated)) return;
+__device__ __forceinline__ void ph_done(const SysDev& d) {
     d.flags[F_REBUILD] = 0;
     d.flags[F_NREBUILD] += 1;
     d.flags[F_BUILT] = 1;
+}
+
+__global__ void __launch_bounds__(128) k_build_md(SysDev d, int N, Box b, double rc2, int capMD, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    ph_build_md<true>(d, N, b, rc2, capMD, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+__global__ void __launch_bounds__(128) k_rev(SysDev d, int N, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    ph_rev(d, N, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+}
+
+// The whole build in ONE launch for small systems: a cluster of 8 CTAs x 1024 threads, phases separated by
+// cluster barriers (hardware barrier across the cluster's SMs, release/acquire at cluster scope).  A step
+// without rebuild then costs one early-exit launch instead of ten.
+constexpr int kClusterCTAs = 8;
+constexpr int64_t kClusterBuildMaxAtoms = 16384;
+__device__ __forceinline__ void cluster_barrier() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__global__ void __cluster_dims__(kClusterCTAs, 1, 1) __launch_bounds__(1024, 1)
+k_build_cluster(SysDev d, const double* xin, const double* vin, int N, Box b, double rc2,
+                int capMD, int first, int n_types, int gated) {
+    if (gate_closed(d.flags, gated)) return;               // uniform over the cluster: nobody reaches a barrier
+    __shared__ int part[1024];
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    ph_clear(d, b.ncell, tid, nth);
+    cluster_barrier();
+    ph_bin(d, xin, N, b, tid, nth);
+    cluster_barrier();
+    if (blockIdx.x == 0) ph_scan(d, b.ncell, part);
+    cluster_barrier();
+    ph_fill(d, N, tid, nth);
+    cluster_barrier();
+    ph_sort_cells(d, b.ncell, tid, nth);
+    cluster_barrier();
+    ph_gather_a(d, xin, vin, N, first, tid, nth);
+    cluster_barrier();
+    ph_gather_b(d, N, vin != nullptr, n_types, tid, nth);
+    cluster_barrier();
+    ph_build_md<false>(d, N, b, rc2, capMD, tid, nth);
+    cluster_barrier();
+    ph_rev(d, N, tid, nth);
+    cluster_barrier();
+    if (tid == 0) ph_done(d);
+}
+
+__global__ void k_build_done(SysDev d, int gated) {
+    if (gate_closed(d.flags, gated)) return;
+    ph_done(d);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -712,14 +786,17 @@ int max_cells_of(int64_t N) { return (int)(2 * N + 64); }
 int grid_for(int64_t n, int block) { return (int)((n + block - 1) / block); }
 int grid_stride(int64_t n) { int g = grid_for(n, 256); return g > 148 * 8 ? 148 * 8 : (g < 1 ? 1 : g); }
 
-constexpr int kBuildLaunches = 10;
-
 // the neighbour build as a fixed launch sequence; gated != 0: every kernel exits unless F_REBUILD is set
 void launch_build(nep_system* s, const double* xin, const double* vin, int first, int gated, cudaStream_t st) {
     const int N = (int)s->N;
     const SysDev& d = s->d;
     const Box& b = s->box;
     const double rc = s->model->h.rc_radial + s->skin;
+    if (s->N <= kClusterBuildMaxAtoms) {
+        k_build_cluster<<<kClusterCTAs, 1024, 0, st>>>(d, xin, vin, N, b, rc * rc, s->capMD, first, s->model->h.n_types, gated);
+        s->launches += 1;
+        return;
+    }
     k_clear_cells<<<grid_stride(b.ncell + 1), 256, 0, st>>>(d, b.ncell, gated);
     k_bin<<<grid_stride(N), 256, 0, st>>>(d, xin, N, b, gated);
     k_scan<<<1, 1024, 0, st>>>(d, b.ncell, gated);
@@ -731,7 +808,7 @@ void launch_build(nep_system* s, const double* xin, const double* vin, int first
     k_build_md<<<gb, 128, 0, st>>>(d, N, b, rc * rc, s->capMD, gated);
     k_rev<<<gb, 128, 0, st>>>(d, N, gated);
     k_build_done<<<1, 1, 0, st>>>(d, gated);
-    s->launches += kBuildLaunches;
+    s->launches += 10;
 }
 
 constexpr int kMainSmemLimit = 112 * 1024;          // two blocks of k_main per SM
@@ -787,13 +864,14 @@ void launch_gen_t(nep_system* s, cudaStream_t st) {
     P.N = (int)s->N; P.capR = s->capR; P.box = s->box;
     P.params = m->params_dev; P.params64 = m->params64_dev;
     P.q_out = s->dump_q; P.fp_out = s->dump_fp;
-    const size_t smem = (size_t)kGenAtomsPerBlock * sizeof(GenSmem<NMAX, TD>);
-    static bool attr_done[64] = {};
+    const size_t smem = (size_t)kGenAtomsPerBlock * sizeof(GenSmem<NMAX, TD>) +
+                        ((size_t)m->H * (sizeof(TD) == 8 ? (P.Dp | 1) : P.Dp + 4) + 2 * m->H + 1) * sizeof(TD);   // + the staged weights
+    static size_t attr_smem[64] = {};              // per device: the largest dynamic size this instantiation was opted in for
     int dev = 0;
     cudaGetDevice(&dev);
-    if (dev < 0 || dev >= 64 || !attr_done[dev]) {
+    if (dev < 0 || dev >= 64 || smem > attr_smem[dev]) {
         cudaError_t e = cudaFuncSetAttribute(k_gen<NMAX, TD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess && dev >= 0 && dev < 64) attr_done[dev] = true;          // on failure the launch below reports it
+        if (e == cudaSuccess && dev >= 0 && dev < 64) attr_smem[dev] = smem;          // on failure the launch below reports it
     }
     const int64_t need = (s->N + kGenAtomsPerBlock - 1) / kGenAtomsPerBlock;
     const int64_t cap = 148 * 16;

@@ -1,19 +1,19 @@
-// nep_gen.cuh -- k_gen: descriptor + network + partial forces for ANY model shape, eight lanes per atom
+// nep_gen.cuh -- k_gen: descriptor + network + partial forces for ANY model shape, a group of lanes per atom
 // (included by nep_b200.cu inside its anonymous namespace, after nep_main.cuh and nep_desc64.cuh).
 //
 // k_main (nep_main.cuh) is one thread per atom with everything in registers: the fastest form once a few
 // hundred thousand atoms fill the machine, but instantiated only for 8 or 9 radial functions per family and
 // serial in the atom (one warp = 32 atoms, ~35 us of dependent instructions).  k_gen is the cooperative form:
-// a group of 8 lanes owns one atom (4 atoms per warp), the runtime shape is free -- n_max^R, n_max^A up to
+// a group of G = 16 lanes owns one atom (2 atoms per warp), the runtime shape is free -- n_max^R, n_max^A up to
 // NMAX-1 (NMAX = 8 or 16), l_max = 1..4, any N_neu, Table I's models included -- and an
 // atom's work is spread over its lanes, so small systems (C0-C2, the paper's 8000-atom protocol,
 // PAPER.md:395) finish in a fraction of k_main's latency.  Per atom:
 //   R   q_n = sum_j g_n(r_ij), Eq. 12: lane = neighbour, partial sums in registers, shuffle reduction
-//   D   s[n][lm] = sum_j g_n(r_ij) b_lm(r^_ij) (Eq. 17-18 route to Eq. 13): a chunk of 8 neighbours leaves
-//       g_n and b_lm in shared memory (lane = neighbour), then lane = three lm columns accumulates
-//       its s[.][lm] in registers (no shuffles, no atomics); q_nl = sum_m C_lm s_nlm^2
+//   D   s[n][lm] = sum_j g_n(r_ij) b_lm(r^_ij) (Eq. 17-18 route to Eq. 13): a chunk of G neighbours leaves
+//       g_n and b_lm in shared memory (lane = neighbour), then lane = (three lm columns, a slice of n)
+//       accumulates its s[n][lm] in registers (no shuffles, no atomics); q_nl = sum_m C_lm s_nlm^2
 //   N   network Eq. 21-22 with the minus biases: lane = neuron for the forward sweep, lane = four
-//       descriptor components for dU/dq; weights come through L1 (ld.global.nc), never staged
+//       descriptor components for dU/dq; the weights are staged in shared memory once per (persistent) block
 //   F   A[n][lm] = 2 Fp_nl C_lm s_nlm in shared memory; lane = neighbour contracts it with g_n'(r_ij) and
 //       g_n(r_ij)/r_ij (broadcast reads) and applies the harmonic gradients: Eq. 23-25, p_ij to global memory
 // TD = float: everything in fp32.  TD = double (multi-species models): R, D and N in fp64 straight from the
@@ -21,9 +21,11 @@
 // pre-activations cancel); F stays fp32.
 #pragma once
 
-constexpr int kGenLanes = 8;                 // lanes per atom
+constexpr int kGenLanes = 16;                // lanes per atom (8: 27 us per C1 evaluation, 16: see DESIGN.md section 6)
+constexpr int kGenGroups = 32 / kGenLanes;   // atoms per warp
+constexpr int kGenSplit = kGenLanes / 8;     // the 8 lm triples x kGenSplit slices of n = the lanes of phase D
 constexpr int kGenWarps = 4;                 // warps per block
-constexpr int kGenAtomsPerBlock = kGenWarps * (32 / kGenLanes);
+constexpr int kGenAtomsPerBlock = kGenWarps * kGenGroups;
 constexpr int kMaxHGen = 128;                // hidden neurons (the paper's largest model has 50)
 
 struct GenParams {
@@ -40,10 +42,10 @@ struct GenParams {
 };
 
 template <int NMAX, typename TD>
-struct alignas(16) GenSmem {                 // per 8-lane group
+struct alignas(16) GenSmem {                 // per group of lanes
     TD S[NMAX][kNumLM];                      // s[n][lm], later (TD = float) A[n][lm] in place
-    TD Gs[kGenLanes][NMAX];                  // chunk: g_n of 8 neighbours
-    TD Bs[kGenLanes][kNumLM];                // chunk: b_lm of 8 neighbours
+    TD Gs[kGenLanes][NMAX + 1];              // chunk: g_n of G neighbours (odd row stride: conflict-free stores)
+    TD Bs[kGenLanes][kNumLM + 1];            // chunk: b_lm of G neighbours
     TD q[NMAX * 5];                          // descriptor
     float Fp[NMAX * 5];                      // dU/dq
     TD hid[kMaxHGen];                        // w2 (1 - tanh^2) per neuron
@@ -82,14 +84,32 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
     extern __shared__ __align__(16) unsigned char gsm_raw[];
     using SM = GenSmem<NMAX, TD>;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int grp = lane >> 3, gl = lane & 7;
-    SM& sm = reinterpret_cast<SM*>(gsm_raw)[warp * 4 + grp];
+    const int grp = lane / kGenLanes, gl = lane % kGenLanes;
+    SM& sm = reinterpret_cast<SM*>(gsm_raw)[warp * kGenGroups + grp];
     const int N = P.N, NR = P.NR, NA = P.NA, LMAX = P.LMAX, H = P.H, D = P.D, Dp = P.Dp, capR = P.capR;
-    const int nlm = LMAX * (LMAX + 2);                       // 3, 8, 15, 24 harmonics for l_max = 1..4
-    const float* b1f = P.params + (size_t)H * Dp;
-    const float* w2f = b1f + H;
+    // weights: staged once per block (the grid-stride loop below reuses them), rows padded by 4 floats so that
+    // the forward sweep's per-lane rows fall into distinct bank groups
+    const int Dps = F64 ? (Dp | 1) : Dp + 4;             // odd stride in 8-byte units for doubles
+    TD* wsm = reinterpret_cast<TD*>(gsm_raw + (size_t)kGenAtomsPerBlock * sizeof(SM));       // w1[H][Dps] | b1[H] | w2[H] | b2
+    {
+        for (int mu = warp; mu < H; mu += kGenWarps) {                    // one row per warp: every load in flight at once
+            TD* dst = wsm + mu * Dps;
+            if (F64) {
+                for (int v = lane; v < Dps; v += 32) dst[v] = v < D ? (TD)P.params64[(size_t)mu * D + v] : (TD)0;
+            } else {
+                for (int c = lane; c < Dp / 4; c += 32) cp_async16(dst + 4 * c, P.params + (size_t)mu * Dp + 4 * c);
+                if (lane < 4) dst[Dp + lane] = (TD)0;
+            }
+        }
+        for (int e = threadIdx.x; e < 2 * H + 1; e += blockDim.x)
+            wsm[H * Dps + e] = F64 ? (TD)P.params64[(size_t)H * D + e] : (TD)P.params[(size_t)H * Dp + e];
+        cp_async_wait_all();
+        __syncthreads();
+    }
+    const TD* b1s = wsm + H * Dps;
+    const TD* w2s = b1s + H;
 
-    for (int base = (blockIdx.x * kGenWarps + warp) * 4; base < N; base += gridDim.x * kGenAtomsPerBlock) {
+    for (int base = (blockIdx.x * kGenWarps + warp) * kGenGroups; base < N; base += gridDim.x * kGenAtomsPerBlock) {
         const int ia = base + grp;
         const bool valid = ia < N;
         const int i = valid ? ia : N - 1;
@@ -140,18 +160,19 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
 #pragma unroll
             for (int n = 0; n < NMAX; ++n) {
                 TD v = qa[n];
-                v += __shfl_xor_sync(0xffffffffu, v, 1);
-                v += __shfl_xor_sync(0xffffffffu, v, 2);
-                v += __shfl_xor_sync(0xffffffffu, v, 4);
-                if (gl == (n & 7) && n < NR) sm.q[n] = v;
+#pragma unroll
+                for (int o = 1; o < kGenLanes; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                if (gl == (n % kGenLanes) && n < NR) sm.q[n] = v;
             }
         }
 
         // ---- D: angular sums s[n][lm] and q_nl (Eq. 13 through Eq. 17-18 with n' = n) ----
         {
-            TD acc[NMAX][3];
+            constexpr int NH = NMAX / kGenSplit;                          // n slice of a lane
+            const int tl = gl & 7, hn = (gl >> 3) * NH;                   // lm triple 3 tl .. 3 tl + 2, n in hn .. hn + NH - 1
+            TD acc[NH][3];
 #pragma unroll
-            for (int n = 0; n < NMAX; ++n) { acc[n][0] = acc[n][1] = acc[n][2] = (TD)0; }
+            for (int n = 0; n < NH; ++n) { acc[n][0] = acc[n][1] = acc[n][2] = (TD)0; }
             for (int c = 0; c < chA; ++c) {
                 const int k = c * kGenLanes + gl;
                 TD g[NMAX], bb[kNumLM];
@@ -171,29 +192,31 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
 #pragma unroll
                 for (int m = 0; m < kNumLM; ++m) sm.Bs[gl][m] = bb[m];
                 __syncwarp();
+                const int kend = min(kGenLanes, __reduce_max_sync(0xffffffffu, nA) - c * kGenLanes);     // warp-uniform
 #pragma unroll
                 for (int kk = 0; kk < kGenLanes; ++kk) {
-                    const TD b0 = sm.Bs[kk][3 * gl], b1 = sm.Bs[kk][3 * gl + 1], b2 = sm.Bs[kk][3 * gl + 2];
+                    if (kk >= kend) break;                                // warp-uniform
+                    const TD b0 = sm.Bs[kk][3 * tl], b1 = sm.Bs[kk][3 * tl + 1], b2 = sm.Bs[kk][3 * tl + 2];
 #pragma unroll
-                    for (int n = 0; n < NMAX; ++n) {
-                        const TD gn = sm.Gs[kk][n];
+                    for (int n = 0; n < NH; ++n) {
+                        const TD gn = sm.Gs[kk][hn + n];
                         acc[n][0] += gn * b0; acc[n][1] += gn * b1; acc[n][2] += gn * b2;
                     }
                 }
                 __syncwarp();
             }
 #pragma unroll
-            for (int n = 0; n < NMAX; ++n) {
-                sm.S[n][3 * gl] = acc[n][0]; sm.S[n][3 * gl + 1] = acc[n][1]; sm.S[n][3 * gl + 2] = acc[n][2];
+            for (int n = 0; n < NH; ++n) {
+                sm.S[hn + n][3 * tl] = acc[n][0]; sm.S[hn + n][3 * tl + 1] = acc[n][1]; sm.S[hn + n][3 * tl + 2] = acc[n][2];
             }
             __syncwarp();
-            for (int o = gl; o < NA * LMAX; o += kGenLanes) {            // q_nl, descriptor order n-major, l = 1..l_max
-                const int n = o / LMAX, l = o - n * LMAX + 1;
-                TD v = (TD)0;
+            for (int n = gl; n < NA; n += kGenLanes) {                   // q_nl, descriptor order n-major, l = 1..l_max
+                TD v[4] = {(TD)0, (TD)0, (TD)0, (TD)0};
 #pragma unroll
-                for (int m = 0; m < kNumLM; ++m)
-                    if (LOF[m] == l) v += (TD)C[m] * sm.S[n][m] * sm.S[n][m];
-                sm.q[NR + o] = v;
+                for (int m = 0; m < kNumLM; ++m) { const TD sv = sm.S[n][m]; v[LOF[m] - 1] += (TD)C[m] * sv * sv; }
+#pragma unroll
+                for (int l = 0; l < 4; ++l)
+                    if (l < LMAX) sm.q[NR + n * LMAX + l] = v[l];
             }
             __syncwarp();
         }
@@ -208,53 +231,32 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
             __syncwarp();
             TD Upart = (TD)0;
             for (int mu = gl; mu < H; mu += kGenLanes) {
-                TD a, w2;
-                if (F64) {
-                    const double* w = P.params64 + (size_t)mu * D;
-                    double a0 = -P.params64[(size_t)H * D + mu], a1 = 0.0;
-                    int v = 0;
-                    for (; v + 1 < D; v += 2) { a0 += w[v] * (double)sm.q[v]; a1 += w[v + 1] * (double)sm.q[v + 1]; }
-                    if (v < D) a0 += w[v] * (double)sm.q[v];
-                    a = (TD)(a0 + a1);
-                    w2 = (TD)P.params64[(size_t)H * D + H + mu];
-                } else {
-                    const float4* w = reinterpret_cast<const float4*>(P.params + (size_t)mu * Dp);
-                    float a0 = -__ldg(&b1f[mu]), a1 = 0.f, a2 = 0.f, a3 = 0.f;
-                    for (int v = 0; v < Dp / 4; ++v) {                  // padded columns of w1 are zero; q is padded with zeros below
-                        const float4 ww = __ldg(&w[v]);
-                        a0 = fmaf(ww.x, (float)sm.q[4 * v], a0); a1 = fmaf(ww.y, (float)sm.q[4 * v + 1], a1);
-                        a2 = fmaf(ww.z, (float)sm.q[4 * v + 2], a2); a3 = fmaf(ww.w, (float)sm.q[4 * v + 3], a3);
-                    }
-                    a = (TD)((a0 + a1) + (a2 + a3));
-                    w2 = (TD)__ldg(&w2f[mu]);
+                const TD* w = wsm + mu * Dps;
+                TD a0 = -b1s[mu], a1 = (TD)0, a2 = (TD)0, a3 = (TD)0;
+#pragma unroll 4
+                for (int v = 0; v < Dp; v += 4) {                       // padded columns of w1 and the padded tail of q are zero
+                    a0 += w[v] * sm.q[v]; a1 += w[v + 1] * sm.q[v + 1]; a2 += w[v + 2] * sm.q[v + 2]; a3 += w[v + 3] * sm.q[v + 3];
                 }
+                const TD a = (a0 + a1) + (a2 + a3);
+                const TD w2 = w2s[mu];
                 TD t, dd;
                 GenMath<TD>::act(a, &t, &dd);
                 Upart += w2 * t;
                 sm.hid[mu] = w2 * dd;
             }
-            Upart += __shfl_xor_sync(0xffffffffu, Upart, 1);
-            Upart += __shfl_xor_sync(0xffffffffu, Upart, 2);
-            Upart += __shfl_xor_sync(0xffffffffu, Upart, 4);
+#pragma unroll
+            for (int o = 1; o < kGenLanes; o <<= 1) Upart += __shfl_xor_sync(0xffffffffu, Upart, o);
             __syncwarp();
             if (gl == 0 && valid) {
-                const TD b2 = F64 ? (TD)P.params64[(size_t)H * D + 2 * H] : (TD)__ldg(&w2f[H]);
-                d.Us[i] = (float)(Upart - b2);
+                d.Us[i] = (float)(Upart - w2s[H]);                        // - b2
             }
             for (int v4 = gl; v4 < Dp / 4; v4 += kGenLanes) {              // four descriptor components per lane
                 TD f0 = (TD)0, f1 = (TD)0, f2 = (TD)0, f3 = (TD)0;
+#pragma unroll 4
                 for (int mu = 0; mu < H; ++mu) {
                     const TD gm = sm.hid[mu];
-                    if (F64) {
-                        const double* w = P.params64 + (size_t)mu * D + 4 * v4;
-                        f0 += gm * (TD)w[0];
-                        if (4 * v4 + 1 < D) f1 += gm * (TD)w[1];
-                        if (4 * v4 + 2 < D) f2 += gm * (TD)w[2];
-                        if (4 * v4 + 3 < D) f3 += gm * (TD)w[3];
-                    } else {
-                        const float4 ww = __ldg(reinterpret_cast<const float4*>(P.params + (size_t)mu * Dp) + v4);
-                        f0 += gm * (TD)ww.x; f1 += gm * (TD)ww.y; f2 += gm * (TD)ww.z; f3 += gm * (TD)ww.w;
-                    }
+                    const TD* w = wsm + mu * Dps + 4 * v4;
+                    f0 += gm * w[0]; f1 += gm * w[1]; f2 += gm * w[2]; f3 += gm * w[3];
                 }
                 sm.Fp[4 * v4] = (float)f0; sm.Fp[4 * v4 + 1] = (float)f1; sm.Fp[4 * v4 + 2] = (float)f2; sm.Fp[4 * v4 + 3] = (float)f3;
             }
@@ -267,11 +269,12 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
 
         // ---- F: partial forces, Eq. 23-25 ----
         float* A = F64 ? sm.A : reinterpret_cast<float*>(&sm.S[0][0]);     // A[n][lm] = 2 Fp_nl C_lm s_nlm (0 beyond l_max)
-        for (int e = gl; e < NMAX * kNumLM; e += kGenLanes) {
-            const int n = e / kNumLM, m = e - n * kNumLM;
-            float v = 0.f;
-            if (n < NA && m < nlm) v = 2.f * C[m] * sm.Fp[NR + n * LMAX + LOF[m] - 1] * (float)sm.S[n][m];
-            A[e] = v;                                                    // in place when TD = float: same element, same lane
+        for (int n = gl; n < NMAX; n += kGenLanes) {                     // row n: in place when TD = float (same lane reads and writes it)
+            float fl[4];
+#pragma unroll
+            for (int l = 0; l < 4; ++l) fl[l] = (n < NA && l < LMAX) ? 2.f * sm.Fp[NR + n * LMAX + l] : 0.f;
+#pragma unroll
+            for (int m = 0; m < kNumLM; ++m) A[n * kNumLM + m] = C[m] * fl[LOF[m] - 1] * (float)sm.S[n][m];
         }
         __syncwarp();
         float fsx = 0.f, fsy = 0.f, fsz = 0.f;
@@ -297,23 +300,27 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
             if (c < chA && __any_sync(0xffffffffu, on && k < nA)) {      // angular family, Eq. 25 (warp-uniform branch)
                 float gs[NMAX], dg[NMAX];
                 radial_gd<NMAX>(r, P.rcA_inv, om, rinv, gs, dg);
-                float Sq[kNumLM], St[kNumLM];
+                f32x2 acc2[kNumLM];                                      // {S'_m, S_m / r} packed: one FFMA2 per (n, m)
 #pragma unroll
-                for (int m = 0; m < kNumLM; ++m) { Sq[m] = 0.f; St[m] = 0.f; }
+                for (int m = 0; m < kNumLM; ++m) acc2[m] = pack2(0.f, 0.f);
 #pragma unroll
                 for (int n = 0; n < NMAX; ++n) {
                     if (n < NA) {                                        // uniform
                         const float4* An = reinterpret_cast<const float4*>(A + n * kNumLM);
+                        const f32x2 dgs = pack2(dg[n], gs[n]);
 #pragma unroll
                         for (int m4 = 0; m4 < kNumLM / 4; ++m4) {
                             const float4 a = An[m4];
-                            Sq[4 * m4] = fmaf(a.x, dg[n], Sq[4 * m4]); St[4 * m4] = fmaf(a.x, gs[n], St[4 * m4]);
-                            Sq[4 * m4 + 1] = fmaf(a.y, dg[n], Sq[4 * m4 + 1]); St[4 * m4 + 1] = fmaf(a.y, gs[n], St[4 * m4 + 1]);
-                            Sq[4 * m4 + 2] = fmaf(a.z, dg[n], Sq[4 * m4 + 2]); St[4 * m4 + 2] = fmaf(a.z, gs[n], St[4 * m4 + 2]);
-                            Sq[4 * m4 + 3] = fmaf(a.w, dg[n], Sq[4 * m4 + 3]); St[4 * m4 + 3] = fmaf(a.w, gs[n], St[4 * m4 + 3]);
+                            acc2[4 * m4] = ffma2(pack2(a.x, a.x), dgs, acc2[4 * m4]);
+                            acc2[4 * m4 + 1] = ffma2(pack2(a.y, a.y), dgs, acc2[4 * m4 + 1]);
+                            acc2[4 * m4 + 2] = ffma2(pack2(a.z, a.z), dgs, acc2[4 * m4 + 2]);
+                            acc2[4 * m4 + 3] = ffma2(pack2(a.w, a.w), dgs, acc2[4 * m4 + 3]);
                         }
                     }
                 }
+                float Sq[kNumLM], St[kNumLM];
+#pragma unroll
+                for (int m = 0; m < kNumLM; ++m) unpack2(acc2[m], Sq[m], St[m]);
 #pragma unroll
                 for (int m = 0; m < kNumLM; ++m) Sq[m] = fmaf(-(float)LOF[m], St[m], Sq[m]);      // S'_m - l_m S_m / r
                 float ax, ay, az;

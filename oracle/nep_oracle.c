@@ -373,21 +373,41 @@ int orc_evaluate(int64_t n, const double *pos, const double *vel, const int *typ
 }
 
 /*
- * Velocity-Verlet NVE (BASELINE.json north_star; the paper times NVT).
- * a = F / (m * 103.642697) A/fs^2 with F in eV/A, m in amu.  Lists from scratch every
- * step.  thermo[n_steps+1][5] = U_tot, K_tot, Jx, Jy, Jz at steps 0..n_steps (J with W
- * and v at the same time level, reading Q12).  pos/vel are updated in place; U,F,W,J
- * hold the state after the last step.  Jsum (nullable, [3][N]) accumulates J_i over
- * steps 1..n_steps.
+ * Velocity-Verlet step of the HNEMD method's equations of motion:
+ *   Eq. 9   F_i^ext = F_e . W_i, read as (F_i^ext)^b = sum_a F_e^a W_i^{ab}, added to F_i in both half-kicks
+ *           (the only reading for which the power of the driving force is F_e . J with J = sum_i W_i . v_i of
+ *           Eq. 7 -- pinned by tests/test_oracle_hnemd.py through the energy balance);
+ *   Eq. 11  K(t) = sum_i W_i(0) . v_i(t), the virial-velocity correlation with a single time origin:
+ *           K^a(t) = sum_i sum_b W0_i^{ab} v_i^b(t), W0 = the per-atom virial at step 0 (or the array given).
+ * With Fe == NULL (or zero) this is plain NVE (BASELINE.json north_star; the paper times NVT).
+ * a = F / (m * 103.642697) A/fs^2 with F in eV/A, m in amu.  Lists from scratch every step.
+ * thermo[n_steps+1][5] = U_tot, K_tot, Jx, Jy, Jz at steps 0..n_steps (J with W and v at the same time level,
+ * reading Q12).  pos/vel are updated in place; U,F,W,J hold the state after the last step (F = the potential
+ * force of Eq. 4, without the driving force).  Jsum (nullable, [3][N]) accumulates J_i over steps 1..n_steps.
+ * Kt (nullable, [n_steps+1][3]) receives K(t) at steps 0..n_steps; W0 (nullable, [9][N]) is W_i(0), default:
+ * the virial of this run's step 0.  No thermostat and no total-force correction: the paper gives neither.
  */
-int orc_md(int64_t n, double *pos, double *vel, const int *type, const double *box,
-           const orc_hyper *h, const int *znum, const double *params, const double *mass_by_type,
-           double dt, int n_steps, int capR, int capA,
-           double *U, double *F, double *W, double *J, double *Jsum, double *thermo) {
+int orc_md_driven(int64_t n, double *pos, double *vel, const int *type, const double *box,
+                  const orc_hyper *h, const int *znum, const double *params, const double *mass_by_type,
+                  double dt, int n_steps, int capR, int capA, const double *Fe, const double *W0, double *Kt,
+                  double *U, double *F, double *W, double *J, double *Jsum, double *thermo) {
     const double conv = 103.642697;
     int rc = orc_evaluate(n, pos, vel, type, box, h, znum, params, capR, capA, U, F, W, J);
     if (rc) return rc;
+    double *W0own = NULL;
+    if (Kt && !W0) {
+        W0own = (double *)malloc(sizeof(double) * 9 * (size_t)n);
+        memcpy(W0own, W, sizeof(double) * 9 * (size_t)n);
+        W0 = W0own;
+    }
+    double *Ft = (double *)malloc(sizeof(double) * 3 * (size_t)n);        /* F_i + F_e . W_i */
     for (int step = 0; step <= n_steps; ++step) {
+        for (int64_t i = 0; i < n; ++i)
+            for (int b = 0; b < 3; ++b) {
+                double f = F[b * n + i];
+                if (Fe) for (int a = 0; a < 3; ++a) f += Fe[a] * W[(3 * a + b) * n + i];     /* Eq. 9 */
+                Ft[b * n + i] = f;
+            }
         if (thermo) {
             double u = 0, k = 0, jx = 0, jy = 0, jz = 0;
             for (int64_t i = 0; i < n; ++i) {
@@ -397,24 +417,46 @@ int orc_md(int64_t n, double *pos, double *vel, const int *type, const double *b
             }
             double *t = thermo + 5 * step; t[0] = u; t[1] = k; t[2] = jx; t[3] = jy; t[4] = jz;
         }
+        if (Kt) {
+            for (int a = 0; a < 3; ++a) {
+                double s = 0;
+                for (int64_t i = 0; i < n; ++i)
+                    for (int b = 0; b < 3; ++b) s += W0[(3 * a + b) * n + i] * vel[b * n + i];   /* Eq. 11 */
+                Kt[3 * step + a] = s;
+            }
+        }
         if (step == n_steps) break;
         for (int64_t i = 0; i < n; ++i) {
             double im = 1.0 / (mass_by_type[type[i]] * conv);
             for (int a = 0; a < 3; ++a) {
-                vel[a * n + i] += 0.5 * dt * F[a * n + i] * im;
+                vel[a * n + i] += 0.5 * dt * Ft[a * n + i] * im;
                 pos[a * n + i] += dt * vel[a * n + i];
             }
         }
         rc = orc_evaluate(n, pos, NULL, type, box, h, znum, params, capR, capA, U, F, W, NULL);
-        if (rc) return rc;
+        if (rc) break;
         for (int64_t i = 0; i < n; ++i) {
             double im = 1.0 / (mass_by_type[type[i]] * conv);
-            for (int a = 0; a < 3; ++a) vel[a * n + i] += 0.5 * dt * F[a * n + i] * im;
+            for (int b = 0; b < 3; ++b) {
+                double f = F[b * n + i];
+                if (Fe) for (int a = 0; a < 3; ++a) f += Fe[a] * W[(3 * a + b) * n + i];     /* Eq. 9 */
+                vel[b * n + i] += 0.5 * dt * f * im;
+            }
             for (int x = 0; x < 3; ++x) {
                 J[x * n + i] = W[(3 * x + 0) * n + i] * vel[i] + W[(3 * x + 1) * n + i] * vel[n + i] + W[(3 * x + 2) * n + i] * vel[2 * n + i];
                 if (Jsum) Jsum[x * n + i] += J[x * n + i];
             }
         }
     }
-    return 0;
+    free(Ft); free(W0own);
+    return rc;
+}
+
+/* Plain NVE: orc_md_driven without driving force (kept as the entry point the round-1 pins use). */
+int orc_md(int64_t n, double *pos, double *vel, const int *type, const double *box,
+           const orc_hyper *h, const int *znum, const double *params, const double *mass_by_type,
+           double dt, int n_steps, int capR, int capA,
+           double *U, double *F, double *W, double *J, double *Jsum, double *thermo) {
+    return orc_md_driven(n, pos, vel, type, box, h, znum, params, mass_by_type, dt, n_steps, capR, capA,
+                         NULL, NULL, NULL, U, F, W, J, Jsum, thermo);
 }

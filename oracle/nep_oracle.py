@@ -11,7 +11,7 @@ import numpy as np
 from . import build as _build
 
 __all__ = ["Hyper", "num_threads", "descriptor_dim", "num_params", "chebyshev", "cutoff", "radial",
-           "legendre", "neighbors", "network", "descriptor_atom", "compute", "evaluate", "md"]
+           "legendre", "neighbors", "network", "descriptor_atom", "compute", "evaluate", "md", "md_driven"]
 
 _lib = C.CDLL(_build.build())
 _dp = C.POINTER(C.c_double)
@@ -35,7 +35,7 @@ def _i(a):
 _lib.orc_num_threads.restype = C.c_int
 _lib.orc_descriptor_dim.restype = C.c_int
 _lib.orc_num_params.restype = C.c_int
-for _f in ("orc_neighbors_brute", "orc_neighbors_cell", "orc_compute", "orc_evaluate", "orc_md"):
+for _f in ("orc_neighbors_brute", "orc_neighbors_cell", "orc_compute", "orc_evaluate", "orc_md", "orc_md_driven"):
     getattr(_lib, _f).restype = C.c_int
 
 
@@ -157,4 +157,25 @@ def md(h: Hyper, znum, params, pos, vel, types, box, masses, dt, n_steps, capR=9
                      _d(out["U"]), _d(out["F"]), _d(out["W"]), _d(out["J"]), _d(out["Jsum"]), _d(out["thermo"]))
     if rc:
         raise RuntimeError("orc_md failed: %d" % rc)
+    return out
+
+
+def md_driven(h: Hyper, znum, params, pos, vel, types, box, masses, dt, n_steps, Fe=None, W0=None, capR=96, capA=64):
+    """Velocity Verlet with the HNEMD driving force F_i += F_e . W_i (Eq. 9) and K(t) = sum_i W_i(0) . v_i(t)
+    (Eq. 11); Fe=None is NVE.  Returns md()'s dict plus Kt[n_steps+1,3]."""
+    pos = np.array(pos, dtype=np.float64, order="C"); vel = np.array(vel, dtype=np.float64, order="C")
+    box = np.ascontiguousarray(box, dtype=np.float64)
+    znum = np.ascontiguousarray(znum, dtype=np.int32); types = np.ascontiguousarray(types, dtype=np.int32)
+    params = np.ascontiguousarray(params, dtype=np.float64); masses = np.ascontiguousarray(masses, dtype=np.float64)
+    fe = None if Fe is None else np.ascontiguousarray(Fe, dtype=np.float64)
+    w0 = None if W0 is None else np.ascontiguousarray(W0, dtype=np.float64)
+    n = pos.shape[1]
+    out = dict(pos=pos, vel=vel, U=np.zeros(n), F=np.zeros((3, n)), W=np.zeros((9, n)), J=np.zeros((3, n)),
+               Jsum=np.zeros((3, n)), thermo=np.zeros((n_steps + 1, 5)), Kt=np.zeros((n_steps + 1, 3)))
+    rc = _lib.orc_md_driven(C.c_int64(n), _d(pos), _d(vel), _i(types), _d(box), C.byref(h), _i(znum), _d(params),
+                            _d(masses), C.c_double(dt), C.c_int(n_steps), C.c_int(capR), C.c_int(capA),
+                            _d(fe), _d(w0), _d(out["Kt"]),
+                            _d(out["U"]), _d(out["F"]), _d(out["W"]), _d(out["J"]), _d(out["Jsum"]), _d(out["thermo"]))
+    if rc:
+        raise RuntimeError("orc_md_driven failed: %d" % rc)
     return out

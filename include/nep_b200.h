@@ -149,6 +149,21 @@ int  nep_md_step(nep_system*, double* pos_dev, double* vel_dev, const double* ma
                  int n_steps, float* energy_dev, float* force_dev, float* virial_dev, float* heat_dev,
                  double* heat_sum_dev, double* thermo_dev, void* cuda_stream);
 
+/* nep_md_step with the equations of motion of the homogeneous nonequilibrium MD method:
+ *   driving_force [3] host, 1/Angstrom, nullable (NULL: identical to nep_md_step).  Eq. 9: the external force
+ *     F_i^ext = F_e . W_i, read as (F_i^ext)^b = sum_a F_e^a W_i^{ab} -- the reading for which the power of the
+ *     driving force is F_e . J with J = sum_i W_i . v_i (Eq. 7-8) -- is added to F_i in both half-kicks.
+ *     force_dev still receives the potential force of Eq. 4.  No thermostat and no total-force correction are
+ *     applied (the paper specifies neither); thermo_dev's J columns give <J(t)> of Eq. 8.
+ *   w0_dev [9][N] fp32 device, nullable; kt_dev [n_steps][3] fp64 device, nullable (needs w0_dev).  Eq. 11: the
+ *     virial-velocity correlation K(t) = sum_i W_i(0) . v_i(t) after each step, W_i(0) being the per-atom virial
+ *     the caller kept from an earlier nep_compute / nep_md_step (same layout as virial_dev).
+ * Everything else as nep_md_step. */
+int  nep_md_step_driven(nep_system*, double* pos_dev, double* vel_dev, const double* mass_by_type, double dt_fs,
+                        int n_steps, const double* driving_force, float* energy_dev, float* force_dev,
+                        float* virial_dev, float* heat_dev, double* heat_sum_dev, double* thermo_dev,
+                        const float* w0_dev, double* kt_dev, void* cuda_stream);
+
 /* Synchronises the stream last used by this system and returns the sticky device status
  * (NEP_OK, NEP_EOVERFLOW, NEP_ESTALE) or NEP_ECUDA.  Clears the sticky word. */
 int  nep_status(nep_system*);

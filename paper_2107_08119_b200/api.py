@@ -16,7 +16,7 @@ _lib = None
 
 SYMBOLS = ["nep_create", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",
            "nep_system_create", "nep_system_destroy", "nep_system_set_path", "nep_system_path", "nep_neighbors", "nep_get_neighbors", "nep_compute", "nep_compute_internals",
-           "nep_md_step", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile", "nep_measure_fp32_peak", "nep_measure_fp32_patterns",
+           "nep_md_step", "nep_md_step_driven", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile", "nep_measure_fp32_peak", "nep_measure_fp32_patterns",
            "nep_strerror"]
 
 
@@ -50,6 +50,7 @@ def lib():
         L.nep_compute.argtypes = [C.c_void_p] * 8
         L.nep_compute_internals.argtypes = [C.c_void_p] * 6
         L.nep_md_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int] + [C.c_void_p] * 7
+        L.nep_md_step_driven.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_int] + [C.c_void_p] * 10
         for f in ("nep_destroy", "nep_system_destroy"):
             getattr(L, f).argtypes = [C.c_void_p]
             getattr(L, f).restype = None
@@ -173,6 +174,18 @@ class System:
         _check(lib().nep_md_step(self._h, _ptr(pos), _ptr(vel), m.ctypes.data_as(C.c_void_p), float(dt), int(n_steps),
                                  _ptr(U), _ptr(F), _ptr(W), _ptr(J), _ptr(heat_sum), _ptr(thermo), _stream()),
                "nep_md_step")
+        return U, F, W, J
+
+    def md_step_driven(self, pos, vel, masses, dt, n_steps, driving_force, out=None, heat_sum=None, thermo=None, w0=None, kt=None):
+        """nep_md_step_driven: HNEMD driving force F_e (Eq. 9) and K(t) = sum_i W_i(0) . v_i(t) (Eq. 11)."""
+        assert pos.dtype == torch.float64 and vel.dtype == torch.float64 and pos.is_contiguous() and vel.is_contiguous()
+        U, F, W, J = out if out is not None else self.alloc_outputs()
+        m = np.ascontiguousarray(masses, dtype=np.float64)
+        fe = None if driving_force is None else np.ascontiguousarray(driving_force, dtype=np.float64)
+        _check(lib().nep_md_step_driven(self._h, _ptr(pos), _ptr(vel), m.ctypes.data_as(C.c_void_p), float(dt), int(n_steps),
+                                        None if fe is None else fe.ctypes.data_as(C.c_void_p),
+                                        _ptr(U), _ptr(F), _ptr(W), _ptr(J), _ptr(heat_sum), _ptr(thermo), _ptr(w0), _ptr(kt),
+                                        _stream()), "nep_md_step_driven")
         return U, F, W, J
 
     def status(self):

@@ -113,6 +113,7 @@ struct nep_system {
     SysDev d;
     Box box;
     bool built, have_forces;
+    bool last_driven; float last_fe[3];    // equations of motion of the last nep_md_step (its kick force is reused)
     int path;                              // NEP_PATH_THREAD or NEP_PATH_GROUP: which kernel evaluates Eq. 12-25
     float* dump_q; float* dump_fp;        // set only inside nep_compute_internals
     cudaStream_t last_stream;
@@ -543,6 +544,10 @@ struct AsmParams {
     const double* vel_in;         // nep_compute: caller-order velocities (nullable)
     float* energy; float* force; float* virial; float* heat;   // caller-order outputs (virial/heat nullable)
     double* heat_sum; double* thermo;
+    int driven;                   // HNEMD: F_i += F_e . W_i (Eq. 9) in both half-kicks
+    float fe[3];                  // F_e, 1/A
+    const float* w0;              // [9][N] caller order, nullable: W_i(0) of Eq. 11
+    double* kt;                   // [n_steps][3], nullable: K(t) = sum_i W_i(0) . v_i(t)
 };
 
 __device__ __forceinline__ int rank_below(const uint4& m, int t) {      // number of set bits at positions < t
@@ -567,7 +572,7 @@ __device__ __forceinline__ bool bit_set(const uint4& m, int t) {
 __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
     const int N = P.N;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    double tU = 0.0, tK = 0.0, tJ[3] = {0.0, 0.0, 0.0};
+    double tU = 0.0, tK = 0.0, tJ[3] = {0.0, 0.0, 0.0}, tKt[3] = {0.0, 0.0, 0.0};
     if (i < N) {
         const int nR = d.nnR[i], nA = d.nnA[i];
         float fx = 0.f, fy = 0.f, fz = 0.f;
@@ -608,9 +613,14 @@ __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
         fx = fs.x - fx; fy = fs.y - fy; fz = fs.z - fz;               // Eq. 4-5
         const int row = d.perm[i];
         const float u = d.Us[i];
-        d.Fs[i] = fx; d.Fs[N + i] = fy; d.Fs[2 * N + i] = fz;
         P.energy[row] = u;
-        P.force[row] = fx; P.force[N + row] = fy; P.force[2 * N + row] = fz;
+        P.force[row] = fx; P.force[N + row] = fy; P.force[2 * N + row] = fz;      // the potential force of Eq. 4
+        if (P.driven) {                                                // Eq. 9: (F^ext)^b = sum_a F_e^a W^{ab}
+            fx = fmaf(P.fe[0], w[0], fmaf(P.fe[1], w[3], fmaf(P.fe[2], w[6], fx)));
+            fy = fmaf(P.fe[0], w[1], fmaf(P.fe[1], w[4], fmaf(P.fe[2], w[7], fy)));
+            fz = fmaf(P.fe[0], w[2], fmaf(P.fe[1], w[5], fmaf(P.fe[2], w[8], fz)));
+        }
+        d.Fs[i] = fx; d.Fs[N + i] = fy; d.Fs[2 * N + i] = fz;         // what the integrator kicks with
         if (P.virial) {
 #pragma unroll
             for (int c = 0; c < 9; ++c) P.virial[(size_t)c * N + row] = w[c];
@@ -639,21 +649,29 @@ __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
                 P.heat_sum[row] += (double)jx; P.heat_sum[N + row] += (double)jy; P.heat_sum[2 * N + row] += (double)jz;
             }
             tJ[0] = jx; tJ[1] = jy; tJ[2] = jz;
+            if (P.md == 1 && P.kt) {                                   // Eq. 11 with the caller's W_i(0)
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+                    tKt[a] = (double)P.w0[(size_t)(3 * a) * N + row] * vx + (double)P.w0[(size_t)(3 * a + 1) * N + row] * vy +
+                             (double)P.w0[(size_t)(3 * a + 2) * N + row] * vz;
+            }
         }
     }
-    if (P.md == 1 && P.thermo) {
-        __shared__ double red[5][4];
-        double v[5] = {tU, tK, tJ[0], tJ[1], tJ[2]};
+    if (P.md == 1 && (P.thermo || P.kt)) {
+        __shared__ double red[8][4];
+        double v[8] = {tU, tK, tJ[0], tJ[1], tJ[2], tKt[0], tKt[1], tKt[2]};
 #pragma unroll
-        for (int c = 0; c < 5; ++c)
+        for (int c = 0; c < 8; ++c)
             for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
         const int wid = threadIdx.x >> 5;
         if ((threadIdx.x & 31) == 0)
-            for (int c = 0; c < 5; ++c) red[c][wid] = v[c];
+            for (int c = 0; c < 8; ++c) red[c][wid] = v[c];
         __syncthreads();
-        if (threadIdx.x < 5) {
+        if (threadIdx.x < 8) {
             const double t = red[threadIdx.x][0] + red[threadIdx.x][1] + red[threadIdx.x][2] + red[threadIdx.x][3];
-            atomicAdd(&P.thermo[(size_t)(d.flags[F_STEP] - 1) * 5 + threadIdx.x], t);
+            const size_t step = (size_t)(d.flags[F_STEP] - 1);
+            if (threadIdx.x < 5) { if (P.thermo) atomicAdd(&P.thermo[step * 5 + threadIdx.x], t); }
+            else if (P.kt) atomicAdd(&P.kt[step * 3 + (threadIdx.x - 5)], t);
         }
     }
 }
@@ -1083,6 +1101,7 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
     // instantiated for) eight lanes share an atom
     s->path = (m->thread_path_ok && n_atoms >= kThreadPathMinAtoms) ? NEP_PATH_THREAD : NEP_PATH_GROUP;
     carve(n_atoms, s->capR, s->capMD, s->max_cells, m->NA, m->h.n_types > 1 ? m->D : 0, &s->d, (char*)workspace_dev);
+    s->last_driven = false; s->last_fe[0] = s->last_fe[1] = s->last_fe[2] = 0.f;
     s->built = false; s->have_forces = false; s->dump_q = nullptr; s->dump_fp = nullptr; s->last_stream = nullptr; s->step_graph = nullptr; s->cap_stream = nullptr; s->g_launches = 0;
     s->launches = 0; s->prof_on = false; s->prof_n = 0;
     for (int k = 0; k < NEP_PHASES; ++k) { s->prof_ms[k] = 0.0; s->prof_cnt[k] = 0; }
@@ -1209,8 +1228,16 @@ int nep_compute_internals(nep_system* s, const double* pos_dev, float* q_dev, fl
 int nep_md_step(nep_system* s, double* pos_dev, double* vel_dev, const double* mass_by_type, double dt_fs, int n_steps,
                 float* energy_dev, float* force_dev, float* virial_dev, float* heat_dev, double* heat_sum_dev,
                 double* thermo_dev, void* cuda_stream) {
+    return nep_md_step_driven(s, pos_dev, vel_dev, mass_by_type, dt_fs, n_steps, nullptr, energy_dev, force_dev, virial_dev,
+                              heat_dev, heat_sum_dev, thermo_dev, nullptr, nullptr, cuda_stream);
+}
+
+int nep_md_step_driven(nep_system* s, double* pos_dev, double* vel_dev, const double* mass_by_type, double dt_fs, int n_steps,
+                       const double* driving_force, float* energy_dev, float* force_dev, float* virial_dev, float* heat_dev,
+                       double* heat_sum_dev, double* thermo_dev, const float* w0_dev, double* kt_dev, void* cuda_stream) {
     if (!s || !pos_dev || !vel_dev || !mass_by_type || !energy_dev || !force_dev || n_steps < 0 || !(dt_fs > 0.0))
         return NEP_EINVAL;
+    if (kt_dev && !w0_dev) return NEP_EINVAL;
     if (!s->built) return NEP_ESTATE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     s->last_stream = st;
@@ -1224,7 +1251,16 @@ int nep_md_step(nep_system* s, double* pos_dev, double* vel_dev, const double* m
     fill_masses(&P, s->model, mass_by_type);
     P.energy = energy_dev; P.force = force_dev; P.virial = virial_dev; P.heat = heat_dev;
     P.heat_sum = heat_sum_dev; P.thermo = thermo_dev;
+    if (driving_force) {
+        P.driven = 1;
+        for (int a = 0; a < 3; ++a) P.fe[a] = (float)driving_force[a];
+        if (!s->have_forces || !s->last_driven || memcmp(s->last_fe, P.fe, sizeof(P.fe)) != 0) s->have_forces = false;
+    } else if (s->last_driven) s->have_forces = false;        // the stored kick force must match this call's equations of motion
+    s->last_driven = driving_force != nullptr;
+    memcpy(s->last_fe, P.fe, sizeof(P.fe));
+    P.w0 = kt_dev ? w0_dev : nullptr; P.kt = kt_dev;
     if (thermo_dev && n_steps > 0) NEP_CUDA_OK(cudaMemsetAsync(thermo_dev, 0, (size_t)n_steps * 5 * sizeof(double), st));
+    if (kt_dev && n_steps > 0) NEP_CUDA_OK(cudaMemsetAsync(kt_dev, 0, (size_t)n_steps * 3 * sizeof(double), st));
     // caller arrays -> sorted state
     phase(s, PH_STATE, st);
     k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, vel_dev, hs2, 1);

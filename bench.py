@@ -42,10 +42,37 @@ def algorithmic_flops_per_atom(n_r, n_a, dim, n_neu, m_r, m_a):
 
 
 def make_workload(name):
+    """c0..c3, c4_<atoms> (BASELINE.json configs) and t1_si / t1_silicene / t1_pbte: the paper's Table I model
+    shapes on the 8000 / 6000-atom cells of its own speed test (random weights)."""
     from paper_2107_08119_b200 import inputs
     if name.startswith("c4_"):
         return inputs.config4(int(name[3:]))
+    if name.startswith("t1_"):
+        return inputs.table1(name[3:])
     return {"c0": inputs.config0, "c1": inputs.config1, "c2": inputs.config2, "c3": inputs.config3}[name]()
+
+
+def caps_for(name, w):
+    """(cap_radial, cap_angular) with head-room for the heated state."""
+    if name.startswith("t1_"):
+        return {"t1_si": (56, 56), "t1_silicene": (32, 32), "t1_pbte": (86, 24)}[name]
+    return (64, 32) if len(w.atomic_numbers) == 1 else (80, 40)
+
+
+def oracle_sample(w, budget_s, max_reps):
+    """Times the oracle as it stands on the workload itself: full fp64 evaluations of U, F, W, J including the
+    list build, repeated until `budget_s` seconds of CPU work (at least one)."""
+    import oracle
+    h = oracle.Hyper(w.rc_r, w.rc_a, w.n_max_r, w.n_max_a, w.l_max, w.n_neurons, len(w.atomic_numbers))
+    t0 = time.perf_counter()
+    reps = 0
+    while reps < 1 or (time.perf_counter() - t0 < budget_s and reps < max_reps):
+        oracle.evaluate(h, w.atomic_numbers, w.params, w.pos, w.vel, w.types, w.box, 96, 64)
+        reps += 1
+    dt = time.perf_counter() - t0
+    sample = ("%s itself (%d atoms): %d full fp64 evaluations of U,F,W,J incl. list build (literal O(M^2) Eq. 13/25), %.1f s"
+              % (w.name, w.n_atoms, reps, dt))
+    return w.n_atoms * reps / dt, oracle.num_threads(), sample, reps, dt
 
 
 class ClockSampler(threading.Thread):
@@ -89,26 +116,16 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import oracle
-    from paper_2107_08119_b200 import inputs
-    w = inputs.si_cells((24, 24, 24))           # 110592 atoms of the C4 lattice, C4 seeds, C0 weights
-    h = oracle.Hyper(w.rc_r, w.rc_a, w.n_max_r, w.n_max_a, w.l_max, w.n_neurons, 1)
-    ev = lambda: oracle.evaluate(h, w.atomic_numbers, w.params, w.pos, w.vel, w.types, w.box)
-    for _ in range(min(args.warmup, 1)):
-        ev()
+    w = make_workload(args.workload)
     steps = max(1, min(args.steps, 20))
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        ev()
-    dt = time.perf_counter() - t0
-    value = w.n_atoms * steps / dt
-    sample = "%d-atom replica of the C4 Si lattice (24^3 cells), %d full evaluations of U,F,W,J" % (w.n_atoms, steps)
+    value, cores, sample, reps, dt = oracle_sample(w, min(60.0, 8.0 * steps), steps)     # each "step" = one evaluation, bounded
+    steps = reps
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-        "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": 0, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": args.workload, "sample": sample},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
@@ -148,7 +165,7 @@ def main():
     K, Wm = args.steps, max(args.warmup, 3)
     w = make_workload(args.workload)
     N = w.n_atoms
-    cap_r, cap_a = (64, 32) if len(w.atomic_numbers) == 1 else (80, 40)
+    cap_r, cap_a = caps_for(args.workload, w)
     model, system, pos, vel = api.from_workload(w, cap_r, cap_a, args.skin, dev)
     out = system.alloc_outputs()
     heat_sum = torch.zeros((3, N), dtype=torch.float64, device=dev)
@@ -232,7 +249,7 @@ def main():
         hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
         hbm_src = "MEASURED_PEAKS.json hbm_gbs"
     except Exception:
-        hbm_peak, hbm_src = 6500.0, "fallback of /opt/skills/guides/B200_PROFILING.md"
+        hbm_peak, hbm_src = 6650.0, "fallback of /opt/skills/guides/B200_PROFILING.md"
     mr, ma = 0.5 * (m_r0 + m_r), 0.5 * (m_a0 + m_a)
     m_md = mr * ((w.rc_r + args.skin) / w.rc_r) ** 3
     bytes_filter = 4 * m_md + 32 + 20 * mr + 32 + 8           # Verlet row, own position, records + jrev, masks, counts
@@ -242,28 +259,24 @@ def main():
         gbs = nbytes * N / (prof[name]["ms"] / max(1, prof[name]["count"]) * 1e-3) / 1e9
         hbm_phases[name] = {"bound": "hbm", "bytes_per_atom": nbytes, "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
                             "frac": gbs / hbm_peak}
-    traffic = None          # dram bytes per k_main launch from the committed ncu capture (1M-atom workload only)
+    # Counters of the dominant kernel from the committed ncu --set full capture of this same command
+    # (profiles/r2_k_main_counters.json; 1M-atom workload, one thread per atom): DRAM bytes per launch and the
+    # EXECUTED FP32 flops per launch (FFMA = 2, FFMA2 = 4, FMUL/FADD = 1, summed over the SASS of one launch).
+    traffic = executed = None
+    counters_src = None
     try:
-        if args.workload == "c4_1048576":
-            traffic = json.load(open(os.path.join(ROOT, "profiles", "r1_traffic.json")))["k_main_dram_bytes_per_launch"]
+        if args.workload == "c4_1048576" and system.path == 1:
+            cj = json.load(open(os.path.join(ROOT, "profiles", "r2_k_main_counters.json")))
+            traffic = cj["k_main_dram_bytes_per_launch"]
+            executed = cj["k_main_executed_fp32_flops_per_launch"]
+            counters_src = cj["capture"]
     except Exception:
-        traffic = None
+        traffic = executed = None
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        import oracle
-        from paper_2107_08119_b200 import inputs
-        ws = inputs.si_cells((24, 24, 24))          # 110592 atoms of the C4 lattice (C4 seeds, C0 weights)
-        h = oracle.Hyper(ws.rc_r, ws.rc_a, ws.n_max_r, ws.n_max_a, ws.l_max, ws.n_neurons, 1)
-        tt = time.perf_counter()
-        reps = 0
-        while reps < 1 or (time.perf_counter() - tt < 10.0 and reps < 40):   # ~10-20 s of CPU work
-            oracle.evaluate(h, ws.atomic_numbers, ws.params, ws.pos, ws.vel, ws.types, ws.box)
-            reps += 1
-        tt = time.perf_counter() - tt
-        cpu = {"value": ws.n_atoms * reps / tt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": "%d-atom replica of the C4 Si lattice (24^3 cells), %d full fp64 evaluations of U,F,W,J "
-                         "incl. list build (literal O(M^2) Eq. 13/25), %.1f s" % (ws.n_atoms, reps, tt)}
+        v, cores, sample, reps, tt = oracle_sample(w, 12.0, 3)      # the config itself, up to 3 evaluations / ~12-20 s
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
     if rank == 0:
         line = {
@@ -283,7 +296,8 @@ def main():
                     "d2h_bytes_per_step": d2h, "steps": ke,
                     "what": "per step: pinned-host pos+vel -> device, nep_md_step(1), pos+vel+U+F+W+J -> pinned host"},
             "gpu_launches": int(launches),
-            "roofline": {"bound": "alu", "kernel": "k_main (descriptor + network + partial forces)",
+            "roofline": {"bound": "alu", "kernel": ("k_main, one thread per atom" if system.path == 1 else "k_gen, 16 lanes per atom") +
+                                                  " (descriptor + network + partial forces)",
                          "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
                          "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (no FP32 figure in MEASURED_PEAKS.json)",
                          "peak_measured_fma_chain": {"ffma": peak_ffma, "ffma2": peak_ffma2, "unit": "TFLOP/s"},
@@ -292,7 +306,9 @@ def main():
                                               "what": "register-resident inner-loop patterns of k_main at its residency (8 warps/SM)"},
                          "frac_of_measured_ffma": achieved / peak_ffma,
                          "flops_per_atom": flops_atom, "kernel_ms": main_ms, "kernel_share_of_step": phase_ms["main"] / tot_phase,
-                         "traffic": traffic},
+                         "traffic": traffic,
+                         "executed_frac": (executed / (main_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS) if executed else None,
+                         "counters_source": counters_src},
             "phase_ms_per_step": phase_ms,
             "roofline_hbm_phases": dict(hbm_phases, peak_source=hbm_src),
             "cpu_baseline": cpu,

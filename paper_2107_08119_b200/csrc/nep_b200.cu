@@ -832,7 +832,7 @@ void launch_build(nep_system* s, const double* xin, const double* vin, int first
 constexpr int kMainSmemLimit = 112 * 1024;          // two blocks of k_main per SM
 template <int NA, bool MULTI>
 size_t main_smem_bytes(int params_floats) {
-    return ((size_t)params_floats + kMainWarps * main_warp_floats<NA, MULTI>()) * sizeof(float);
+    return ((size_t)params_floats + kMainWarps * main_warp_floats<NA, MULTI>() + kMainBarFloats) * sizeof(float);
 }
 
 template <int NR, int NA, bool MULTI>

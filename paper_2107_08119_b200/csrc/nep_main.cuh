@@ -219,10 +219,30 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
+// Bulk copy global -> shared through the TMA engine (cp.async.bulk, SASS UBLKCP), completed on an mbarrier: one
+// instruction moves the whole weight blob of a block instead of one cp.async per 16 bytes per thread.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@!p bra WAIT_%=;\n\t}"
+                 ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
 // floats of shared memory: staged weights, then one region per warp
 __host__ __device__ constexpr int main_wfloats(int H, int Dp) { return (H * Dp + 2 * H + 1 + 3) & ~3; }
 template <int NA, bool MULTI>
 __host__ __device__ constexpr int main_warp_floats() { return (kRowsS + kRowsO) * 32 * 4 + (MULTI ? kRowsS * 32 : 0); }
+constexpr int kMainBarFloats = 4;     // the weights' mbarrier lives behind the last warp's region
 
 template <int NR, int NA, bool MULTI>
 __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParams P,
@@ -250,14 +270,21 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
     const float* zrow = Z.zz + (MULTI ? d.type_s[i] * kMaxTypes : 0);
     auto omega_of = [&](const float4& e) { return MULTI ? zrow[__float_as_int(e.w) & (kMaxTypes - 1)] : 1.f; };
 
-    // ---- P0: every neighbour record of the atom in flight at once (cp.async), weights staged meanwhile ----
+    // ---- P0: every neighbour record of the atom in flight at once (cp.async); the weights arrive as ONE bulk copy ----
     {
+        unsigned long long* wbar = reinterpret_cast<unsigned long long*>(sm + wfl + kMainWarps * main_warp_floats<NA, MULTI>());
+        if (threadIdx.x == 0) mbar_init(wbar, 1);
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            mbar_expect_tx(wbar, (unsigned)wfl * 4u);
+            bulk_g2s(sm, params, (unsigned)wfl * 4u, wbar);
+        }
         const int ka = min(nA, kRowsS), ko = min(nO, kRowsO);
         for (int k = 0; k < ka; ++k) cp_async16(&srec[k * 32 + lane], &grec[(size_t)k * N]);
         for (int o = 0; o < ko; ++o) cp_async16(&praw[o * 32 + lane], &grec[(size_t)(P.capR - 1 - o) * N]);
-        for (int k = threadIdx.x; k < wfl / 4; k += 32 * kMainWarps) cp_async16(sm + 4 * k, params + 4 * k);
         cp_async_wait_all();
-        __syncthreads();
+        mbar_wait(wbar, 0);
+        __syncwarp();
     }
 
     // neighbour k (an angular one) as unit vector, distance and Eq. 19 weight

@@ -69,12 +69,9 @@ def test_reference_arm_rank0_only_under_gloo():
     code = (
         "import os, sys, torch.distributed as dist\n"
         "dist.init_process_group('gloo', rank=int(os.environ['RANK']), world_size=2)\n"
-        "sys.argv = ['bench.py', '--impl', 'reference', '--gpus', '2', '--steps', '1', '--warmup', '0']\n"
+        "sys.argv = ['bench.py', '--impl', 'reference', '--gpus', '2', '--steps', '1', '--warmup', '0', '--workload', 'c0']\n"
         "sys.path.insert(0, %r)\n"
         "import bench\n"
-        "import paper_2107_08119_b200.inputs as inp\n"
-        "orig = inp.si_cells\n"
-        "inp.si_cells = lambda cells, **kw: orig((4, 4, 4), **kw)\n"      # small sample for the CPU test
         "bench.main()\n"
         "dist.barrier(); dist.destroy_process_group()\n" % ROOT)
     procs = [subprocess.Popen([sys.executable, "-c", code], env=dict(env, RANK=str(r), WORLD_SIZE="2"),

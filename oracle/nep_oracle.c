@@ -46,6 +46,8 @@
 
 #define ORC_MAX_N 32   /* radial functions per family */
 #define ORC_MAX_L 8
+#define ORC_MAX_D 1200 /* descriptor components (variants included) */
+#define ORC_MAX_H 256  /* neurons per hidden layer */
 
 typedef struct {
     double rc_r, rc_a;          /* r_c^R, r_c^A (Table I)                    */
@@ -53,7 +55,18 @@ typedef struct {
     int lmax;                   /* l = 1..lmax                               */
     int nneu;                   /* N_neu                                     */
     int ntypes;                 /* 1 => omega_ij = 1; >1 => Eq. 19           */
+    /* variants the paper mentions but does not use (0 = the paper's own form): */
+    int nlayers;                /* hidden layers, 0 or 1 = the single layer of Eq. 21-22; 2, 3: "generalization to
+                                   more hidden layers is straightforward"                         */
+    int nneu2, nneu3;           /* widths of hidden layers 2 and 3                                              */
+    int kind;                   /* 0: q_nl of Eq. 13; 1: the SOAP-like q_nn'l of Eq. 17      */
 } orc_hyper;
+
+static int orc_layers(const orc_hyper *h, int *width) {  /* hidden-layer widths; returns their number */
+    int L = h->nlayers < 1 ? 1 : h->nlayers;
+    width[0] = h->nneu; width[1] = h->nneu2; width[2] = h->nneu3;
+    return L;
+}
 
 int orc_num_threads(void) {
 #ifdef _OPENMP
@@ -64,9 +77,16 @@ int orc_num_threads(void) {
 }
 
 int orc_descriptor_dim(const orc_hyper *h) {              /* Eq. 16 */
+    if (h->kind == 1)                                     /* q_nn'l = q_n'nl: the pairs n <= n' */
+        return (h->nmax_r + 1) + ((h->nmax_a + 1) * (h->nmax_a + 2) / 2) * h->lmax;
     return (h->nmax_r + 1) + (h->nmax_a + 1) * h->lmax;
 }
 int orc_num_params(const orc_hyper *h) {                  /* Eq. 26 */
+    if (h->nlayers > 1) {                                 /* every layer: weights + biases; output: weights + bias */
+        int w[3], L = orc_layers(h, w), in = orc_descriptor_dim(h), np = 0;
+        for (int k = 0; k < L; ++k) { np += (in + 1) * w[k]; in = w[k]; }
+        return np + in + 1;
+    }
     return (orc_descriptor_dim(h) + 2) * h->nneu + 1;
 }
 
@@ -207,7 +227,41 @@ static inline double omega_ij(const orc_hyper *h, const int *znum, const int *ty
 }
 
 /* Eq. 21-22 and dU/dq (chain rule through tanh).  params: w1[H][D] | b1[H] | w2[H] | b2. */
+/* More hidden layers: x^(k) = tanh(W^(k) x^(k-1) - b^(k)), x^(0) = q, U = w_out . x^(L) - b_out, every
+ * bias with the minus sign of Eq. 21-22.  params: W1[H1][D] | b1[H1] | W2[H2][H1] | b2[H2] | ... | w_out[H_L] | b_out.
+ * dU/dq by back-propagation: delta^(L) = w_out (1 - x^(L)^2), delta^(k-1) = (W^(k))^T delta^(k) (1 - x^(k-1)^2). */
+static void orc_network_deep(const orc_hyper *h, const double *params, const double *q, double *U, double *Fp) {
+    int w[3], L = orc_layers(h, w), D = orc_descriptor_dim(h);
+    double x[4][ORC_MAX_D > ORC_MAX_H ? ORC_MAX_D : ORC_MAX_H], delta[ORC_MAX_D > ORC_MAX_H ? ORC_MAX_D : ORC_MAX_H], prev[ORC_MAX_D > ORC_MAX_H ? ORC_MAX_D : ORC_MAX_H];
+    const double *W[3], *b[3];
+    int in = D; const double *p = params;
+    for (int v = 0; v < D; ++v) x[0][v] = q[v];
+    for (int k = 0; k < L; ++k) {
+        W[k] = p; b[k] = p + (size_t)w[k] * in; p = b[k] + w[k];
+        for (int m = 0; m < w[k]; ++m) {
+            double a = 0.0;
+            for (int v = 0; v < in; ++v) a += W[k][m * in + v] * x[k][v];
+            x[k + 1][m] = tanh(a - b[k][m]);
+        }
+        in = w[k];
+    }
+    double u = 0.0;
+    for (int m = 0; m < in; ++m) { u += p[m] * x[L][m]; delta[m] = p[m] * (1.0 - x[L][m] * x[L][m]); }
+    *U = u - p[in];
+    for (int k = L - 1; k >= 0; --k) {
+        int nin = k == 0 ? D : w[k - 1];
+        for (int v = 0; v < nin; ++v) {
+            double s = 0.0;
+            for (int m = 0; m < w[k]; ++m) s += delta[m] * W[k][m * nin + v];
+            prev[v] = k == 0 ? s : s * (1.0 - x[k][v] * x[k][v]);
+        }
+        for (int v = 0; v < nin; ++v) delta[v] = prev[v];
+    }
+    for (int v = 0; v < D; ++v) Fp[v] = delta[v];
+}
+
 void orc_network(const orc_hyper *h, const double *params, const double *q, double *U, double *Fp) {
+    if (h->nlayers > 1) { orc_network_deep(h, params, q, U, Fp); return; }
     int D = orc_descriptor_dim(h), H = h->nneu;
     const double *w1 = params, *b1 = params + (size_t)H * D, *w2 = b1 + H, *b2 = w2 + H;
     double u = 0.0;
@@ -247,6 +301,15 @@ void orc_descriptor_atom(const orc_hyper *h, const int *znum, const int *type, i
             orc_radial(rk, h->rc_a, h->nmax_a, omega_ij(h, znum, type, i, k), gk, dg);
             double c = (dj[0] * dk[0] + dj[1] * dk[1] + dj[2] * dk[2]) / (rj * rk);
             orc_legendre(c, h->lmax, P, dP);
+            if (h->kind == 1) {                /* Eq. 17 written as the double sum it came from:
+                                                  g_n(r_ij) g_n'(r_ik) (2l+1)/(4 pi) P_l, for the pairs n <= n' */
+                int v = h->nmax_r + 1;
+                for (int m = 0; m <= h->nmax_a; ++m)
+                    for (int m2 = m; m2 <= h->nmax_a; ++m2)
+                        for (int l = 1; l <= h->lmax; ++l)
+                            q[v++] += g[m] * gk[m2] * ((2 * l + 1) / (4.0 * M_PI)) * P[l];
+                continue;
+            }
             for (int m = 0; m <= h->nmax_a; ++m)
                 for (int l = 1; l <= h->lmax; ++l)
                     q[(h->nmax_r + 1) + m * h->lmax + (l - 1)] += g[m] * gk[m] * P[l];
@@ -276,7 +339,7 @@ int orc_compute(int64_t n, const double *pos, const double *vel, const int *type
 
     #pragma omp parallel for schedule(dynamic, 16)
     for (int64_t i = 0; i < n; ++i) {
-        double q[ORC_MAX_N * (ORC_MAX_L + 1) + 2], Fp[ORC_MAX_N * (ORC_MAX_L + 1) + 2], Ui;
+        double q[ORC_MAX_D], Fp[ORC_MAX_D], Ui;
         const int *LR = idxR + i * (int64_t)capR, *LA = idxA + i * (int64_t)capA;
         int nR = cntR[i], nA = cntA[i];
         orc_descriptor_atom(h, znum, type, n, pos, box, i, nR, LR, nA, LA, q);
@@ -311,6 +374,23 @@ int orc_compute(int64_t n, const double *pos, const double *vel, const int *type
                 orc_radial(rk, h->rc_a, h->nmax_a, omega_ij(h, znum, type, i, k), gk, dgk);
                 double c = (dj[0] * dk[0] + dj[1] * dk[1] + dj[2] * dk[2]) / (rj * rk);
                 orc_legendre(c, h->lmax, P, dP);
+                if (h->kind == 1) {            /* d q_nn'l / d r_ij: atom j enters the double sum once as the first
+                                                  factor (radial index n) and once as the second (n') */
+                    int v = h->nmax_r + 1;
+                    for (int m = 0; m <= h->nmax_a; ++m)
+                        for (int m2 = m; m2 <= h->nmax_a; ++m2)
+                            for (int l = 1; l <= h->lmax; ++l) {
+                                double fp = Fp[v++] * ((2 * l + 1) / (4.0 * M_PI));
+                                for (int x = 0; x < 3; ++x) {
+                                    double rhat_j = dj[x] / rj, rhat_k = dk[x] / rk;
+                                    double ang = dP[l] * (1.0 / rj) * (rhat_k - rhat_j * c);
+                                    double first = dg[m] * gk[m2] * rhat_j * P[l] + g[m] * gk[m2] * ang;
+                                    double second = gk[m] * dg[m2] * rhat_j * P[l] + gk[m] * g[m2] * ang;
+                                    acc[x] += fp * (first + second);
+                                }
+                            }
+                    continue;
+                }
                 for (int m = 0; m <= h->nmax_a; ++m)
                     for (int l = 1; l <= h->lmax; ++l) {
                         double fp = Fp[(h->nmax_r + 1) + m * h->lmax + (l - 1)];

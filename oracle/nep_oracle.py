@@ -21,7 +21,9 @@ _ip = C.POINTER(C.c_int)
 class Hyper(C.Structure):
     """Table I hyper-parameters; n_max inclusive (Eq. 16)."""
     _fields_ = [("rc_r", C.c_double), ("rc_a", C.c_double), ("nmax_r", C.c_int), ("nmax_a", C.c_int),
-                ("lmax", C.c_int), ("nneu", C.c_int), ("ntypes", C.c_int)]
+                ("lmax", C.c_int), ("nneu", C.c_int), ("ntypes", C.c_int),
+                # variants (default 0 = the paper's own form): hidden layers 2-3 and the SOAP-like q_nn'l of Eq. 17
+                ("nlayers", C.c_int), ("nneu2", C.c_int), ("nneu3", C.c_int), ("kind", C.c_int)]
 
 
 def _d(a):

@@ -70,6 +70,27 @@ typedef struct {
  *          (n=1: l=1..l_max) | ...].  n_params must equal (D+2)H+1 (Eq. 26) else NEP_EINVAL. */
 int  nep_create(const nep_hyper* hyper, const int* atomic_number, const double* params, size_t n_params,
                 nep_model** out);
+/* Variants the paper mentions without using them; evaluated by the eight/sixteen-lanes-per-atom
+ * kernel (NEP_PATH_GROUP) only:
+ *   n_hidden_layers 1..3 ("generalization to more hidden layers is straightforward"):
+ *     x^(k) = tanh(W^(k) x^(k-1) - b^(k)), x^(0) = q, U = w_out . x^(L) - b_out, every bias with the minus sign of
+ *     Eq. 21-22; params order  W1[H1][D] | b1[H1] | W2[H2][H1] | b2[H2] | ... | w_out[H_L] | b_out; widths
+ *     base.n_neurons, n_neurons_2, n_neurons_3 (each 1..128); n_params = sum_k (in_k + 1) H_k + H_L + 1.
+ *   angular_kind NEP_ANGULAR_QNNL: the SOAP-like q_nn'l of Eq. 17-18,
+ *     q_nn'l = (2l+1)/(4 pi) sum_jk g_n(r_ij) g_n'(r_ik) P_l(cos theta_ijk) = sum_m c_nlm c*_n'lm, for the pairs n <= n'
+ *     (q_nn'l = q_n'nl), ordered n, then n' >= n, then l; N_des = (n_max_R+1) + (n_max_A+1)(n_max_A+2)/2 l_max;
+ *     needs n_max_radial, n_max_angular <= 7.
+ * nep_create(h, ...) is nep_create_ex with one hidden layer and NEP_ANGULAR_QNL. */
+enum { NEP_ANGULAR_QNL = 0, NEP_ANGULAR_QNNL = 1 };
+typedef struct {
+    nep_hyper base;
+    int n_hidden_layers;    /* 1..3 */
+    int n_neurons_2;        /* width of hidden layer 2 (n_hidden_layers >= 2) */
+    int n_neurons_3;        /* width of hidden layer 3 (n_hidden_layers == 3) */
+    int angular_kind;       /* NEP_ANGULAR_QNL or NEP_ANGULAR_QNNL */
+} nep_hyper_ex;
+int  nep_create_ex(const nep_hyper_ex* hyper, const int* atomic_number, const double* params, size_t n_params,
+                   nep_model** out);
 int  nep_descriptor_dim(const nep_model*);          /* Eq. 16 */
 int  nep_num_params(const nep_model*);              /* Eq. 26 */
 void nep_destroy(nep_model*);

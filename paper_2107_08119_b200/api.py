@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libnep_b200.so")
 _lib = None
 
-SYMBOLS = ["nep_create", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",
+SYMBOLS = ["nep_create", "nep_create_ex", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",
            "nep_system_create", "nep_system_destroy", "nep_system_set_path", "nep_system_path", "nep_neighbors", "nep_get_neighbors", "nep_compute", "nep_compute_internals",
            "nep_md_step", "nep_md_step_driven", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile", "nep_measure_fp32_peak", "nep_measure_fp32_patterns",
            "nep_strerror"]
@@ -31,6 +31,11 @@ class Hyper(C.Structure):
                 ("n_max_angular", C.c_int), ("l_max", C.c_int), ("n_neurons", C.c_int), ("n_types", C.c_int)]
 
 
+class HyperEx(C.Structure):
+    _fields_ = [("base", Hyper), ("n_hidden_layers", C.c_int), ("n_neurons_2", C.c_int), ("n_neurons_3", C.c_int),
+                ("angular_kind", C.c_int)]
+
+
 def lib():
     """Loads the C-ABI library (built by paper_2107_08119_b200/build.py).  Fails loudly if absent."""
     global _lib
@@ -43,6 +48,7 @@ def lib():
         L.nep_workspace_bytes.restype = C.c_size_t
         L.nep_workspace_bytes.argtypes = [C.c_void_p, C.c_int64, C.c_int, C.c_int, C.c_double]
         L.nep_create.argtypes = [C.POINTER(Hyper), C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_void_p)]
+        L.nep_create_ex.argtypes = [C.POINTER(HyperEx), C.c_void_p, C.c_void_p, C.c_size_t, C.POINTER(C.c_void_p)]
         L.nep_system_create.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_void_p,
                                         C.c_size_t, C.POINTER(C.c_void_p)]
         L.nep_neighbors.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -83,13 +89,22 @@ def _check(code, where):
 class Model:
     """nep_create / nep_destroy."""
 
-    def __init__(self, rc_radial, rc_angular, n_max_radial, n_max_angular, l_max, n_neurons, atomic_numbers, params):
+    def __init__(self, rc_radial, rc_angular, n_max_radial, n_max_angular, l_max, n_neurons, atomic_numbers, params,
+                 hidden_layers=None, angular_kind=0):
+        """hidden_layers: None (one layer of n_neurons) or a list of 1..3 widths; angular_kind 1: q_nn'l (nep_create_ex)."""
         zs = np.ascontiguousarray(atomic_numbers, dtype=np.int32)
         par = np.ascontiguousarray(params, dtype=np.float64)
         self.hyper = Hyper(rc_radial, rc_angular, n_max_radial, n_max_angular, l_max, n_neurons, len(zs))
         self._h = C.c_void_p()
-        _check(lib().nep_create(C.byref(self.hyper), zs.ctypes.data_as(C.c_void_p), par.ctypes.data_as(C.c_void_p),
-                                par.size, C.byref(self._h)), "nep_create")
+        if hidden_layers is None and angular_kind == 0:
+            _check(lib().nep_create(C.byref(self.hyper), zs.ctypes.data_as(C.c_void_p), par.ctypes.data_as(C.c_void_p),
+                                    par.size, C.byref(self._h)), "nep_create")
+        else:
+            w = list(hidden_layers) if hidden_layers is not None else [n_neurons]
+            self.hyper.n_neurons = w[0]
+            hx = HyperEx(self.hyper, len(w), w[1] if len(w) > 1 else 0, w[2] if len(w) > 2 else 0, angular_kind)
+            _check(lib().nep_create_ex(C.byref(hx), zs.ctypes.data_as(C.c_void_p), par.ctypes.data_as(C.c_void_p),
+                                       par.size, C.byref(self._h)), "nep_create_ex")
 
     @property
     def descriptor_dim(self):

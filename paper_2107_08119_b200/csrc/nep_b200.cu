@@ -103,6 +103,9 @@ struct nep_model {
     double* params64_dev;       // multi-species models: the Eq. 26 vector in double, caller order (k_desc64, k_gen<double>)
     Desc64Params p64;
     bool thread_path_ok;        // k_main / k_desc64 are instantiated for this shape
+    // variants (nep_create_ex): SOAP-like descriptor, two or three hidden layers
+    int kind, nlayers, lw[3], lin_p[3], off_w[3], off_b[3], off_out, blob_elems;
+    float* blob_dev; double* blob64_dev;
 };
 
 struct nep_system {
@@ -882,8 +885,12 @@ void launch_gen_t(nep_system* s, cudaStream_t st) {
     P.N = (int)s->N; P.capR = s->capR; P.box = s->box;
     P.params = m->params_dev; P.params64 = m->params64_dev;
     P.q_out = s->dump_q; P.fp_out = s->dump_fp;
-    const size_t smem = (size_t)kGenAtomsPerBlock * sizeof(GenSmem<NMAX, TD>) +
-                        ((size_t)m->H * (sizeof(TD) == 8 ? (P.Dp | 1) : P.Dp + 4) + 2 * m->H + 1) * sizeof(TD);   // + the staged weights
+    P.kind = m->kind; P.nlayers = m->nlayers; P.off_out = m->off_out; P.blob_elems = m->blob_elems;
+    for (int k = 0; k < 3; ++k) { P.lw[k] = m->lw[k]; P.lin_p[k] = m->lin_p[k]; P.off_w[k] = m->off_w[k]; P.off_b[k] = m->off_b[k]; }
+    P.blob = m->blob_dev; P.blob64 = m->blob64_dev;
+    const size_t wbytes = m->nlayers > 1 ? (size_t)m->blob_elems * sizeof(TD)
+                                         : ((size_t)m->H * (sizeof(TD) == 8 ? (P.Dp | 1) : P.Dp + 4) + 2 * m->H + 1) * sizeof(TD);
+    const size_t smem = (size_t)kGenAtomsPerBlock * sizeof(GenSmem<NMAX, TD>) + ((wbytes + 15) & ~(size_t)15);     // + the staged weights
     static size_t attr_smem[64] = {};              // per device: the largest dynamic size this instantiation was opted in for
     int dev = 0;
     cudaGetDevice(&dev);
@@ -1025,7 +1032,16 @@ const char* nep_strerror(int code) {
 }
 
 int nep_create(const nep_hyper* hy, const int* atomic_number, const double* params, size_t n_params, nep_model** out) {
-    if (!hy || !params || !out) return NEP_EINVAL;
+    if (!hy) return NEP_EINVAL;
+    nep_hyper_ex hx;
+    memset(&hx, 0, sizeof(hx));
+    hx.base = *hy; hx.n_hidden_layers = 1; hx.angular_kind = NEP_ANGULAR_QNL;
+    return nep_create_ex(&hx, atomic_number, params, n_params, out);
+}
+
+int nep_create_ex(const nep_hyper_ex* hx, const int* atomic_number, const double* params, size_t n_params, nep_model** out) {
+    if (!hx || !params || !out) return NEP_EINVAL;
+    const nep_hyper* hy = &hx->base;
     *out = nullptr;
     if (!(hy->rc_radial > 0.0) || !(hy->rc_angular > 0.0) || hy->rc_angular > hy->rc_radial) return NEP_EINVAL;
     if (hy->n_max_radial < 0 || hy->n_max_radial > 15 || hy->n_max_angular < 0 || hy->n_max_angular > 15) return NEP_EINVAL;
@@ -1033,35 +1049,84 @@ int nep_create(const nep_hyper* hy, const int* atomic_number, const double* para
     if (hy->n_neurons < 1 || hy->n_neurons > kMaxHGen) return NEP_EINVAL;
     if (hy->n_types < 1 || hy->n_types > kMaxTypes) return NEP_EINVAL;
     if (hy->n_types > 1 && !atomic_number) return NEP_EINVAL;
+    const int L = hx->n_hidden_layers;
+    if (L < 1 || L > 3) return NEP_EINVAL;
+    if (L >= 2 && (hx->n_neurons_2 < 1 || hx->n_neurons_2 > kMaxHGen)) return NEP_EINVAL;
+    if (L >= 3 && (hx->n_neurons_3 < 1 || hx->n_neurons_3 > kMaxHGen)) return NEP_EINVAL;
+    if (hx->angular_kind != NEP_ANGULAR_QNL && hx->angular_kind != NEP_ANGULAR_QNNL) return NEP_EINVAL;
+    if (hx->angular_kind == NEP_ANGULAR_QNNL && (hy->n_max_radial > 7 || hy->n_max_angular > 7)) return NEP_EINVAL;
     nep_model* m = new (std::nothrow) nep_model();
     if (!m) return NEP_ENOMEM;
     m->h = *hy;
+    m->kind = hx->angular_kind; m->nlayers = L;
+    m->blob_dev = nullptr; m->blob64_dev = nullptr; m->params_dev = nullptr; m->params64_dev = nullptr;
     m->NR = hy->n_max_radial + 1; m->NA = hy->n_max_angular + 1; m->H = hy->n_neurons;
-    m->D = m->NR + m->NA * hy->l_max;                    // Eq. 16
-    m->npar = (m->D + 2) * m->H + 1;                     // Eq. 26
+    m->D = m->NR + (m->kind == NEP_ANGULAR_QNNL ? m->NA * (m->NA + 1) / 2 : m->NA) * hy->l_max;     // Eq. 16 (pairs n <= n' for Eq. 17)
+    m->lw[0] = hy->n_neurons; m->lw[1] = L >= 2 ? hx->n_neurons_2 : 0; m->lw[2] = L >= 3 ? hx->n_neurons_3 : 0;
+    {
+        int in = m->D, np = 0;
+        for (int k = 0; k < L; ++k) { np += (in + 1) * m->lw[k]; in = m->lw[k]; }
+        m->npar = np + in + 1;                           // Eq. 26 for L = 1: (D + 2) H + 1
+    }
     // staged fp32 layout: w1[H][Dp] (rows zero-padded to a multiple of 4) | b1[H] | w2[H] | b2
     const int H = m->H, D = m->D, Dp = (D + 3) & ~3;
     m->params_floats = (H * Dp + 2 * H + 1 + 3) & ~3;
     if (n_params != (size_t)m->npar) { delete m; return NEP_EINVAL; }
-    m->thread_path_ok = main_supported(m);
+    m->thread_path_ok = L == 1 && m->kind == NEP_ANGULAR_QNL && main_supported(m);
     if (!device_ok()) { delete m; set_cuda_error(cudaErrorNoDevice, "nep_create"); return NEP_ECUDA; }
     for (int t = 0; t < kMaxTypes; ++t) m->Z[t] = (hy->n_types > 1 && t < hy->n_types) ? atomic_number[t] : 1;
-    float* stage = new float[(size_t)m->params_floats]();
-    for (int mu = 0; mu < H; ++mu)
-        for (int v = 0; v < D; ++v) stage[mu * Dp + v] = (float)params[(size_t)mu * D + v];
-    for (int k = 0; k < 2 * H + 1; ++k) stage[H * Dp + k] = (float)params[(size_t)H * D + k];
     for (int a = 0; a < kMaxTypes; ++a)
         for (int b = 0; b < kMaxTypes; ++b) m->zz.zz[a * kMaxTypes + b] = (float)sqrt((double)m->Z[a] * (double)m->Z[b]);   // Eq. 19
-    cudaError_t e = cudaMalloc(&m->params_dev, (size_t)m->params_floats * sizeof(float));
-    if (e == cudaSuccess) e = cudaMemcpy(m->params_dev, stage, (size_t)m->params_floats * sizeof(float), cudaMemcpyHostToDevice);
-    delete[] stage;
-    m->params64_dev = nullptr;
     m->p64.rcR = hy->rc_radial; m->p64.rcA = hy->rc_angular; m->p64.H = H;
     for (int a = 0; a < kMaxTypes; ++a)
         for (int b = 0; b < kMaxTypes; ++b) m->p64.zz[a * kMaxTypes + b] = sqrt((double)m->Z[a] * (double)m->Z[b]);   // Eq. 19
-    if (e == cudaSuccess && hy->n_types > 1) {
-        e = cudaMalloc(&m->params64_dev, (size_t)m->npar * sizeof(double));
-        if (e == cudaSuccess) e = cudaMemcpy(m->params64_dev, params, (size_t)m->npar * sizeof(double), cudaMemcpyHostToDevice);
+    cudaError_t e = cudaSuccess;
+    if (L == 1) {
+        float* stage = new float[(size_t)m->params_floats]();
+        for (int mu = 0; mu < H; ++mu)
+            for (int v = 0; v < D; ++v) stage[mu * Dp + v] = (float)params[(size_t)mu * D + v];
+        for (int k = 0; k < 2 * H + 1; ++k) stage[H * Dp + k] = (float)params[(size_t)H * D + k];
+        e = cudaMalloc(&m->params_dev, (size_t)m->params_floats * sizeof(float));
+        if (e == cudaSuccess) e = cudaMemcpy(m->params_dev, stage, (size_t)m->params_floats * sizeof(float), cudaMemcpyHostToDevice);
+        delete[] stage;
+        if (e == cudaSuccess && hy->n_types > 1) {
+            e = cudaMalloc(&m->params64_dev, (size_t)m->npar * sizeof(double));
+            if (e == cudaSuccess) e = cudaMemcpy(m->params64_dev, params, (size_t)m->npar * sizeof(double), cudaMemcpyHostToDevice);
+        }
+    } else {
+        // deep network: one padded blob  W1[H1][in_p] | b1 | W2[H2][H1_p] | b2 | ... | w_out | b_out  (sections 4-aligned)
+        int off = 0, in = D;
+        for (int k = 0; k < L; ++k) {
+            m->lin_p[k] = (in + 3) & ~3;
+            m->off_w[k] = off; off += m->lw[k] * m->lin_p[k];
+            m->off_b[k] = off; off += (m->lw[k] + 3) & ~3;
+            in = m->lw[k];
+        }
+        m->off_out = off; off += (in + 1 + 3) & ~3;
+        m->blob_elems = off;
+        double* blob = new double[(size_t)off]();
+        const double* p = params;
+        in = D;
+        for (int k = 0; k < L; ++k) {
+            for (int mu = 0; mu < m->lw[k]; ++mu)
+                for (int v = 0; v < in; ++v) blob[m->off_w[k] + mu * m->lin_p[k] + v] = p[(size_t)mu * in + v];
+            p += (size_t)m->lw[k] * in;
+            for (int mu = 0; mu < m->lw[k]; ++mu) blob[m->off_b[k] + mu] = p[mu];
+            p += m->lw[k];
+            in = m->lw[k];
+        }
+        for (int mu = 0; mu <= in; ++mu) blob[m->off_out + mu] = p[mu];
+        if (hy->n_types > 1) {
+            e = cudaMalloc(&m->blob64_dev, (size_t)off * sizeof(double));
+            if (e == cudaSuccess) e = cudaMemcpy(m->blob64_dev, blob, (size_t)off * sizeof(double), cudaMemcpyHostToDevice);
+        } else {
+            float* bf = new float[(size_t)off];
+            for (int k = 0; k < off; ++k) bf[k] = (float)blob[k];
+            e = cudaMalloc(&m->blob_dev, (size_t)off * sizeof(float));
+            if (e == cudaSuccess) e = cudaMemcpy(m->blob_dev, bf, (size_t)off * sizeof(float), cudaMemcpyHostToDevice);
+            delete[] bf;
+        }
+        delete[] blob;
     }
     if (e != cudaSuccess) { set_cuda_error(e, "nep_create"); nep_destroy(m); return NEP_ECUDA; }
     *out = m;
@@ -1075,6 +1140,8 @@ void nep_destroy(nep_model* m) {
     if (!m) return;
     if (m->params_dev) cudaFree(m->params_dev);
     if (m->params64_dev) cudaFree(m->params64_dev);
+    if (m->blob_dev) cudaFree(m->blob_dev);
+    if (m->blob64_dev) cudaFree(m->blob64_dev);
     delete m;
 }
 

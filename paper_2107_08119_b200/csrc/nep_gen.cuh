@@ -37,6 +37,14 @@ struct GenParams {
     Box box;
     const float* params;                     // staged fp32 layout w1[H][Dp] | b1[H] | w2[H] | b2
     const double* params64;                  // fp64 layout w1[H][D] | b1[H] | w2[H] | b2 (TD = double)
+    // variants: the SOAP-like descriptor q_nn'l of Eq. 17 and two or three hidden layers
+    int kind;                                // 0: q_nl (Eq. 13), 1: q_nn'l for the pairs n <= n' (Eq. 17)
+    int nlayers;                             // hidden layers; > 1: the padded blob below replaces params / params64
+    int lw[3], lin_p[3];                     // width of hidden layer k and the padded length of its input rows
+    int off_w[3], off_b[3], off_out;         // element offsets of W_k, b_k and of w_out | b_out in the blob
+    int blob_elems;
+    const float* blob;                       // W1[H1][in_p] | b1 | W2[H2][H1_p] | b2 | ... | w_out | b_out, sections 4-aligned
+    const double* blob64;
     float* q_out;                            // nullable parity hooks, [D][N] caller order
     float* fp_out;
 };
@@ -46,9 +54,10 @@ struct alignas(16) GenSmem {                 // per group of lanes
     TD S[NMAX][kNumLM];                      // s[n][lm], later (TD = float) A[n][lm] in place
     TD Gs[kGenLanes][NMAX + 1];              // chunk: g_n of G neighbours (odd row stride: conflict-free stores)
     TD Bs[kGenLanes][kNumLM + 1];            // chunk: b_lm of G neighbours
-    TD q[NMAX * 5];                          // descriptor
-    float Fp[NMAX * 5];                      // dU/dq
-    TD hid[kMaxHGen];                        // w2 (1 - tanh^2) per neuron
+    TD q[NMAX == 8 ? 152 : NMAX * 5];        // descriptor (NMAX = 8 also holds the 8 + 36 x 4 components of q_nn'l)
+    float Fp[NMAX == 8 ? 152 : NMAX * 5];    // dU/dq
+    TD hid[kMaxHGen];                        // w2 (1 - tanh^2) per neuron; deep networks: layer 1
+    TD act[2][kMaxHGen];                     // deep networks: layers 2 and 3
     float A[sizeof(TD) == 8 ? NMAX * kNumLM : 1];    // TD = double: fp32 copy of A for the force phase
 };
 
@@ -91,7 +100,10 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
     // the forward sweep's per-lane rows fall into distinct bank groups
     const int Dps = F64 ? (Dp | 1) : Dp + 4;             // odd stride in 8-byte units for doubles
     TD* wsm = reinterpret_cast<TD*>(gsm_raw + (size_t)kGenAtomsPerBlock * sizeof(SM));       // w1[H][Dps] | b1[H] | w2[H] | b2
-    {
+    if (P.nlayers > 1) {                                                  // deep network: the host-padded blob as it is
+        for (int e = threadIdx.x; e < P.blob_elems; e += blockDim.x) wsm[e] = F64 ? (TD)P.blob64[e] : (TD)P.blob[e];
+        __syncthreads();
+    } else {
         for (int mu = warp; mu < H; mu += kGenWarps) {                    // one row per warp: every load in flight at once
             TD* dst = wsm + mu * Dps;
             if (F64) {
@@ -210,6 +222,19 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
                 sm.S[hn + n][3 * tl] = acc[n][0]; sm.S[hn + n][3 * tl + 1] = acc[n][1]; sm.S[hn + n][3 * tl + 2] = acc[n][2];
             }
             __syncwarp();
+            if (P.kind == 1) {                                           // q_nn'l = (2l+1)/(4 pi) sum_m C_lm s_nlm s_n'lm, n <= n'
+                for (int pi2 = gl; pi2 < NA * (NA + 1) / 2; pi2 += kGenLanes) {
+                    int n = 0, rem = pi2;
+                    while (rem >= NA - n) { rem -= NA - n; ++n; }
+                    const int n2 = n + rem;
+                    TD v[4] = {(TD)0, (TD)0, (TD)0, (TD)0};
+#pragma unroll
+                    for (int m = 0; m < kNumLM; ++m) v[LOF[m] - 1] += (TD)C[m] * sm.S[n][m] * sm.S[n2][m];
+#pragma unroll
+                    for (int l = 0; l < 4; ++l)
+                        if (l < LMAX) sm.q[NR + pi2 * LMAX + l] = v[l] * (TD)((2 * l + 3) * 0.07957747154594767);    // (2l+1)/(4 pi), l = index + 1
+                }
+            } else
             for (int n = gl; n < NA; n += kGenLanes) {                   // q_nl, descriptor order n-major, l = 1..l_max
                 TD v[4] = {(TD)0, (TD)0, (TD)0, (TD)0};
 #pragma unroll
@@ -226,7 +251,55 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
         }
 
         // ---- N: network, Eq. 21-22 (minus biases), and Fp = dU/dq ----
-        {
+        if (P.nlayers > 1) {                  // more hidden layers: x^(k) = tanh(W^(k) x^(k-1) - b^(k))
+            if (gl < Dp - D) sm.q[D + gl] = (TD)0;
+            __syncwarp();
+            const int L = P.nlayers;
+            TD* bufs[3] = {sm.hid, sm.act[0], sm.act[1]};
+            const TD* xin = sm.q;
+            for (int k = 0; k < L; ++k) {
+                const int wk = P.lw[k], inp = P.lin_p[k];
+                const TD* W = wsm + P.off_w[k];
+                const TD* bk = wsm + P.off_b[k];
+                TD* xout = bufs[k];
+                for (int mu = gl; mu < wk; mu += kGenLanes) {
+                    const TD* w = W + mu * inp;
+                    TD a0 = -bk[mu], a1 = (TD)0;
+                    for (int v = 0; v < inp; v += 2) { a0 += w[v] * xin[v]; a1 += w[v + 1] * xin[v + 1]; }
+                    TD t, dd;
+                    GenMath<TD>::act(a0 + a1, &t, &dd);
+                    xout[mu] = t;
+                }
+                if (gl < 4 && wk + gl < kMaxHGen) xout[wk + gl] = (TD)0;  // zero tail up to the next layer's padded row length
+                __syncwarp();
+                xin = xout;
+            }
+            const int HL = P.lw[L - 1];
+            const TD* wout = wsm + P.off_out;
+            TD* xl = bufs[L - 1];
+            TD Upart = (TD)0;
+            for (int m = gl; m < HL; m += kGenLanes) {
+                const TD t = xl[m];
+                Upart += wout[m] * t;
+                xl[m] = wout[m] * ((TD)1 - t) * ((TD)1 + t);              // delta^(L)
+            }
+#pragma unroll
+            for (int o = 1; o < kGenLanes; o <<= 1) Upart += __shfl_xor_sync(0xffffffffu, Upart, o);
+            if (gl == 0 && valid) d.Us[i] = (float)(Upart - wout[HL]);
+            __syncwarp();
+            for (int k = L - 1; k >= 0; --k) {                            // delta^(k-1) = (W^(k))^T delta^(k) (1 - x^(k-1)^2)
+                const int wk = P.lw[k], inp = P.lin_p[k], nin = k == 0 ? D : P.lw[k - 1];
+                const TD* W = wsm + P.off_w[k];
+                const TD* dk = bufs[k];
+                for (int v = gl; v < nin; v += kGenLanes) {
+                    TD sacc = (TD)0;
+                    for (int m = 0; m < wk; ++m) sacc += dk[m] * W[m * inp + v];
+                    if (k == 0) sm.Fp[v] = (float)sacc;
+                    else { const TD t = bufs[k - 1][v]; bufs[k - 1][v] = sacc * ((TD)1 - t) * ((TD)1 + t); }
+                }
+                __syncwarp();
+            }
+        } else {
             if (gl < Dp - D) sm.q[D + gl] = (TD)0;                        // the padded tail of q (w1's padded columns are zero too)
             __syncwarp();
             TD Upart = (TD)0;
@@ -269,6 +342,29 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
 
         // ---- F: partial forces, Eq. 23-25 ----
         float* A = F64 ? sm.A : reinterpret_cast<float*>(&sm.S[0][0]);     // A[n][lm] = 2 Fp_nl C_lm s_nlm (0 beyond l_max)
+        if (P.kind == 1) {
+            // A[n][m] = (2l+1)/(4 pi) C_m [ 2 Fp_nn s_n + sum_{b>n} Fp_nb s_b + sum_{a<n} Fp_an s_a ]: needs every row of s,
+            // so it is built beside s (TD = float: in the chunk buffers, free by now)
+            if (!F64) A = reinterpret_cast<float*>(&sm.Gs[0][0]);
+            for (int e = gl; e < NMAX * kNumLM; e += kGenLanes) {
+                const int n = e / kNumLM, m = e - n * kNumLM;
+                float acc = 0.f;
+                if (n < NA) {
+                    int lm1 = 0;                                          // l - 1 of component m
+                    lm1 = m < 3 ? 0 : (m < 8 ? 1 : (m < 15 ? 2 : 3));
+                    if (lm1 < LMAX) {
+                        for (int b = 0; b < NA; ++b) {
+                            const int lo = min(n, b), hi = max(n, b);
+                            const int pidx = lo * NA - lo * (lo - 1) / 2 + (hi - lo);
+                            const float f = sm.Fp[NR + pidx * LMAX + lm1] * (b == n ? 2.f : 1.f);
+                            acc = fmaf(f, (float)sm.S[b][m], acc);
+                        }
+                        acc *= clm(m) * (float)((2 * lm1 + 3) * 0.07957747154594767);
+                    }
+                }
+                A[e] = acc;
+            }
+        } else
         for (int n = gl; n < NMAX; n += kGenLanes) {                     // row n: in place when TD = float (same lane reads and writes it)
             float fl[4];
 #pragma unroll

@@ -1,0 +1,78 @@
+"""GPU parity of the variants of SURVEY.md 8(f) f-4 (nep_create_ex): two or three hidden layers and the
+SOAP-like descriptor q_nn'l of Eq. 17-18, against the oracle's variant branches."""
+import numpy as np
+import pytest
+
+from paper_2107_08119_b200 import inputs
+from test_gpu_parity import TOL_REL, _gpu, check_lists, compare_outputs
+
+pytestmark = pytest.mark.gpu
+
+
+def _setup(oracle, w, layers, kind, caps, skin, seed=41):
+    torch, api = _gpu()
+    h = oracle.Hyper(w.rc_r, w.rc_a, w.n_max_r, w.n_max_a, w.l_max, layers[0], len(w.atomic_numbers))
+    h.nlayers = len(layers); h.nneu2 = layers[1] if len(layers) > 1 else 0; h.nneu3 = layers[2] if len(layers) > 2 else 0
+    h.kind = kind
+    npar = oracle.num_params(h)
+    par = (2.0 * inputs.uniform01(seed, npar) - 1.0) / np.sqrt(30.0)
+    model = api.Model(w.rc_r, w.rc_a, w.n_max_r, w.n_max_a, w.l_max, layers[0], w.atomic_numbers, par,
+                      hidden_layers=layers if len(layers) > 1 else (layers if kind else None), angular_kind=kind)
+    assert model.descriptor_dim == oracle.descriptor_dim(h) and model.num_params == npar
+    types = torch.from_numpy(w.types).cuda()
+    system = api.System(model, types, caps[0], caps[1], skin)
+    assert system.path == 2
+    pos = torch.from_numpy(w.pos).cuda().contiguous(); vel = torch.from_numpy(w.vel).cuda().contiguous()
+    return h, par, model, system, pos, vel
+
+
+@pytest.mark.parametrize("which", ["c0", "c2", "c3_replica"])
+@pytest.mark.parametrize("layers,kind", [((30, 20), 0), ((24, 16, 9), 0), ((30,), 1), ((20, 12), 1)])
+def test_variants_match_oracle(oracle, which, layers, kind):
+    w, caps, skin = {"c0": (inputs.config0(), (64, 32), 0.4), "c2": (inputs.config2(), (80, 40), 1.0),
+                     "c3_replica": (inputs.config3(cells=(4, 4, 4)), (80, 40), 1.0)}[which]
+    h, par, model, system, pos, vel = _setup(oracle, w, layers, kind, caps, skin)
+    system.neighbors(pos, w.box)
+    out = system.compute(pos, vel)
+    system.status()
+    ref = oracle.evaluate(h, w.atomic_numbers, par, w.pos, w.vel, w.types, w.box, 96, 64)
+    compare_outputs(out, ref, label="%s layers %s kind %d" % (which, layers, kind))
+
+
+def test_soap_like_intermediate_rows(oracle):
+    torch, api = _gpu()
+    w = inputs.config0()
+    h, par, model, system, pos, vel = _setup(oracle, w, (30,), 1, (64, 32), 0.4)
+    system.neighbors(pos, w.box)
+    q, fp, p = [t.cpu().numpy().astype(np.float64) for t in system.compute_internals(pos)]
+    system.status()
+    ocR, oiR, _ = oracle.neighbors(w.pos, w.box, w.rc_r, 96)
+    ocA, oiA, _ = oracle.neighbors(w.pos, w.box, w.rc_a, 64)
+    ref = oracle.compute(h, w.atomic_numbers, par, w.pos, w.vel, w.types, w.box, ocR, oiR, ocA, oiA, want_internals=True)
+    assert q.shape[0] == 8 + 36 * 4
+    assert np.abs(q.T - ref["q"]).max() <= 2e-6 * np.abs(ref["q"]).max()
+    assert np.abs(fp.T - ref["Fp"]).max() <= 2e-5 * np.abs(ref["Fp"]).max()
+
+
+def test_md_with_deep_network_conserves_energy_like_the_oracle(oracle):
+    torch, api = _gpu()
+    w = inputs.config1()
+    h, par, model, system, pos, vel = _setup(oracle, w, (30, 20), 0, (64, 32), 1.0)
+    system.neighbors(pos, w.box)
+    thermo = torch.zeros((40, 5), dtype=torch.float64, device="cuda")
+    system.md_step(pos, vel, w.masses, w.dt, 40, thermo=thermo)
+    system.status()
+    ref = oracle.md(h, w.atomic_numbers, par, w.pos, w.vel, w.types, w.box, w.masses, w.dt, 40)
+    th = thermo.cpu().numpy()
+    E, Eref = th[:, 0] + th[:, 1], ref["thermo"][1:, 0] + ref["thermo"][1:, 1]
+    assert np.abs(E - Eref).max() / w.n_atoms < 1e-5
+    assert np.abs(pos.cpu().numpy() - ref["pos"]).max() < 1e-4
+
+
+def test_create_ex_validation():
+    torch, api = _gpu()
+    w = inputs.config0()
+    with pytest.raises(api.NepError):          # q_nn'l needs n_max <= 7
+        api.Model(w.rc_r, w.rc_a, 8, 8, 4, 30, w.atomic_numbers, np.zeros(10), hidden_layers=[30], angular_kind=1)
+    with pytest.raises(api.NepError):          # four hidden layers
+        api.Model(w.rc_r, w.rc_a, 7, 7, 4, 30, w.atomic_numbers, np.zeros(10), hidden_layers=[30, 20, 10, 5])

@@ -540,3 +540,91 @@ int orc_md(int64_t n, double *pos, double *vel, const int *type, const double *b
     return orc_md_driven(n, pos, vel, type, box, h, znum, params, mass_by_type, dt, n_steps, capR, capA,
                          NULL, NULL, NULL, U, F, W, J, Jsum, thermo);
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Training side (Sec. II E): the loss of Eq. 29-34 over a set of structures and one
+ * generation of the separable natural evolution strategy, Eq. 35-39.  Plain loops, one structure and
+ * one population member at a time; "all structures concatenated" is only the layout of
+ * the inputs: positions / types / forces of structure n occupy atoms first[n] .. first[n+1]-1.
+ *
+ * Readings (the paper is silent; Q23-Q25):
+ *   Q23  "eV/atom for energy and virial": U(n) and W(n) of Eq. 30 / 32 are the structure's
+ *        total energy and total virial divided by its number of atoms.
+ *   Q24  the six independent components mu nu of Eq. 32 are xx, yy, zz, xy, yz, zx of the total virial.
+ *   Q25  the rank-based utilities u_k are not printed ("see Ref. 44"): the standard NES choice
+ *        u_k = max(0, ln(N_pop/2 + 1) - ln k) / sum_j max(0, ln(N_pop/2 + 1) - ln j) - 1/N_pop  for the member of
+ *        rank k (k = 1 the smallest loss), which sums to zero.  Ties are broken by member index.
+ * ------------------------------------------------------------------------------------------------ */
+
+/* Eq. 30-34 and 29 for ONE parameter vector z.  box[S][3]; first[S+1]; pos/F_tar [3][N] concatenated; e_tar[S] per
+ * atom; v_tar[S][6] per atom; lambda[5] = lambda_e, lambda_f, lambda_v, lambda_1, lambda_2.
+ * out[6] = L_e, L_f, L_v, L_1, L_2, L.  Returns 0 or orc_evaluate's error. */
+int orc_loss(int S, const int64_t *first, const double *pos, const int *type, const double *box,
+             const orc_hyper *h, const int *znum, const double *z, int capR, int capA,
+             const double *e_tar, const double *f_tar, const double *v_tar, const double *lambda, double *out) {
+    const int64_t N = first[S];
+    const int npar = orc_num_params(h);
+    double sse_e = 0.0, sse_f = 0.0, sse_v = 0.0;
+    static const int comp[6] = {0, 4, 8, 1, 5, 6};            /* xx yy zz xy yz zx of the row-major 3x3 */
+    for (int n = 0; n < S; ++n) {
+        const int64_t a0 = first[n], nat = first[n + 1] - a0;
+        double *p = (double *)malloc(sizeof(double) * 3 * nat);
+        double *U = (double *)malloc(sizeof(double) * nat), *F = (double *)malloc(sizeof(double) * 3 * nat);
+        double *W = (double *)malloc(sizeof(double) * 9 * nat);
+        for (int a = 0; a < 3; ++a) for (int64_t i = 0; i < nat; ++i) p[a * nat + i] = pos[a * N + a0 + i];
+        int rc = orc_evaluate(nat, p, NULL, type + a0, box + 3 * n, h, znum, z, capR, capA, U, F, W, NULL);
+        if (rc) { free(p); free(U); free(F); free(W); return rc; }
+        double e = 0.0, w[6] = {0, 0, 0, 0, 0, 0};
+        for (int64_t i = 0; i < nat; ++i) {
+            e += U[i];
+            for (int c = 0; c < 6; ++c) w[c] += W[comp[c] * nat + i];
+            for (int a = 0; a < 3; ++a) { double df = F[a * nat + i] - f_tar[a * N + a0 + i]; sse_f += df * df; }   /* Eq. 31 */
+        }
+        e /= (double)nat;                                                                   /* Q23 */
+        sse_e += (e - e_tar[n]) * (e - e_tar[n]);                                           /* Eq. 30 */
+        for (int c = 0; c < 6; ++c) { double dv = w[c] / (double)nat - v_tar[6 * n + c]; sse_v += dv * dv; }   /* Eq. 32 */
+        free(p); free(U); free(F); free(W);
+    }
+    double l1 = 0.0, l2 = 0.0;
+    for (int k = 0; k < npar; ++k) { l1 += fabs(z[k]); l2 += z[k] * z[k]; }
+    out[0] = sqrt(sse_e / S); out[1] = sqrt(sse_f / (3.0 * N)); out[2] = sqrt(sse_v / (6.0 * S));
+    out[3] = l1 / npar; out[4] = sqrt(l2 / npar);                                           /* Eq. 33-34 */
+    out[5] = lambda[0] * out[0] + lambda[1] * out[1] + lambda[2] * out[2] + lambda[3] * out[3] + lambda[4] * out[4];   /* Eq. 29 */
+    return 0;
+}
+
+/* Eq. 35: z_k = m + s (.) r_k for the whole population; z, r [npop][npar]. */
+void orc_snes_sample(int npop, int npar, const double *m, const double *s, const double *r, double *z) {
+    for (int k = 0; k < npop; ++k)
+        for (int n = 0; n < npar; ++n) z[(size_t)k * npar + n] = m[n] + s[n] * r[(size_t)k * npar + n];
+}
+
+/* Rank-based utilities of reading Q25: util[k] for member k given the losses. */
+void orc_snes_utilities(int npop, const double *loss, double *util) {
+    double norm = 0.0;
+    for (int j = 1; j <= npop; ++j) { double v = log(npop / 2.0 + 1.0) - log((double)j); norm += v > 0 ? v : 0; }
+    for (int k = 0; k < npop; ++k) {
+        int rank = 1;                                   /* 1 = smallest loss; ties by index */
+        for (int j = 0; j < npop; ++j) if (loss[j] < loss[k] || (loss[j] == loss[k] && j < k)) ++rank;
+        double v = log(npop / 2.0 + 1.0) - log((double)rank);
+        util[k] = (v > 0 ? v : 0) / norm - 1.0 / npop;
+    }
+}
+
+/* Eq. 36-39: one update of (m, s) from the population's random vectors and losses. */
+void orc_snes_update(int npop, int npar, const double *r, const double *loss, double eta_m, double eta_s,
+                     double *m, double *s) {
+    double *u = (double *)malloc(sizeof(double) * npop);
+    orc_snes_utilities(npop, loss, u);
+    for (int n = 0; n < npar; ++n) {
+        double gm = 0.0, gs = 0.0;
+        for (int k = 0; k < npop; ++k) {
+            double rk = r[(size_t)k * npar + n];
+            gm += u[k] * rk;                            /* Eq. 36 */
+            gs += u[k] * (rk * rk - 1.0);               /* Eq. 37 */
+        }
+        m[n] += eta_m * (s[n] * gm);                    /* Eq. 38 */
+        s[n] *= exp(0.5 * eta_s * gs);                  /* Eq. 39 */
+    }
+    free(u);
+}

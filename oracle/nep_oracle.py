@@ -11,7 +11,8 @@ import numpy as np
 from . import build as _build
 
 __all__ = ["Hyper", "num_threads", "descriptor_dim", "num_params", "chebyshev", "cutoff", "radial",
-           "legendre", "neighbors", "network", "descriptor_atom", "compute", "evaluate", "md", "md_driven"]
+           "legendre", "neighbors", "network", "descriptor_atom", "compute", "evaluate", "md", "md_driven",
+           "loss", "snes_sample", "snes_utilities", "snes_update"]
 
 _lib = C.CDLL(_build.build())
 _dp = C.POINTER(C.c_double)
@@ -181,3 +182,44 @@ def md_driven(h: Hyper, znum, params, pos, vel, types, box, masses, dt, n_steps,
     if rc:
         raise RuntimeError("orc_md_driven failed: %d" % rc)
     return out
+
+
+_lib.orc_loss.restype = C.c_int
+
+
+def loss(h: Hyper, znum, z, first, pos, types, boxes, e_tar, f_tar, v_tar, lambdas, capR=96, capA=64):
+    """Eq. 29-34 for one parameter vector: -> [L_e, L_f, L_v, L_1, L_2, L]."""
+    first = np.ascontiguousarray(first, dtype=np.int64); pos = np.ascontiguousarray(pos, dtype=np.float64)
+    types = np.ascontiguousarray(types, dtype=np.int32); boxes = np.ascontiguousarray(boxes, dtype=np.float64)
+    znum = np.ascontiguousarray(znum, dtype=np.int32); z = np.ascontiguousarray(z, dtype=np.float64)
+    e_tar = np.ascontiguousarray(e_tar, dtype=np.float64); f_tar = np.ascontiguousarray(f_tar, dtype=np.float64)
+    v_tar = np.ascontiguousarray(v_tar, dtype=np.float64); lam = np.ascontiguousarray(lambdas, dtype=np.float64)
+    assert z.size == num_params(h)
+    out = np.zeros(6)
+    rc = _lib.orc_loss(C.c_int(len(first) - 1), first.ctypes.data_as(C.POINTER(C.c_int64)), _d(pos), _i(types), _d(boxes),
+                       C.byref(h), _i(znum), _d(z), C.c_int(capR), C.c_int(capA), _d(e_tar), _d(f_tar), _d(v_tar), _d(lam), _d(out))
+    if rc:
+        raise RuntimeError("orc_loss failed: %d" % rc)
+    return out
+
+
+def snes_sample(m, s, r):
+    m = np.ascontiguousarray(m, dtype=np.float64); s = np.ascontiguousarray(s, dtype=np.float64)
+    r = np.ascontiguousarray(r, dtype=np.float64)
+    z = np.zeros_like(r)
+    _lib.orc_snes_sample(C.c_int(r.shape[0]), C.c_int(r.shape[1]), _d(m), _d(s), _d(r), _d(z))
+    return z
+
+
+def snes_utilities(losses):
+    l = np.ascontiguousarray(losses, dtype=np.float64); u = np.zeros_like(l)
+    _lib.orc_snes_utilities(C.c_int(l.size), _d(l), _d(u))
+    return u
+
+
+def snes_update(m, s, r, losses, eta_m, eta_s):
+    """Eq. 36-39: returns the updated (m, s)."""
+    m = np.array(m, dtype=np.float64); s = np.array(s, dtype=np.float64)
+    r = np.ascontiguousarray(r, dtype=np.float64); l = np.ascontiguousarray(losses, dtype=np.float64)
+    _lib.orc_snes_update(C.c_int(r.shape[0]), C.c_int(r.shape[1]), _d(r), _d(l), C.c_double(eta_m), C.c_double(eta_s), _d(m), _d(s))
+    return m, s

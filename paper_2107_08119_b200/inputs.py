@@ -309,3 +309,43 @@ def table1(which: str, cells=None, sigma: float = 0.1) -> Workload:
     dim = descriptor_dim(hyp[2], hyp[3], hyp[4])
     return Workload("table1_" + which, np.ascontiguousarray(r.T), vel, types, box, hyp[0], hyp[1], hyp[2], hyp[3],
                     hyp[4], hyp[5], zs, masses, make_params(dim, hyp[5], 25), 1.0, 100)
+
+
+# --------------------------------------------------------------------------- training-side inputs
+@dataclasses.dataclass
+class TrainingSet:
+    """Small periodic structures concatenated into one system: atoms first[n] .. first[n+1]-1 belong
+    to structure n, which has its own orthorhombic box boxes[n]."""
+    first: np.ndarray        # (S+1,) int64
+    pos: np.ndarray          # (3, N) float64, concatenated
+    types: np.ndarray        # (N,) int32
+    boxes: np.ndarray        # (S, 3) float64
+
+    @property
+    def n_structures(self) -> int:
+        return self.boxes.shape[0]
+
+    @property
+    def n_atoms(self) -> int:
+        return self.pos.shape[1]
+
+
+def training_set(n_structures: int = 24, seed: int = 50, cells=(2, 2, 2)) -> TrainingSet:
+    """Seeded stand-in for a training set of ~100-atom structures: diamond-Si supercells with a
+    per-structure lattice constant in [5.35, 5.60] A (strain), an anisotropic stretch of up to 2 % per axis and a Gaussian
+    jitter of 0.03-0.15 A, every third structure with a vacancy (63 atoms).  Every box edge exceeds 2 r_c^R = 10 A."""
+    u = uniform01(seed, 8 * n_structures)
+    pos, boxes, first = [], [], [0]
+    for n in range(n_structures):
+        a = 5.35 + 0.25 * u[8 * n]
+        stretch = 1.0 + 0.02 * (2.0 * u[8 * n + 1:8 * n + 4] - 1.0)
+        sigma = 0.03 + 0.12 * u[8 * n + 4]
+        box = np.array(cells, dtype=np.float64) * a * stretch
+        r = _lattice(_DIAMOND_BASIS, a, cells) * stretch
+        if n % 3 == 2:
+            r = np.delete(r, int(u[8 * n + 5] * r.shape[0]), axis=0)
+        r = _jitter_wrap(r, sigma, seed + 1000 + n, box)
+        pos.append(r); boxes.append(box); first.append(first[-1] + r.shape[0])
+    allpos = np.concatenate(pos, axis=0)
+    return TrainingSet(np.array(first, dtype=np.int64), np.ascontiguousarray(allpos.T), np.zeros(allpos.shape[0], dtype=np.int32),
+                       np.array(boxes))

@@ -216,6 +216,43 @@ int  nep_measure_fp32_peak(double* tflops_ffma, double* tflops_ffma2, void* cuda
  * They are the attainable ceilings of k_main's inner loops, reported beside the nominal peak. */
 int  nep_measure_fp32_patterns(double tflops[3], void* cuda_stream);
 
+/* ---- training side (Sec. II E-F) ------------------------------------------------ */
+
+/* The loss of Eq. 29-34 for a population of parameter vectors over a training set of small periodic structures
+ * "combined into a single one", and the separable natural evolution strategy of Eq. 35-39.
+ * Structure n owns atoms first[n] .. first[n+1]-1 of the concatenated arrays and its own orthorhombic box
+ * boxes[n][3] (every edge > 2 r_c^R: minimum image inside the structure).  Readings (Q23-Q25): U(n) and
+ * W(n) of Eq. 30 / 32 are per atom ("eV/atom for energy and virial"); the six virial components are
+ * xx, yy, zz, xy, yz, zx; the rank utilities u_k of Eq. 36-37, which the paper defers to its Ref. 44, are
+ * max(0, ln(N_pop/2+1) - ln k) normalised to sum 1, minus 1/N_pop (k = 1 the smallest loss, ties by member index).
+ * The structures do not move, so lists and records are built once in nep_trainer_create; single-species models only.
+ *   first [S+1], boxes [S][3]: HOST.  pos_dev [3][N] fp64 (N = first[S]).
+ *   e_tar_dev [S] (per atom), f_tar_dev [3][N], v_tar_dev [S][6] (per atom): fp32 DEVICE targets, caller-owned, must
+ *   outlive the trainer; all three nullable if only nep_trainer_predict is used. */
+typedef struct nep_trainer nep_trainer;
+size_t nep_trainer_workspace_bytes(const nep_hyper_ex*, int n_structures, int64_t n_atoms, int cap_radial, int cap_angular);
+int  nep_trainer_create(const nep_hyper_ex*, int n_structures, const int64_t* first, const double* boxes,
+                        const double* pos_dev, const float* e_tar_dev, const float* f_tar_dev, const float* v_tar_dev,
+                        int cap_radial, int cap_angular, void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
+                        nep_trainer** out);
+void nep_trainer_destroy(nep_trainer*);
+int  nep_trainer_num_params(const nep_trainer*);
+int  nep_trainer_status(nep_trainer*);      /* as nep_status (capacity overflow) */
+
+/* Eq. 29-34 for n_pop parameter vectors z_dev [n_pop][N_par] (fp64 device, the order of nep_create / nep_create_ex):
+ * loss_dev [n_pop][6] = L_e, L_f, L_v, L_1, L_2 and the weighted total L; lambda [5] HOST = lambda_e, _f, _v, _1, _2. */
+int  nep_trainer_losses(nep_trainer*, const double* z_dev, int n_pop, const double* lambda, double* loss_dev, void* cuda_stream);
+
+/* One parameter vector: per-atom energy e_dev [S], forces f_dev [3][N], per-atom virial v_dev [S][6] (each nullable). */
+int  nep_trainer_predict(nep_trainer*, const double* z_dev, float* e_dev, float* f_dev, float* v_dev, void* cuda_stream);
+
+/* Eq. 35: z_k = m + s (.) r_k; r_dev [n_pop][n_par] standard normals supplied by the caller. */
+int  nep_snes_sample(const double* m_dev, const double* s_dev, const double* r_dev, int n_pop, int n_par, double* z_dev,
+                     void* cuda_stream);
+/* Eq. 36-39: natural gradients from the ranks of loss_dev[k * loss_stride], then m and s in place (n_pop <= 1024). */
+int  nep_snes_update(double* m_dev, double* s_dev, const double* r_dev, const double* loss_dev, int loss_stride, int n_pop,
+                     int n_par, double eta_m, double eta_s, void* cuda_stream);
+
 const char* nep_strerror(int code);
 
 #ifdef __cplusplus

@@ -17,6 +17,8 @@ _lib = None
 SYMBOLS = ["nep_create", "nep_create_ex", "nep_descriptor_dim", "nep_num_params", "nep_destroy", "nep_workspace_bytes",
            "nep_system_create", "nep_system_destroy", "nep_system_set_path", "nep_system_path", "nep_neighbors", "nep_get_neighbors", "nep_compute", "nep_compute_internals",
            "nep_md_step", "nep_md_step_driven", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile", "nep_measure_fp32_peak", "nep_measure_fp32_patterns",
+           "nep_trainer_workspace_bytes", "nep_trainer_create", "nep_trainer_destroy", "nep_trainer_num_params", "nep_trainer_status",
+           "nep_trainer_losses", "nep_trainer_predict", "nep_snes_sample", "nep_snes_update",
            "nep_strerror"]
 
 
@@ -68,6 +70,17 @@ def lib():
         L.nep_launch_count.argtypes = [C.c_void_p]
         L.nep_launch_count.restype = C.c_int64
         L.nep_profile.argtypes = [C.c_void_p, C.c_int]
+        L.nep_trainer_workspace_bytes.restype = C.c_size_t
+        L.nep_trainer_workspace_bytes.argtypes = [C.POINTER(HyperEx), C.c_int, C.c_int64, C.c_int, C.c_int]
+        L.nep_trainer_create.argtypes = [C.POINTER(HyperEx), C.c_int] + [C.c_void_p] * 6 + [C.c_int, C.c_int, C.c_void_p, C.c_size_t,
+                                          C.c_void_p, C.POINTER(C.c_void_p)]
+        L.nep_trainer_destroy.argtypes = [C.c_void_p]; L.nep_trainer_destroy.restype = None
+        L.nep_trainer_num_params.argtypes = [C.c_void_p]; L.nep_trainer_status.argtypes = [C.c_void_p]
+        L.nep_trainer_losses.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nep_trainer_predict.argtypes = [C.c_void_p] * 6
+        L.nep_snes_sample.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.nep_snes_update.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double,
+                                      C.c_double, C.c_void_p]
         L.nep_get_profile.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
@@ -255,3 +268,67 @@ def from_workload(w, cap_radial=64, cap_angular=32, skin=1.0, device="cuda:0", p
     pos = torch.from_numpy(w.pos).to(device).contiguous()
     vel = torch.from_numpy(w.vel).to(device).contiguous()
     return model, system, pos, vel
+
+
+class Trainer:
+    """nep_trainer_*: the loss of Eq. 29-34 for a population over concatenated structures, and SNES (Eq. 35-39)."""
+
+    def __init__(self, rc_radial, rc_angular, n_max_radial, n_max_angular, l_max, hidden_layers, first, boxes, pos,
+                 e_tar=None, f_tar=None, v_tar=None, angular_kind=0, cap_radial=64, cap_angular=32):
+        w = list(hidden_layers)
+        base = Hyper(rc_radial, rc_angular, n_max_radial, n_max_angular, l_max, w[0], 1)
+        self.hx = HyperEx(base, len(w), w[1] if len(w) > 1 else 0, w[2] if len(w) > 2 else 0, angular_kind)
+        first = np.ascontiguousarray(first, dtype=np.int64); boxes = np.ascontiguousarray(boxes, dtype=np.float64)
+        self.n_structures, self.n = len(first) - 1, int(first[-1])
+        assert pos.is_cuda and pos.dtype == torch.float64 and pos.is_contiguous() and pos.shape == (3, self.n)
+        self._keep = (pos, e_tar, f_tar, v_tar)              # the library keeps these pointers
+        nbytes = lib().nep_trainer_workspace_bytes(C.byref(self.hx), self.n_structures, self.n, cap_radial, cap_angular)
+        if nbytes == 0:
+            raise NepError(-1, "nep_trainer_workspace_bytes")
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=pos.device)
+        off = (-self.workspace.data_ptr()) % 256
+        self._h = C.c_void_p()
+        _check(lib().nep_trainer_create(C.byref(self.hx), self.n_structures, first.ctypes.data_as(C.c_void_p),
+                                        boxes.ctypes.data_as(C.c_void_p), _ptr(pos), _ptr(e_tar), _ptr(f_tar), _ptr(v_tar),
+                                        cap_radial, cap_angular, C.c_void_p(self.workspace.data_ptr() + off), nbytes, _stream(),
+                                        C.byref(self._h)), "nep_trainer_create")
+        self.num_params = lib().nep_trainer_num_params(self._h)
+
+    def losses(self, z, lambdas):
+        """z [n_pop, N_par] fp64 cuda -> [n_pop, 6] = L_e, L_f, L_v, L_1, L_2, L."""
+        assert z.is_cuda and z.dtype == torch.float64 and z.is_contiguous() and z.shape[1] == self.num_params
+        lam = np.ascontiguousarray(lambdas, dtype=np.float64)
+        out = torch.zeros((z.shape[0], 6), dtype=torch.float64, device=z.device)
+        _check(lib().nep_trainer_losses(self._h, _ptr(z), z.shape[0], lam.ctypes.data_as(C.c_void_p), _ptr(out), _stream()),
+               "nep_trainer_losses")
+        return out
+
+    def predict(self, z):
+        dev = z.device
+        e = torch.zeros(self.n_structures, dtype=torch.float32, device=dev)
+        f = torch.zeros((3, self.n), dtype=torch.float32, device=dev)
+        v = torch.zeros((self.n_structures, 6), dtype=torch.float32, device=dev)
+        _check(lib().nep_trainer_predict(self._h, _ptr(z), _ptr(e), _ptr(f), _ptr(v), _stream()), "nep_trainer_predict")
+        return e, f, v
+
+    def status(self):
+        _check(lib().nep_trainer_status(self._h), "nep_trainer_status")
+
+    def __del__(self):
+        if getattr(self, "_h", None) and self._h.value and _lib is not None:
+            _lib.nep_trainer_destroy(self._h)
+            self._h = C.c_void_p()
+
+
+def snes_sample(m, s, r):
+    z = torch.empty_like(r)
+    _check(lib().nep_snes_sample(_ptr(m), _ptr(s), _ptr(r), r.shape[0], r.shape[1], _ptr(z), _stream()), "nep_snes_sample")
+    return z
+
+
+def snes_update(m, s, r, loss, eta_m, eta_s):
+    """In place on m, s; loss: [n_pop] or [n_pop, 6] (the total is column 5)."""
+    stride = 1 if loss.dim() == 1 else loss.shape[1]
+    ptr = loss.data_ptr() + (0 if loss.dim() == 1 else 5 * loss.element_size())
+    _check(lib().nep_snes_update(_ptr(m), _ptr(s), _ptr(r), C.c_void_p(ptr), stride, r.shape[0], r.shape[1], float(eta_m),
+                                 float(eta_s), _stream()), "nep_snes_update")

@@ -116,6 +116,7 @@ struct nep_system {
     SysDev d;
     Box box;
     bool built, have_forces;
+    const double* batch_boxes; const int* batch_sid;     // set by nep_trainer: concatenated structures, one box each
     bool last_driven; float last_fe[3];    // equations of motion of the last nep_md_step (its kick force is reused)
     int path;                              // NEP_PATH_THREAD or NEP_PATH_GROUP: which kernel evaluates Eq. 12-25
     float* dump_q; float* dump_fp;        // set only inside nep_compute_internals
@@ -422,14 +423,21 @@ struct FilterParams {
     Box b;
     double rcR2, rcA2;
     int capR, capA;
+    const double* boxes;        // nullable: concatenated structures (training side), [S][6] = L[3], 1/L[3] of structure sid[i]
+    const int* sid;
 };
 
 __global__ void __launch_bounds__(128) k_filter(SysDev d, int N, const __grid_constant__ FilterParams F) {
-    const Box& b = F.b;
     const int capR = F.capR;
     const int gi = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = gi < N;
     const int i = min(gi, N - 1);                // a lane without atom only takes part in the warp statistics
+    Box b = F.b;
+    if (F.boxes) {                               // every structure of a concatenated set has its own box
+        const double* bx = F.boxes + 6 * (size_t)F.sid[i];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { b.L[a] = bx[a]; b.invL[a] = bx[3 + a]; }
+    }
     const int lane = threadIdx.x & 31;
     const double4 pi = d.xs4[i];
     const int cnt = valid ? d.md_cnt[i] : 0;
@@ -926,6 +934,7 @@ FilterParams filter_params(const nep_system* s) {
     F.b = s->box;
     F.rcR2 = h.rc_radial * h.rc_radial; F.rcA2 = h.rc_angular * h.rc_angular;
     F.capR = s->capR; F.capA = s->capA;
+    F.boxes = s->batch_boxes; F.sid = s->batch_sid;
     return F;
 }
 
@@ -1169,6 +1178,7 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
     s->path = (m->thread_path_ok && n_atoms >= kThreadPathMinAtoms) ? NEP_PATH_THREAD : NEP_PATH_GROUP;
     carve(n_atoms, s->capR, s->capMD, s->max_cells, m->NA, m->h.n_types > 1 ? m->D : 0, &s->d, (char*)workspace_dev);
     s->last_driven = false; s->last_fe[0] = s->last_fe[1] = s->last_fe[2] = 0.f;
+    s->batch_boxes = nullptr; s->batch_sid = nullptr;
     s->built = false; s->have_forces = false; s->dump_q = nullptr; s->dump_fp = nullptr; s->last_stream = nullptr; s->step_graph = nullptr; s->cap_stream = nullptr; s->g_launches = 0;
     s->launches = 0; s->prof_on = false; s->prof_n = 0;
     for (int k = 0; k < NEP_PHASES; ++k) { s->prof_ms[k] = 0.0; s->prof_cnt[k] = 0; }
@@ -1470,3 +1480,5 @@ int nep_get_profile(nep_system* s, double ms[8], int64_t count[8]) {
 }
 
 }  // extern "C"
+
+#include "nep_train.cuh"

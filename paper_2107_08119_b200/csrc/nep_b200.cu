@@ -71,7 +71,7 @@ struct SysDev {                 // device pointers into the caller's workspace
 };
 
 constexpr int kMaxH = 64;           // hidden neurons k_main supports (it stages the weights in shared memory)
-constexpr int64_t kThreadPathMinAtoms = 150000;   // nep_system_create: from here on k_main (one thread per atom) is chosen
+constexpr int64_t kThreadPathMinAtoms = 12000;    // nep_system_create: from here on k_main (one thread per atom) is chosen (crossover measured at ~8-10k atoms)
 
 // sqrt(Z_a Z_b) of Eq. 19, passed to k_main by value (kernel-parameter constant bank)
 struct ZZParams {
@@ -506,6 +506,74 @@ __global__ void __launch_bounds__(128) k_filter(SysDev d, int N, const __grid_co
     }
 }
 
+// The same filter with eight lanes per atom (small systems): lane l of the group takes Verlet entries l, l + 8, ...;
+// the entries of a chunk of eight are judged at once, their record slots follow from the chunk's ballots (order of
+// the Verlet row preserved, so rows, masks and counts are bit-identical to k_filter's).  Indices are fetched two
+// chunks ahead and positions one chunk ahead: a row of 48 entries costs ~6 short rounds instead of 6 batches in series.
+__global__ void __launch_bounds__(128) k_filter_group(SysDev d, int N, const __grid_constant__ FilterParams F) {
+    const int capR = F.capR;
+    const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+    const int ia = gt >> 3, gl = threadIdx.x & 7, lane = threadIdx.x & 31, gsh = lane & 24;       // gsh: first lane of the group
+    const bool valid = ia < N;
+    const int i = valid ? ia : N - 1;
+    Box b = F.b;
+    if (F.boxes) {
+        const double* bx = F.boxes + 6 * (size_t)F.sid[i];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { b.L[a] = bx[a]; b.invL[a] = bx[3 + a]; }
+    }
+    const double4 pi = d.xs4[i];
+    const int cnt = valid ? d.md_cnt[i] : 0;
+    const int nch = (__reduce_max_sync(0xffffffffu, cnt) + 7) >> 3;       // warp-uniform trip count
+    int nA = 0, nO = 0;
+    unsigned mR[4] = {0u, 0u, 0u, 0u}, mA[4] = {0u, 0u, 0u, 0u};
+    auto entry = [&](int c) { const int s = c * 8 + gl; return s < cnt ? d.md_idx[(size_t)s * N + i] : (unsigned)i; };
+    unsigned e1 = entry(0), e2 = entry(1);
+    double4 p1 = ldg256(&d.xs4[e1 & kJMask]);
+    for (int c = 0; c < nch; ++c) {
+        const unsigned e = e1;
+        const double4 pj = p1;
+        e1 = e2; e2 = entry(c + 2);
+        p1 = ldg256(&d.xs4[e1 & kJMask]);
+        const int s = c * 8 + gl;
+        const double dx = min_image(pj.x - pi.x, b.L[0], b.invL[0]);
+        const double dy = min_image(pj.y - pi.y, b.L[1], b.invL[1]);
+        const double dz = min_image(pj.z - pi.z, b.L[2], b.invL[2]);
+        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        const bool inR = s < cnt && r2 < F.rcR2, inA = inR && r2 < F.rcA2;
+        const unsigned bR = (__ballot_sync(0xffffffffu, inR) >> gsh) & 0xffu, bA = (__ballot_sync(0xffffffffu, inA) >> gsh) & 0xffu;
+        const unsigned below = (1u << gl) - 1u, bO = bR & ~bA;
+        if (inR && nA + nO + __popc(bR & below) < capR) {
+            const int slot = inA ? nA + __popc(bA & below) : capR - 1 - (nO + __popc(bO & below));
+            const int ty = (int)__double_as_longlong(pj.w);
+            d.rec[(size_t)slot * N + i] = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(ty));
+            d.jrev[(size_t)slot * N + i] = e;
+        }
+        nA += __popc(bA); nO += __popc(bO);
+#pragma unroll
+        for (int wq = 0; wq < 4; ++wq)
+            if ((c >> 2) == wq) { mR[wq] |= bR << ((c & 3) * 8); mA[wq] |= bA << ((c & 3) * 8); }
+    }
+    const int nR = nA + nO;
+    const bool over = nR > capR || nA > F.capA;
+    if (valid && gl == 0) {
+        d.nnA[i] = over ? 0 : nA;
+        d.nnR[i] = over ? 0 : nR;
+        if (over) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
+        d.masks[2 * (size_t)i] = make_uint4(mR[0], mR[1], mR[2], mR[3]);
+        d.masks[2 * (size_t)i + 1] = make_uint4(mA[0], mA[1], mA[2], mA[3]);
+    }
+    int xR = nR, xA = nA;
+    for (int o = 16; o > 0; o >>= 1) {
+        xR = max(xR, __shfl_xor_sync(0xffffffffu, xR, o));
+        xA = max(xA, __shfl_xor_sync(0xffffffffu, xA, o));
+    }
+    if (lane == 0) {
+        if (xR > d.flags[F_MAXR]) atomicMax(&d.flags[F_MAXR], xR);
+        if (xA > d.flags[F_MAXA]) atomicMax(&d.flags[F_MAXA], xA);
+    }
+}
+
 // lists in the caller's numbering for nep_get_neighbors
 __global__ void k_export_lists(SysDev d, int N, int which, int capR, int cap_out, int* count, int* index) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -580,22 +648,29 @@ __device__ __forceinline__ bool bit_set(const uint4& m, int t) {
     return (v >> (t & 31)) & 1u;
 }
 
+// LANES = 1: one thread per atom (large systems: fewest instructions).  LANES = 8: eight lanes share an atom's
+// neighbours (small systems: the three dependent loads of ~28 neighbours become one or two rounds instead of four
+// batches in series), partial sums reduced by shuffles, lane 0 of the group finishes the atom.
+template <int LANES>
 __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
     const int N = P.N;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+    const int ia = gt / LANES, gl = gt % LANES;
+    const bool has_atom = ia < N;
+    const int i = has_atom ? ia : N - 1;
     double tU = 0.0, tK = 0.0, tJ[3] = {0.0, 0.0, 0.0}, tKt[3] = {0.0, 0.0, 0.0};
-    if (i < N) {
-        const int nR = d.nnR[i], nA = d.nnA[i];
-        float fx = 0.f, fy = 0.f, fz = 0.f;
-        float w[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        constexpr int B = 8;             // batch the three dependent loads (jrev -> masks -> p) for MLP
-        for (int k0 = 0; k0 < nR; k0 += B) {
+    float fx = 0.f, fy = 0.f, fz = 0.f;
+    float w[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    const int nR = has_atom ? d.nnR[i] : 0, nA = has_atom ? d.nnA[i] : 0;
+    {
+        constexpr int B = LANES == 1 ? 8 : 4;    // batch the three dependent loads (jrev -> masks -> p) for MLP
+        for (int k0 = 0; k0 < nR; k0 += B * LANES) {
             unsigned jr[B];
             float4 eb[B], pb[B];
             uint4 mrb[B], mab[B];
 #pragma unroll
             for (int u = 0; u < B; ++u) {
-                const int k = min(k0 + u, nR - 1);
+                const int k = min(k0 + u * LANES + gl, nR - 1);
                 const int slot = k < nA ? k : P.capR - 1 - (k - nA);
                 jr[u] = d.jrev[(size_t)slot * N + i];
                 eb[u] = d.rec[(size_t)slot * N + i];
@@ -612,7 +687,7 @@ __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
             }
 #pragma unroll
             for (int u = 0; u < B; ++u) {
-                if (k0 + u >= nR) break;
+                if (k0 + u * LANES + gl >= nR) continue;
                 const float4 e = eb[u], pj = pb[u];
                 fx += pj.x; fy += pj.y; fz += pj.z;
                 w[0] = fmaf(e.x, pj.x, w[0]); w[1] = fmaf(e.x, pj.y, w[1]); w[2] = fmaf(e.x, pj.z, w[2]);
@@ -620,6 +695,16 @@ __global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
                 w[6] = fmaf(e.z, pj.x, w[6]); w[7] = fmaf(e.z, pj.y, w[7]); w[8] = fmaf(e.z, pj.z, w[8]);
             }
         }
+    }
+    if (LANES > 1) {
+#pragma unroll
+        for (int o = 1; o < LANES; o <<= 1) {
+            fx += __shfl_xor_sync(0xffffffffu, fx, o); fy += __shfl_xor_sync(0xffffffffu, fy, o); fz += __shfl_xor_sync(0xffffffffu, fz, o);
+#pragma unroll
+            for (int c = 0; c < 9; ++c) w[c] += __shfl_xor_sync(0xffffffffu, w[c], o);
+        }
+    }
+    if (has_atom && gl == 0) {
         const float4 fs = d.Fself[i];
         fx = fs.x - fx; fy = fs.y - fy; fz = fs.z - fz;               // Eq. 4-5
         const int row = d.perm[i];
@@ -943,8 +1028,20 @@ void launch_order(nep_system* s, cudaStream_t st) {
     s->launches += 1;
 }
 
+// small systems: the gather kernels spread an atom's neighbours over eight lanes (latency, not throughput, is what
+// a 4096-atom step waits for)
+constexpr int64_t kGroupGatherMaxAtoms = 16384;
+bool group_gather(const nep_system* s) { return s->N <= kGroupGatherMaxAtoms; }
+
+void launch_assemble(nep_system* s, const AsmParams& P, cudaStream_t st) {
+    if (group_gather(s)) k_assemble<8><<<grid_for(s->N * 8, 128), 128, 0, st>>>(s->d, P);
+    else k_assemble<1><<<grid_for(s->N, 128), 128, 0, st>>>(s->d, P);
+    s->launches += 1;
+}
+
 void launch_filter(nep_system* s, cudaStream_t st) {
-    k_filter<<<grid_for(s->N, 128), 128, 0, st>>>(s->d, (int)s->N, filter_params(s));
+    if (group_gather(s)) k_filter_group<<<grid_for(s->N * 8, 128), 128, 0, st>>>(s->d, (int)s->N, filter_params(s));
+    else k_filter<<<grid_for(s->N, 128), 128, 0, st>>>(s->d, (int)s->N, filter_params(s));
     s->launches += 1;
     if (s->path == NEP_PATH_THREAD) launch_order(s, st);         // k_gen takes the atoms in sorted order as they are
 }
@@ -993,8 +1090,8 @@ void launch_step(nep_system* s, const AsmParams& P, double dt_fs, double hs2, cu
     phase(s, PH_MAIN, st);
     launch_main(s, st);
     phase(s, PH_ASSEMBLE, st);
-    k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
-    s->launches += 2;
+    launch_assemble(s, P, st);
+    s->launches += 1;
 }
 
 // The step as a CUDA graph, captured on a library-owned stream (the caller's may be the legacy default
@@ -1275,9 +1372,9 @@ int nep_compute(nep_system* s, const double* pos_dev, const double* vel_dev, flo
     P.vel_in = vel_dev; P.energy = energy_dev; P.force = force_dev; P.virial = virial_dev;
     P.heat = vel_dev ? heat_dev : nullptr;
     phase(s, PH_ASSEMBLE, st);
-    k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
+    launch_assemble(s, P, st);
     phase(s, -1, st);
-    s->launches += 2;
+    s->launches += 1;
     NEP_CUDA_OK(cudaGetLastError());
     s->have_forces = false;
     return NEP_OK;
@@ -1351,8 +1448,7 @@ int nep_md_step_driven(nep_system* s, double* pos_dev, double* vel_dev, const do
         launch_main(s, st);
         P.md = 2;
         phase(s, PH_ASSEMBLE, st);
-        k_assemble<<<grid_for(N, 128), 128, 0, st>>>(s->d, P);
-        s->launches += 1;
+        launch_assemble(s, P, st);
     }
     P.md = 1;
     if (s->prof_on || n_steps < 2) {

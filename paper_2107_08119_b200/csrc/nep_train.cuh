@@ -308,8 +308,7 @@ void train_eval_member(nep_trainer* t, const double* z_dev, cudaStream_t st) {
     P.N = (int)t->N; P.capR = s->capR; P.capMD = s->capMD; P.md = 0;
     fill_masses(&P, m, nullptr);
     P.energy = t->U; P.force = t->F; P.virial = t->W;
-    k_assemble<<<grid_for(t->N, 128), 128, 0, st>>>(s->d, P);
-    s->launches += 1;
+    launch_assemble(s, P, st);
 }
 }  // namespace
 

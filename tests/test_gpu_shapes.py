@@ -45,11 +45,14 @@ def test_group_path_on_baseline_configs(oracle, which):
 
 def test_auto_path_switches_with_size(oracle):
     """nep_system_create picks eight lanes per atom for small systems and one thread per atom for large ones;
-    sizes on either side of the switch give the same results as the oracle (C4-32768 above, C4-262144 here)."""
+    sizes on either side of the switch (12000 atoms) give the same results as the oracle (C2 with 8000 atoms in
+    test_group_path_on_baseline_configs, C4-262144 here)."""
     torch, api = _gpu()
-    w_small = inputs.config4(32768)
-    _, s_small, _, _ = api.from_workload(w_small, 64, 32, 1.0)
+    w_small = inputs.config2()
+    _, s_small, _, _ = api.from_workload(w_small, 80, 40, 1.0)
     assert s_small.path == GROUP
+    _, s_mid, _, _ = api.from_workload(inputs.config4(32768), 64, 32, 1.0)
+    assert s_mid.path == THREAD
     w_big = inputs.config4(262144)
     system, out = _run(oracle, w_big, 64, 32, 1.0, None, ocap=(64, 32))
     assert system.path == THREAD

@@ -338,20 +338,36 @@ __device__ __forceinline__ void ph_build_md(const SysDev& d, int N, const Box& b
     }
 }
 
-// reverse slot: position of i in j's (ascending) row, by binary search
+// reverse slot: position of i in j's (ascending) row, by binary search -- eight searches at a time, so that the
+// dependent probes of one search overlap those of seven others (the probes are L2 round trips)
 __device__ __forceinline__ void ph_rev(const SysDev& d, int N, int tid, int nth) {
+    constexpr int B = 8;
     for (int i = tid; i < N; i += nth) {
         const int cnt = d.md_cnt[i];
-        for (int s = 0; s < cnt; ++s) {
-            const int j = (int)(d.md_idx[(size_t)s * N + i] & kJMask);
-            int lo = 0, hi = d.md_cnt[j] - 1, found = 0;
-            while (lo <= hi) {
-                const int mid = (lo + hi) >> 1;
-                const int v = (int)(d.md_idx[(size_t)mid * N + j] & kJMask);
-                if (v == i) { found = mid; break; }
-                if (v < i) lo = mid + 1; else hi = mid - 1;
+        for (int s0 = 0; s0 < cnt; s0 += B) {
+            int j[B], lo[B], hi[B];
+#pragma unroll
+            for (int u = 0; u < B; ++u) {
+                j[u] = (int)(d.md_idx[(size_t)min(s0 + u, cnt - 1) * N + i] & kJMask);
+                lo[u] = 0;
             }
-            d.md_idx[(size_t)s * N + i] = (unsigned)j | ((unsigned)found << 24);
+#pragma unroll
+            for (int u = 0; u < B; ++u) hi[u] = d.md_cnt[j[u]] - 1;
+            // rows hold at most kMaxCapMD < 128 entries: seven halvings always suffice; a finished search keeps lo == hi
+#pragma unroll 1
+            for (int it = 0; it < 7; ++it) {
+                int v[B];
+#pragma unroll
+                for (int u = 0; u < B; ++u) v[u] = (int)(d.md_idx[(size_t)((lo[u] + hi[u]) >> 1) * N + j[u]] & kJMask);
+#pragma unroll
+                for (int u = 0; u < B; ++u) {
+                    const int mid = (lo[u] + hi[u]) >> 1;
+                    if (v[u] < i) lo[u] = min(mid + 1, hi[u]); else hi[u] = mid;       // first entry >= i
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < B; ++u)
+                if (s0 + u < cnt) d.md_idx[(size_t)(s0 + u) * N + i] = (unsigned)j[u] | ((unsigned)lo[u] << 24);
         }
     }
 }

@@ -443,7 +443,8 @@ struct FilterParams {
     const int* sid;
 };
 
-__global__ void __launch_bounds__(128) k_filter(SysDev d, int N, const __grid_constant__ FilterParams F) {
+// 4 blocks per SM (128 registers; 5 / 6 blocks per SM spill: 0.62 -> 0.71 / 0.81 ms at 1M atoms)
+__global__ void __launch_bounds__(128, 4) k_filter(SysDev d, int N, const __grid_constant__ FilterParams F) {
     const int capR = F.capR;
     const int gi = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = gi < N;
@@ -668,7 +669,8 @@ __device__ __forceinline__ bool bit_set(const uint4& m, int t) {
 // neighbours (small systems: the three dependent loads of ~28 neighbours become one or two rounds instead of four
 // batches in series), partial sums reduced by shuffles, lane 0 of the group finishes the atom.
 template <int LANES>
-__global__ void __launch_bounds__(128) k_assemble(SysDev d, AsmParams P) {
+// 4 blocks per SM = at most 128 registers (measured at 1M atoms: 3 / 4 / 5 / 6 blocks per SM -> 0.45 / 0.39 / 0.47 / 0.57 ms)
+__global__ void __launch_bounds__(128, 4) k_assemble(SysDev d, AsmParams P) {
     const int N = P.N;
     const int gt = blockIdx.x * blockDim.x + threadIdx.x;
     const int ia = gt / LANES, gl = gt % LANES;

@@ -112,7 +112,7 @@ void nep_system_destroy(nep_system*);
 
 /* Which kernel evaluates Eq. 12-25 (the descriptor, the network and the partial forces):
  *   NEP_PATH_THREAD  one thread per atom (k_main): every per-atom quantity in registers; instantiated for
- *                    n_max_radial == n_max_angular in {7, 8}, l_max == 4, n_neurons <= 64 -- the BASELINE.json
+ *                    n_max_radial / n_max_angular = 7/7, 8/8 or 12/6, l_max == 4, n_neurons <= 64 -- the BASELINE.json
  *                    shapes (D = 40 / 45); the faster form from ~1e4 atoms (nep_system_create switches at 12000)
  *   NEP_PATH_GROUP   eight lanes per atom (k_gen): any shape nep_create accepts, Table I's 80-50-1, 65-40-1 and
  *                    41-40-1 models included; the form for small systems

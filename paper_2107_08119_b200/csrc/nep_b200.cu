@@ -978,7 +978,8 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
 }
 
 bool main_supported(const nep_model* m) {
-    if (!((m->NR == 8 && m->NA == 8) || (m->NR == 9 && m->NA == 9)) || m->H > kMaxH || m->h.l_max != 4) return false;
+    // instantiated shapes: the BASELINE.json models (8/8, 9/9 radial functions) and Table I's PbTe model (13/7)
+    if (!((m->NR == 8 && m->NA == 8) || (m->NR == 9 && m->NA == 9) || (m->NR == 13 && m->NA == 7)) || m->H > kMaxH || m->h.l_max != 4) return false;
     // the staged weights must fit beside the per-warp record rows (H = 64 with D = 45 and Eq. 19 does not)
     const size_t smem = m->h.n_types > 1 ? main_smem_bytes<8, true>(m->params_floats) : main_smem_bytes<8, false>(m->params_floats);
     return smem <= (size_t)kMainSmemLimit;
@@ -1029,6 +1030,7 @@ void launch_main(nep_system* s, cudaStream_t st) {
     if (s->path == NEP_PATH_GROUP) { launch_gen(s, st); return; }
     if (m->NR == 8 && m->NA == 8) { if (multi) launch_main_t<8, 8, true>(s, st); else launch_main_t<8, 8, false>(s, st); }
     else if (m->NR == 9 && m->NA == 9) { if (multi) launch_main_t<9, 9, true>(s, st); else launch_main_t<9, 9, false>(s, st); }
+    else if (m->NR == 13 && m->NA == 7) { if (multi) launch_main_t<13, 7, true>(s, st); else launch_main_t<13, 7, false>(s, st); }
 }
 
 FilterParams filter_params(const nep_system* s) {

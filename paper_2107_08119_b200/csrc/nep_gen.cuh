@@ -306,9 +306,19 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
             for (int mu = gl; mu < H; mu += kGenLanes) {
                 const TD* w = wsm + mu * Dps;
                 TD a0 = -b1s[mu], a1 = (TD)0, a2 = (TD)0, a3 = (TD)0;
+                if (F64) {
 #pragma unroll 4
-                for (int v = 0; v < Dp; v += 4) {                       // padded columns of w1 and the padded tail of q are zero
-                    a0 += w[v] * sm.q[v]; a1 += w[v + 1] * sm.q[v + 1]; a2 += w[v + 2] * sm.q[v + 2]; a3 += w[v + 3] * sm.q[v + 3];
+                    for (int v = 0; v < Dp; v += 4) {                   // padded columns of w1 and the padded tail of q are zero
+                        a0 += w[v] * sm.q[v]; a1 += w[v + 1] * sm.q[v + 1]; a2 += w[v + 2] * sm.q[v + 2]; a3 += w[v + 3] * sm.q[v + 3];
+                    }
+                } else {                                                // one LDS.128 of weights and one of q per four FMAs
+                    const float4* w4 = reinterpret_cast<const float4*>(w);
+                    const float4* q4 = reinterpret_cast<const float4*>(&sm.q[0]);
+#pragma unroll 5
+                    for (int v = 0; v < Dp / 4; ++v) {
+                        const float4 ww = w4[v], qq = q4[v];
+                        a0 += (TD)ww.x * (TD)qq.x; a1 += (TD)ww.y * (TD)qq.y; a2 += (TD)ww.z * (TD)qq.z; a3 += (TD)ww.w * (TD)qq.w;
+                    }
                 }
                 const TD a = (a0 + a1) + (a2 + a3);
                 const TD w2 = w2s[mu];
@@ -325,11 +335,20 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
             }
             for (int v4 = gl; v4 < Dp / 4; v4 += kGenLanes) {              // four descriptor components per lane
                 TD f0 = (TD)0, f1 = (TD)0, f2 = (TD)0, f3 = (TD)0;
+                if (F64) {
 #pragma unroll 4
-                for (int mu = 0; mu < H; ++mu) {
-                    const TD gm = sm.hid[mu];
-                    const TD* w = wsm + mu * Dps + 4 * v4;
-                    f0 += gm * w[0]; f1 += gm * w[1]; f2 += gm * w[2]; f3 += gm * w[3];
+                    for (int mu = 0; mu < H; ++mu) {
+                        const TD gm = sm.hid[mu];
+                        const TD* w = wsm + mu * Dps + 4 * v4;
+                        f0 += gm * w[0]; f1 += gm * w[1]; f2 += gm * w[2]; f3 += gm * w[3];
+                    }
+                } else {
+#pragma unroll 5
+                    for (int mu = 0; mu < H; ++mu) {
+                        const TD gm = sm.hid[mu];
+                        const float4 ww = *reinterpret_cast<const float4*>(wsm + mu * Dps + 4 * v4);
+                        f0 += gm * (TD)ww.x; f1 += gm * (TD)ww.y; f2 += gm * (TD)ww.z; f3 += gm * (TD)ww.w;
+                    }
                 }
                 sm.Fp[4 * v4] = (float)f0; sm.Fp[4 * v4 + 1] = (float)f1; sm.Fp[4 * v4 + 2] = (float)f2; sm.Fp[4 * v4 + 3] = (float)f3;
             }
@@ -400,18 +419,16 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
 #pragma unroll
                 for (int m = 0; m < kNumLM; ++m) acc2[m] = pack2(0.f, 0.f);
 #pragma unroll
-                for (int n = 0; n < NMAX; ++n) {
-                    if (n < NA) {                                        // uniform
-                        const float4* An = reinterpret_cast<const float4*>(A + n * kNumLM);
-                        const f32x2 dgs = pack2(dg[n], gs[n]);
+                for (int n = 0; n < NMAX; ++n) {                         // rows n >= NA of A are zero: no branch (a uniform
+                    const float4* An = reinterpret_cast<const float4*>(A + n * kNumLM);      // `if (n < NA)` cost a MOV per FFMA2)
+                    const f32x2 dgs = pack2(dg[n], gs[n]);
 #pragma unroll
-                        for (int m4 = 0; m4 < kNumLM / 4; ++m4) {
-                            const float4 a = An[m4];
-                            acc2[4 * m4] = ffma2(pack2(a.x, a.x), dgs, acc2[4 * m4]);
-                            acc2[4 * m4 + 1] = ffma2(pack2(a.y, a.y), dgs, acc2[4 * m4 + 1]);
-                            acc2[4 * m4 + 2] = ffma2(pack2(a.z, a.z), dgs, acc2[4 * m4 + 2]);
-                            acc2[4 * m4 + 3] = ffma2(pack2(a.w, a.w), dgs, acc2[4 * m4 + 3]);
-                        }
+                    for (int m4 = 0; m4 < kNumLM / 4; ++m4) {
+                        const float4 a = An[m4];
+                        acc2[4 * m4] = ffma2(pack2(a.x, a.x), dgs, acc2[4 * m4]);
+                        acc2[4 * m4 + 1] = ffma2(pack2(a.y, a.y), dgs, acc2[4 * m4 + 1]);
+                        acc2[4 * m4 + 2] = ffma2(pack2(a.z, a.z), dgs, acc2[4 * m4 + 2]);
+                        acc2[4 * m4 + 3] = ffma2(pack2(a.w, a.w), dgs, acc2[4 * m4 + 3]);
                     }
                 }
                 float Sq[kNumLM], St[kNumLM];

@@ -225,16 +225,17 @@ int  nep_measure_fp32_patterns(double tflops[3], void* cuda_stream);
  * W(n) of Eq. 30 / 32 are per atom ("eV/atom for energy and virial"); the six virial components are
  * xx, yy, zz, xy, yz, zx; the rank utilities u_k of Eq. 36-37, which the paper defers to its Ref. 44, are
  * max(0, ln(N_pop/2+1) - ln k) normalised to sum 1, minus 1/N_pop (k = 1 the smallest loss, ties by member index).
- * The structures do not move, so lists and records are built once in nep_trainer_create; single-species models only.
- *   first [S+1], boxes [S][3]: HOST.  pos_dev [3][N] fp64 (N = first[S]).
+ * The structures do not move, so lists and records are built once in nep_trainer_create.
+ *   atomic_number [n_types] HOST (Eq. 19; NULL when n_types == 1).  first [S+1], boxes [S][3]: HOST.
+ *   pos_dev [3][N] fp64 (N = first[S]); type_dev [N] int32 device, 0..n_types-1 (NULL: all zero; copied).
  *   e_tar_dev [S] (per atom), f_tar_dev [3][N], v_tar_dev [S][6] (per atom): fp32 DEVICE targets, caller-owned, must
  *   outlive the trainer; all three nullable if only nep_trainer_predict is used. */
 typedef struct nep_trainer nep_trainer;
 size_t nep_trainer_workspace_bytes(const nep_hyper_ex*, int n_structures, int64_t n_atoms, int cap_radial, int cap_angular);
-int  nep_trainer_create(const nep_hyper_ex*, int n_structures, const int64_t* first, const double* boxes,
-                        const double* pos_dev, const float* e_tar_dev, const float* f_tar_dev, const float* v_tar_dev,
-                        int cap_radial, int cap_angular, void* workspace_dev, size_t workspace_bytes, void* cuda_stream,
-                        nep_trainer** out);
+int  nep_trainer_create(const nep_hyper_ex*, const int* atomic_number, int n_structures, const int64_t* first,
+                        const double* boxes, const double* pos_dev, const int* type_dev, const float* e_tar_dev,
+                        const float* f_tar_dev, const float* v_tar_dev, int cap_radial, int cap_angular,
+                        void* workspace_dev, size_t workspace_bytes, void* cuda_stream, nep_trainer** out);
 void nep_trainer_destroy(nep_trainer*);
 int  nep_trainer_num_params(const nep_trainer*);
 int  nep_trainer_status(nep_trainer*);      /* as nep_status (capacity overflow) */

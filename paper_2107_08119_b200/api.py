@@ -72,8 +72,8 @@ def lib():
         L.nep_profile.argtypes = [C.c_void_p, C.c_int]
         L.nep_trainer_workspace_bytes.restype = C.c_size_t
         L.nep_trainer_workspace_bytes.argtypes = [C.POINTER(HyperEx), C.c_int, C.c_int64, C.c_int, C.c_int]
-        L.nep_trainer_create.argtypes = [C.POINTER(HyperEx), C.c_int] + [C.c_void_p] * 6 + [C.c_int, C.c_int, C.c_void_p, C.c_size_t,
-                                          C.c_void_p, C.POINTER(C.c_void_p)]
+        L.nep_trainer_create.argtypes = [C.POINTER(HyperEx), C.c_void_p, C.c_int] + [C.c_void_p] * 7 + [C.c_int, C.c_int, C.c_void_p,
+                                          C.c_size_t, C.c_void_p, C.POINTER(C.c_void_p)]
         L.nep_trainer_destroy.argtypes = [C.c_void_p]; L.nep_trainer_destroy.restype = None
         L.nep_trainer_num_params.argtypes = [C.c_void_p]; L.nep_trainer_status.argtypes = [C.c_void_p]
         L.nep_trainer_losses.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -274,22 +274,25 @@ class Trainer:
     """nep_trainer_*: the loss of Eq. 29-34 for a population over concatenated structures, and SNES (Eq. 35-39)."""
 
     def __init__(self, rc_radial, rc_angular, n_max_radial, n_max_angular, l_max, hidden_layers, first, boxes, pos,
-                 e_tar=None, f_tar=None, v_tar=None, angular_kind=0, cap_radial=64, cap_angular=32):
+                 e_tar=None, f_tar=None, v_tar=None, angular_kind=0, cap_radial=64, cap_angular=32, types=None,
+                 atomic_numbers=(14,)):
         w = list(hidden_layers)
-        base = Hyper(rc_radial, rc_angular, n_max_radial, n_max_angular, l_max, w[0], 1)
+        zs = np.ascontiguousarray(atomic_numbers, dtype=np.int32)
+        base = Hyper(rc_radial, rc_angular, n_max_radial, n_max_angular, l_max, w[0], len(zs))
         self.hx = HyperEx(base, len(w), w[1] if len(w) > 1 else 0, w[2] if len(w) > 2 else 0, angular_kind)
         first = np.ascontiguousarray(first, dtype=np.int64); boxes = np.ascontiguousarray(boxes, dtype=np.float64)
         self.n_structures, self.n = len(first) - 1, int(first[-1])
         assert pos.is_cuda and pos.dtype == torch.float64 and pos.is_contiguous() and pos.shape == (3, self.n)
-        self._keep = (pos, e_tar, f_tar, v_tar)              # the library keeps these pointers
+        self._keep = (pos, e_tar, f_tar, v_tar, types)       # the library keeps the target pointers
         nbytes = lib().nep_trainer_workspace_bytes(C.byref(self.hx), self.n_structures, self.n, cap_radial, cap_angular)
         if nbytes == 0:
             raise NepError(-1, "nep_trainer_workspace_bytes")
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=pos.device)
         off = (-self.workspace.data_ptr()) % 256
         self._h = C.c_void_p()
-        _check(lib().nep_trainer_create(C.byref(self.hx), self.n_structures, first.ctypes.data_as(C.c_void_p),
-                                        boxes.ctypes.data_as(C.c_void_p), _ptr(pos), _ptr(e_tar), _ptr(f_tar), _ptr(v_tar),
+        _check(lib().nep_trainer_create(C.byref(self.hx), zs.ctypes.data_as(C.c_void_p), self.n_structures,
+                                        first.ctypes.data_as(C.c_void_p), boxes.ctypes.data_as(C.c_void_p), _ptr(pos), _ptr(types),
+                                        _ptr(e_tar), _ptr(f_tar), _ptr(v_tar),
                                         cap_radial, cap_angular, C.c_void_p(self.workspace.data_ptr() + off), nbytes, _stream(),
                                         C.byref(self._h)), "nep_trainer_create")
         self.num_params = lib().nep_trainer_num_params(self._h)

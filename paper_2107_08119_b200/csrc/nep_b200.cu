@@ -997,6 +997,7 @@ void launch_gen_t(nep_system* s, cudaStream_t st) {
     P.N = (int)s->N; P.capR = s->capR; P.box = s->box;
     P.params = m->params_dev; P.params64 = m->params64_dev;
     P.q_out = s->dump_q; P.fp_out = s->dump_fp;
+    P.boxes = s->batch_boxes; P.sid = s->batch_sid;
     P.kind = m->kind; P.nlayers = m->nlayers; P.off_out = m->off_out; P.blob_elems = m->blob_elems;
     for (int k = 0; k < 3; ++k) { P.lw[k] = m->lw[k]; P.lin_p[k] = m->lin_p[k]; P.off_w[k] = m->off_w[k]; P.off_b[k] = m->off_b[k]; }
     P.blob = m->blob_dev; P.blob64 = m->blob64_dev;

@@ -45,6 +45,8 @@ struct GenParams {
     int blob_elems;
     const float* blob;                       // W1[H1][in_p] | b1 | W2[H2][H1_p] | b2 | ... | w_out | b_out, sections 4-aligned
     const double* blob64;
+    const double* boxes;                     // nullable: concatenated structures (training side), [S][6] = L[3], 1/L[3]
+    const int* sid;                          //   structure of (sorted) atom i
     float* q_out;                            // nullable parity hooks, [D][N] caller order
     float* fp_out;
 };
@@ -131,7 +133,15 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
         const int chA = (__reduce_max_sync(0xffffffffu, nA) + kGenLanes - 1) / kGenLanes;
         const int ti = d.type_s[i];
         double4 pi = make_double4(0.0, 0.0, 0.0, 0.0);
-        if (F64) pi = d.xs4[i];
+        double bL[3] = {P.box.L[0], P.box.L[1], P.box.L[2]}, bI[3] = {P.box.invL[0], P.box.invL[1], P.box.invL[2]};
+        if (F64) {
+            pi = d.xs4[i];
+            if (P.boxes) {                                                // every structure of a concatenated set has its own box
+                const double* bx = P.boxes + 6 * (size_t)P.sid[i];
+#pragma unroll
+                for (int a = 0; a < 3; ++a) { bL[a] = bx[a]; bI[a] = bx[3 + a]; }
+            }
+        }
 
         // neighbour k of the atom in the descriptor precision: unit vector, distance, Eq. 19 weight
         auto nbr = [&](int k, TD& x, TD& y, TD& z, TD& r, TD& om) {
@@ -139,9 +149,9 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
             if (F64) {
                 const int j = (int)(d.jrev[(size_t)slot * N + i] & kJMask);
                 const double4 pj = d.xs4[j];
-                const double dx = min_image(pj.x - pi.x, P.box.L[0], P.box.invL[0]);
-                const double dy = min_image(pj.y - pi.y, P.box.L[1], P.box.invL[1]);
-                const double dz = min_image(pj.z - pi.z, P.box.L[2], P.box.invL[2]);
+                const double dx = min_image(pj.x - pi.x, bL[0], bI[0]);
+                const double dy = min_image(pj.y - pi.y, bL[1], bI[1]);
+                const double dz = min_image(pj.z - pi.z, bL[2], bI[2]);
                 const double rr = sqrt(dx * dx + dy * dy + dz * dz), ri = 1.0 / rr;
                 x = (TD)(dx * ri); y = (TD)(dy * ri); z = (TD)(dz * ri); r = (TD)rr;
                 om = (TD)P.zz64[ti * kMaxTypes + ((int)__double_as_longlong(pj.w) & (kMaxTypes - 1))];

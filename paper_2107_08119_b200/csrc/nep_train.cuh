@@ -5,7 +5,7 @@
 // The structures are static, so the neighbour lists and the per-step records are built ONCE (nep_trainer_create);
 // a population member then costs: stage its weights, k_gen (descriptor + network + partial forces over all atoms of
 // all structures), k_assemble (F, W), one reduction per structure.  Readings Q23-Q25: energy and virial per
-// atom, the six components xx yy zz xy yz zx, the standard NES rank utilities.  Single-species models only.
+// atom, the six components xx yy zz xy yz zx, the standard NES rank utilities.  Multi-species sets (Eq. 19): k_gen<double>.
 #pragma once
 
 struct nep_trainer {
@@ -16,7 +16,7 @@ struct nep_trainer {
     int* sid;                   // [N] structure of atom i
     int* first;                 // [S + 1]
     double* boxes;              // [S][6]: L[3], 1/L[3]
-    int* type_zero;             // [N]
+    int* types;                 // [N] (a copy of the caller's, or zeros)
     int* stage_map;             // [stage_n] index into z of every staged weight (-1: padding)
     float *U, *F, *W;           // [N], [3][N], [9][N] outputs of the member being evaluated
     double* sse;                // [3] squared-error sums of the member being evaluated
@@ -26,17 +26,20 @@ struct nep_trainer {
 namespace {
 
 // Verlet list of a concatenated set: thread i scans the atoms of its own structure (small: O(100) atoms), ascending j
-__global__ void k_build_batch(SysDev d, int N, const double* __restrict__ pos, const int* __restrict__ sid,
-                              const int* __restrict__ first, const double* __restrict__ boxes, double rc2, int capMD) {
+__global__ void k_build_batch(SysDev d, int N, const double* __restrict__ pos, const int* __restrict__ type, int n_types,
+                              const int* __restrict__ sid, const int* __restrict__ first, const double* __restrict__ boxes,
+                              double rc2, int capMD) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int n = sid[i];
     const double* bx = boxes + 6 * (size_t)n;
     const double xi = pos[i], yi = pos[N + i], zi = pos[2 * (size_t)N + i];
-    d.perm[i] = i; d.type_s[i] = 0;
+    int ty = type[i];
+    if (ty < 0 || ty >= n_types) { atomicOr(&d.flags[F_STATUS], ST_BADTYPE); ty = 0; }
+    d.perm[i] = i; d.type_s[i] = ty;
     d.xs[i] = xi; d.xs[N + i] = yi; d.xs[2 * (size_t)N + i] = zi;
     d.xref[i] = xi; d.xref[N + i] = yi; d.xref[2 * (size_t)N + i] = zi;
-    d.xs4[i] = make_double4(xi, yi, zi, __longlong_as_double(0ll));
+    d.xs4[i] = make_double4(xi, yi, zi, __longlong_as_double((long long)ty));
     int cnt = 0;
     for (int j = first[n]; j < first[n + 1]; ++j) {
         if (j == i) continue;
@@ -53,10 +56,11 @@ __global__ void k_build_batch(SysDev d, int N, const double* __restrict__ pos, c
     atomicMax(&d.flags[F_MAXMD], cnt);
 }
 
-// z (fp64, Eq. 26 order or the deep-network order) -> the staged fp32 layout the kernels read
-__global__ void k_stage_params(const double* __restrict__ z, const int* __restrict__ map, float* __restrict__ dst, int n) {
+// z (fp64, Eq. 26 order or the deep-network order) -> the staged layout the kernels read (fp32, or fp64 for Eq. 19)
+template <typename T>
+__global__ void k_stage_params(const double* __restrict__ z, const int* __restrict__ map, T* __restrict__ dst, int n) {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e < n) dst[e] = map[e] >= 0 ? (float)z[map[e]] : 0.f;
+    if (e < n) dst[e] = map[e] >= 0 ? (T)z[map[e]] : (T)0;
 }
 
 // one block per structure: per-atom energy and virial of the structure, squared errors of Eq. 30-32
@@ -165,14 +169,15 @@ TrainLayout train_layout(size_t sys_bytes, int S, int64_t N, int stage_n) {
     return L;
 }
 
-int train_stage_n(const nep_model* m) { return m->nlayers > 1 ? m->blob_elems : m->params_floats; }
+// elements of the staged weight buffer: the padded blob (deep), the raw Eq. 26 vector (fp64 path) or the padded fp32 layout
+int train_stage_n(const nep_model* m) { return m->nlayers > 1 ? m->blob_elems : (m->h.n_types > 1 ? m->npar : m->params_floats); }
 
 }  // namespace
 
 extern "C" {
 
 size_t nep_trainer_workspace_bytes(const nep_hyper_ex* hx, int n_structures, int64_t n_atoms, int cap_radial, int cap_angular) {
-    if (!hx || n_structures < 1 || n_atoms < 1 || hx->base.n_types != 1) return 0;
+    if (!hx || n_structures < 1 || n_atoms < 1 || hx->base.n_types < 1 || hx->base.n_types > kMaxTypes) return 0;
     // the system part is sized by a model of this shape; only NA, D and n_types enter carve()
     nep_model tmp;
     tmp.h = hx->base;
@@ -185,12 +190,14 @@ size_t nep_trainer_workspace_bytes(const nep_hyper_ex* hx, int n_structures, int
     return train_layout(sys, n_structures, n_atoms, stage_max).total;
 }
 
-int nep_trainer_create(const nep_hyper_ex* hx, int n_structures, const int64_t* first, const double* boxes, const double* pos_dev,
-                       const float* e_tar_dev, const float* f_tar_dev, const float* v_tar_dev, int cap_radial, int cap_angular,
-                       void* workspace_dev, size_t workspace_bytes, void* cuda_stream, nep_trainer** out) {
+int nep_trainer_create(const nep_hyper_ex* hx, const int* atomic_number, int n_structures, const int64_t* first, const double* boxes,
+                       const double* pos_dev, const int* type_dev, const float* e_tar_dev, const float* f_tar_dev,
+                       const float* v_tar_dev, int cap_radial, int cap_angular, void* workspace_dev, size_t workspace_bytes,
+                       void* cuda_stream, nep_trainer** out) {
     if (!out) return NEP_EINVAL;
     *out = nullptr;
-    if (!hx || !first || !boxes || !pos_dev || !workspace_dev || n_structures < 1 || hx->base.n_types != 1) return NEP_EINVAL;
+    if (!hx || !first || !boxes || !pos_dev || !workspace_dev || n_structures < 1) return NEP_EINVAL;
+    if (hx->base.n_types > 1 && (!atomic_number || !type_dev)) return NEP_EINVAL;
     const int S = n_structures;
     const int64_t N = first[S];
     if (first[0] != 0 || N < 1) return NEP_EINVAL;
@@ -216,7 +223,7 @@ int nep_trainer_create(const nep_hyper_ex* hx, int n_structures, const int64_t* 
         npar += in + 1;
     }
     double* zeros = new double[(size_t)(npar > 0 ? npar : 1)]();
-    int rc = nep_create_ex(hx, nullptr, zeros, (size_t)npar, &t->model);
+    int rc = nep_create_ex(hx, atomic_number, zeros, (size_t)npar, &t->model);
     delete[] zeros;
     if (rc != NEP_OK) { delete t; return rc; }
     nep_model* m = t->model;
@@ -225,7 +232,7 @@ int nep_trainer_create(const nep_hyper_ex* hx, int n_structures, const int64_t* 
     const TrainLayout Lay = train_layout(sys_bytes, S, N, t->stage_n);
     char* base = (char*)workspace_dev;
     t->sid = (int*)(base + Lay.sid); t->first = (int*)(base + Lay.first); t->boxes = (double*)(base + Lay.boxes);
-    t->type_zero = (int*)(base + Lay.tz); t->stage_map = (int*)(base + Lay.map);
+    t->types = (int*)(base + Lay.tz); t->stage_map = (int*)(base + Lay.map);
     t->U = (float*)(base + Lay.U); t->F = (float*)(base + Lay.F); t->W = (float*)(base + Lay.W); t->sse = (double*)(base + Lay.sse);
     t->e_tar = e_tar_dev; t->f_tar = f_tar_dev; t->v_tar = v_tar_dev;
     // host tables -> device
@@ -237,7 +244,9 @@ int nep_trainer_create(const nep_hyper_ex* hx, int n_structures, const int64_t* 
     for (int n = 0; n <= S; ++n) h_first[n] = (int)first[n];
     int* h_map = new int[(size_t)t->stage_n];
     for (int e = 0; e < t->stage_n; ++e) h_map[e] = -1;
-    if (m->nlayers == 1) {
+    if (m->nlayers == 1 && m->h.n_types > 1) {
+        for (int e = 0; e < t->stage_n; ++e) h_map[e] = e;                 // k_gen<double> reads the Eq. 26 vector as it is
+    } else if (m->nlayers == 1) {
         const int H = m->H, D = m->D, Dp = (D + 3) & ~3;
         for (int mu = 0; mu < H; ++mu) for (int v = 0; v < D; ++v) h_map[mu * Dp + v] = mu * D + v;
         for (int k = 0; k < 2 * H + 1; ++k) h_map[H * Dp + k] = H * D + k;
@@ -257,10 +266,11 @@ int nep_trainer_create(const nep_hyper_ex* hx, int n_structures, const int64_t* 
     if (e == cudaSuccess) e = cudaMemcpyAsync(t->first, h_first, ((size_t)S + 1) * 4, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(t->boxes, h_box, (size_t)S * 48, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(t->stage_map, h_map, (size_t)t->stage_n * 4, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && type_dev) e = cudaMemcpyAsync(t->types, type_dev, (size_t)N * 4, cudaMemcpyDeviceToDevice, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     delete[] h_sid; delete[] h_first; delete[] h_box; delete[] h_map;
     if (e != cudaSuccess) { set_cuda_error(e, "nep_trainer_create"); nep_destroy(t->model); delete t; return NEP_ECUDA; }
-    rc = nep_system_create(m, N, t->type_zero, cap_radial, cap_angular, 0.0, workspace_dev, sys_bytes, &t->sys);
+    rc = nep_system_create(m, N, t->types, cap_radial, cap_angular, 0.0, workspace_dev, sys_bytes, &t->sys);
     if (rc != NEP_OK) { nep_destroy(t->model); delete t; return rc; }
     nep_system* s = t->sys;
     s->path = NEP_PATH_GROUP;
@@ -271,7 +281,7 @@ int nep_trainer_create(const nep_hyper_ex* hx, int n_structures, const int64_t* 
     // lists and records once: the structures do not move
     const int Ni = (int)N;
     const double rc2 = hx->base.rc_radial * hx->base.rc_radial;
-    k_build_batch<<<grid_for(N, 128), 128, 0, st>>>(s->d, Ni, pos_dev, t->sid, t->first, t->boxes, rc2, s->capMD);
+    k_build_batch<<<grid_for(N, 128), 128, 0, st>>>(s->d, Ni, pos_dev, t->types, m->h.n_types, t->sid, t->first, t->boxes, rc2, s->capMD);
     k_rev<<<grid_for(N, 128), 128, 0, st>>>(s->d, Ni, 0);
     k_build_done<<<1, 1, 0, st>>>(s->d, 0);
     s->launches += 3;
@@ -299,8 +309,10 @@ namespace {
 // one member: stage its weights, evaluate all atoms of all structures, assemble F and W
 void train_eval_member(nep_trainer* t, const double* z_dev, cudaStream_t st) {
     nep_model* m = t->model; nep_system* s = t->sys;
-    float* dst = m->nlayers > 1 ? m->blob_dev : m->params_dev;
-    k_stage_params<<<grid_for(t->stage_n, 256), 256, 0, st>>>(z_dev, t->stage_map, dst, t->stage_n);
+    if (m->h.n_types > 1)
+        k_stage_params<double><<<grid_for(t->stage_n, 256), 256, 0, st>>>(z_dev, t->stage_map, m->nlayers > 1 ? m->blob64_dev : m->params64_dev, t->stage_n);
+    else
+        k_stage_params<float><<<grid_for(t->stage_n, 256), 256, 0, st>>>(z_dev, t->stage_map, m->nlayers > 1 ? m->blob_dev : m->params_dev, t->stage_n);
     s->launches += 1;
     launch_main(s, st);
     AsmParams P;

@@ -330,22 +330,26 @@ class TrainingSet:
         return self.pos.shape[1]
 
 
-def training_set(n_structures: int = 24, seed: int = 50, cells=(2, 2, 2)) -> TrainingSet:
+def training_set(n_structures: int = 24, seed: int = 50, cells=(2, 2, 2), material: str = "si") -> TrainingSet:
     """Seeded stand-in for a training set of ~100-atom structures: diamond-Si supercells with a
     per-structure lattice constant in [5.35, 5.60] A (strain), an anisotropic stretch of up to 2 % per axis and a Gaussian
     jitter of 0.03-0.15 A, every third structure with a vacancy (63 atoms).  Every box edge exceeds 2 r_c^R = 10 A."""
     u = uniform01(seed, 8 * n_structures)
-    pos, boxes, first = [], [], [0]
+    pos, boxes, first, types = [], [], [0], []
+    pbte = material == "pbte"      # rock-salt PbTe, a in [6.35, 6.60] A (every edge > 2 x 6.0 A), Pb = type 0, Te = type 1
+    basis = np.concatenate([_FCC, _FCC + np.array([.5, 0, 0])]) if pbte else _DIAMOND_BASIS
     for n in range(n_structures):
-        a = 5.35 + 0.25 * u[8 * n]
+        a = (6.35 if pbte else 5.35) + 0.25 * u[8 * n]
         stretch = 1.0 + 0.02 * (2.0 * u[8 * n + 1:8 * n + 4] - 1.0)
         sigma = 0.03 + 0.12 * u[8 * n + 4]
         box = np.array(cells, dtype=np.float64) * a * stretch
-        r = _lattice(_DIAMOND_BASIS, a, cells) * stretch
+        r = _lattice(basis, a, cells) * stretch
+        ty = np.tile(np.array([0, 0, 0, 0, 1, 1, 1, 1], dtype=np.int32), r.shape[0] // 8) if pbte else np.zeros(r.shape[0], dtype=np.int32)
         if n % 3 == 2:
-            r = np.delete(r, int(u[8 * n + 5] * r.shape[0]), axis=0)
+            k = int(u[8 * n + 5] * r.shape[0])
+            r = np.delete(r, k, axis=0); ty = np.delete(ty, k)
         r = _jitter_wrap(r, sigma, seed + 1000 + n, box)
-        pos.append(r); boxes.append(box); first.append(first[-1] + r.shape[0])
+        pos.append(r); boxes.append(box); first.append(first[-1] + r.shape[0]); types.append(ty)
     allpos = np.concatenate(pos, axis=0)
-    return TrainingSet(np.array(first, dtype=np.int64), np.ascontiguousarray(allpos.T), np.zeros(allpos.shape[0], dtype=np.int32),
+    return TrainingSet(np.array(first, dtype=np.int64), np.ascontiguousarray(allpos.T), np.concatenate(types).astype(np.int32),
                        np.array(boxes))

@@ -10,13 +10,13 @@ from test_gpu_parity import _gpu
 pytestmark = pytest.mark.gpu
 
 
-def _oracle_targets(oracle, h, ts, z):
+def _oracle_targets(oracle, h, ts, z, znum=(14,)):
     e, v = [], []
     f = np.zeros((3, ts.n_atoms))
     comp = [0, 4, 8, 1, 5, 6]
     for n in range(ts.n_structures):
         a0, a1 = ts.first[n], ts.first[n + 1]
-        out = oracle.evaluate(h, [14], z, np.ascontiguousarray(ts.pos[:, a0:a1]), None, ts.types[a0:a1], ts.boxes[n])
+        out = oracle.evaluate(h, list(znum), z, np.ascontiguousarray(ts.pos[:, a0:a1]), None, ts.types[a0:a1], ts.boxes[n])
         e.append(out["U"].sum() / (a1 - a0)); v.append(out["W"].sum(axis=1)[comp] / (a1 - a0)); f[:, a0:a1] = out["F"]
     return np.array(e), f, np.array(v)
 
@@ -98,3 +98,33 @@ def test_training_loop_reduces_the_loss():
     tr.status()
     print("best loss first/last:", best[0], best[-1])
     assert best[-1] < 0.6 * best[0]
+
+
+def test_multispecies_population_losses_match_oracle(oracle):
+    """A PbTe training set (Eq. 19 weights, descriptor and network in fp64 on the GPU) against orc_loss."""
+    torch, api = _gpu()
+    ts = inputs.training_set(8, seed=75, material="pbte")
+    znum = (82, 52)
+    h = oracle.Hyper(6.0, 4.5, 5, 3, 4, 12, 2)
+    npar = oracle.num_params(h)
+    teacher = (2 * inputs.uniform01(76, npar) - 1) / math.sqrt(30.0)
+    e, f, v = _oracle_targets(oracle, h, ts, teacher, znum)
+    dev = "cuda"
+    pos = torch.from_numpy(ts.pos).to(dev); types = torch.from_numpy(ts.types).to(dev)
+    e_t = torch.from_numpy(e.astype(np.float32)).to(dev); f_t = torch.from_numpy(f.astype(np.float32)).to(dev).contiguous()
+    v_t = torch.from_numpy(v.astype(np.float32)).to(dev).contiguous()
+    tr = api.Trainer(6.0, 4.5, 5, 3, 4, (12,), ts.first, ts.boxes, pos, e_t, f_t, v_t, cap_radial=80, cap_angular=40,
+                     types=types, atomic_numbers=znum)
+    npop = 4
+    z = teacher[None, :] + 0.02 * inputs.normal(77, npop * npar).reshape(npop, npar)
+    z[0] = teacher
+    lam = [1.0, 1.0, 1.0, 0.05, 0.05]
+    L = tr.losses(torch.from_numpy(z).to(dev).contiguous(), lam).cpu().numpy()
+    tr.status()
+    for k in range(npop):
+        ref = oracle.loss(h, list(znum), z[k], ts.first, ts.pos, ts.types, ts.boxes, e.astype(np.float32), f.astype(np.float32),
+                          v.astype(np.float32), lam)
+        print(k, L[k], ref)
+        for c in (0, 1, 2):
+            assert abs(L[k, c] - ref[c]) < 2e-4 * max(ref[c], 1e-3) + 5e-6, (k, c)
+    assert np.argmin(L[:, 5]) == 0

@@ -252,8 +252,8 @@ def main():
         hbm_peak, hbm_src = 6650.0, "fallback of /opt/skills/guides/B200_PROFILING.md"
     mr, ma = 0.5 * (m_r0 + m_r), 0.5 * (m_a0 + m_a)
     m_md = mr * ((w.rc_r + args.skin) / w.rc_r) ** 3
-    bytes_filter = 4 * m_md + 32 + 20 * mr + 32 + 8           # Verlet row, own position, records + jrev, masks, counts
-    bytes_asm = 20 * mr + 16 * mr + 32 + 16 + 4 + 24 + 64 + 12 + 48   # records + jrev, p_ji, masks, Fself, U, v rw, outputs, Fs, kick
+    bytes_filter = 4 * m_md + 32 + 16 * mr + 32 + 8           # Verlet row, own position, records (with j | rev), masks, counts
+    bytes_asm = 16 * mr + 16 * mr + 32 + 16 + 4 + 24 + 64 + 12 + 48   # records, p_ji, masks, Fself, U, v rw, outputs, Fs, kick
     hbm_phases = {}
     for name, nbytes in (("filter", bytes_filter), ("assemble", bytes_asm)):
         gbs = nbytes * N / (prof[name]["ms"] / max(1, prof[name]["count"]) * 1e-3) / 1e9

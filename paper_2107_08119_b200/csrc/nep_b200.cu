@@ -60,8 +60,9 @@ struct SysDev {                 // device pointers into the caller's workspace
     unsigned* md_idx;           // [cap_md][N]  j | rev << 24   (rev: slot of i in j's Verlet row, < 128)
     int* nnR;                   // [N]
     int* nnA;                   // [N]
-    float4* rec;                // [cap_R][N]  {dx, dy, dz, bits(type_j)}                     (read by k_main, k_assemble)
-    unsigned* jrev;             // [cap_R][N]  j | rev << 24 of the same slots                 (read by k_assemble)
+    float4* rec;                // [ceil(cap_R/2)][N][2]  {dx, dy, dz, bits(j | rev << 24)}: slots 2k and 2k+1 of an atom share one
+                                //   32-byte sector (k_filter stores them as ONE full sector: partial-sector stores run at a
+                                //   quarter of the rate); element (slot, i) at rix(slot, i, N)      (read by k_main, k_assemble)
     uint4* masks;               // [N][2] bit s set: Verlet slot s is inside r_c^R ([0]) / r_c^A ([1])
     float4* p;                  // [N][cap_R] partial forces dU_i/dr_ij at the record slots
     float2* spark0;             // [NA*6][ceil(N/kWin)*kWin] angular sums s[n][lm] of lm half 0 / half 1: parked here by k_main
@@ -85,6 +86,9 @@ struct Desc64Params {
     int H, N, capR;
     float* q_out;                         // nullable parity hook, [D][N] caller order
 };
+
+// element (slot, i) of the pair-major record array
+__host__ __device__ __forceinline__ size_t rix(int slot, int i, int N) { return ((((size_t)(slot >> 1)) * N + i) << 1) | (size_t)(slot & 1); }
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -292,6 +296,12 @@ __device__ __forceinline__ void ldg256(const uint4* p, uint4& a, uint4& b) {    
     b = make_uint4((unsigned)z, (unsigned)(z >> 32), (unsigned)w, (unsigned)(w >> 32));
 }
 
+// one 32-byte sector as one store (STG.E.256): {a, b} to a 32-byte aligned address
+__device__ __forceinline__ void stg256(float4* p, const float4& a, const float4& b) {
+    asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(a.x), "f"(a.y), "f"(a.z), "f"(a.w),
+                 "f"(b.x), "f"(b.y), "f"(b.z), "f"(b.w) : "memory");
+}
+
 __device__ __forceinline__ double min_image(double t, double L, double invL) { return t - L * rint(t * invL); }
 
 // Verlet list: all j != i with |r_ij|^2 < (r_c^R + skin)^2, rows ascending in the sorted index j
@@ -434,7 +444,8 @@ __global__ void k_build_done(SysDev d, int gated) {
 //   d = (x_j - x_i) - L rint((x_j - x_i)/L);  (dx*dx + dy*dy) + dz*dz < rc*rc     (no FMA contraction)
 // so the sets agree bit for bit (reading Q9).  Angular neighbours (r < r_c^A) are packed
 // from slot 0 upwards, radial-only ones (r_c^A <= r < r_c^R) from slot capR-1 downwards.  Records,
-// jrev, the slot masks and the counts go to global memory (k_main and k_assemble read them).
+// the slot masks and the counts go to global memory (k_main and k_assemble read them).  A record is
+// {r_ij (fp32 from the fp64 difference), j | rev << 24}; two records of an atom leave as ONE 32-byte store.
 struct FilterParams {
     Box b;
     double rcR2, rcA2;
@@ -458,7 +469,8 @@ __global__ void __launch_bounds__(128, 4) k_filter(SysDev d, int N, const __grid
     const int lane = threadIdx.x & 31;
     const double4 pi = d.xs4[i];
     const int cnt = valid ? d.md_cnt[i] : 0;
-    int nA = 0, nO = 0;
+    int nA = 0, nO = 0, kA = 0, kO = 0;          // accepted / stored (<= capR in total) angular and radial-only neighbours
+    float4 hA = make_float4(0.f, 0.f, 0.f, 0.f), hO = hA;       // the record of a pair that arrived first
     unsigned mR[4] = {0u, 0u, 0u, 0u}, mA[4] = {0u, 0u, 0u, 0u};
     constexpr int B = 8;                 // batch: B list entries, then B position gathers, in flight together
     unsigned en[B];                      // list entries of the NEXT batch: their loads overlap this batch's gathers
@@ -487,10 +499,17 @@ __global__ void __launch_bounds__(128, 4) k_filter(SysDev d, int N, const __grid
             if (r2 < F.rcR2) {
                 const bool ang = r2 < F.rcA2;
                 if (nA + nO < capR) {
-                    const int slot = ang ? nA : capR - 1 - nO;
-                    const int ty = (int)__double_as_longlong(pj.w);
-                    d.rec[(size_t)slot * N + i] = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(ty));
-                    d.jrev[(size_t)slot * N + i] = e;
+                    const float4 rv = make_float4((float)dx, (float)dy, (float)dz, __uint_as_float(e));
+                    if (ang) {                                   // slots ascend: an even slot waits for its odd partner
+                        if (nA & 1) stg256(&d.rec[rix(nA - 1, i, N)], hA, rv); else hA = rv;
+                        kA = nA + 1;
+                    } else {                                     // slots descend: an odd slot waits for the even one below it
+                        const int slot = capR - 1 - nO;
+                        if (slot & 1) hO = rv;
+                        else if (nO > 0) stg256(&d.rec[rix(slot, i, N)], rv, hO);
+                        else d.rec[rix(slot, i, N)] = rv;
+                        kO = nO + 1;
+                    }
                 }
                 bR |= 1u << u;
                 if (ang) bA |= 1u << u;
@@ -502,6 +521,9 @@ __global__ void __launch_bounds__(128, 4) k_filter(SysDev d, int N, const __grid
         for (int wq = 0; wq < 4; ++wq)
             if ((s0 >> 5) == wq) { mR[wq] |= bR << (s0 & 31); mA[wq] |= bA << (s0 & 31); }
     }
+    // records still waiting for a partner leave as single 16-byte stores
+    if (kA & 1) d.rec[rix(kA - 1, i, N)] = hA;
+    if (kO > 0 && ((capR - kO) & 1)) d.rec[rix(capR - kO, i, N)] = hO;
     const int nR = nA + nO;
     const bool over = nR > capR || nA > F.capA;
     if (valid) {
@@ -562,9 +584,7 @@ __global__ void __launch_bounds__(128) k_filter_group(SysDev d, int N, const __g
         const unsigned below = (1u << gl) - 1u, bO = bR & ~bA;
         if (inR && nA + nO + __popc(bR & below) < capR) {
             const int slot = inA ? nA + __popc(bA & below) : capR - 1 - (nO + __popc(bO & below));
-            const int ty = (int)__double_as_longlong(pj.w);
-            d.rec[(size_t)slot * N + i] = make_float4((float)dx, (float)dy, (float)dz, __int_as_float(ty));
-            d.jrev[(size_t)slot * N + i] = e;
+            d.rec[rix(slot, i, N)] = make_float4((float)dx, (float)dy, (float)dz, __uint_as_float(e));
         }
         nA += __popc(bA); nO += __popc(bO);
 #pragma unroll
@@ -603,7 +623,7 @@ __global__ void k_export_lists(SysDev d, int N, int which, int capR, int cap_out
         int v = -1;
         if (k < n) {
             const int slot = k < nA ? k : capR - 1 - (k - nA);
-            v = d.perm[d.jrev[(size_t)slot * N + i] & kJMask];
+            v = d.perm[__float_as_uint(d.rec[rix(slot, i, N)].w) & kJMask];
         }
         index[(size_t)row * cap_out + k] = v;
     }
@@ -681,7 +701,7 @@ __global__ void __launch_bounds__(128, 4) k_assemble(SysDev d, AsmParams P) {
     float w[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     const int nR = has_atom ? d.nnR[i] : 0, nA = has_atom ? d.nnA[i] : 0;
     {
-        constexpr int B = LANES == 1 ? 8 : 4;    // batch the three dependent loads (jrev -> masks -> p) for MLP
+        constexpr int B = LANES == 1 ? 8 : 4;    // batch the three dependent loads (record -> masks -> p) for MLP
         for (int k0 = 0; k0 < nR; k0 += B * LANES) {
             unsigned jr[B];
             float4 eb[B], pb[B];
@@ -690,8 +710,8 @@ __global__ void __launch_bounds__(128, 4) k_assemble(SysDev d, AsmParams P) {
             for (int u = 0; u < B; ++u) {
                 const int k = min(k0 + u * LANES + gl, nR - 1);
                 const int slot = k < nA ? k : P.capR - 1 - (k - nA);
-                jr[u] = d.jrev[(size_t)slot * N + i];
-                eb[u] = d.rec[(size_t)slot * N + i];
+                eb[u] = d.rec[rix(slot, i, N)];
+                jr[u] = __float_as_uint(eb[u].w);
             }
 #pragma unroll
             for (int u = 0; u < B; ++u) ldg256(&d.masks[2 * (size_t)(jr[u] & kJMask)], mrb[u], mab[u]);
@@ -899,8 +919,7 @@ Layout carve(int64_t N, int capR, int capMD, int max_cells, int NA, int D64, Sys
     t.md_idx = (unsigned*)take(n * 4 * capMD);
     t.nnR = (int*)take(n * 4);
     t.nnA = (int*)take(n * 4);
-    t.rec = (float4*)take(n * 16 * capR);
-    t.jrev = (unsigned*)take(n * 4 * capR);
+    t.rec = (float4*)take(n * 32 * (size_t)((capR + 1) / 2));
     t.masks = (uint4*)take(n * 32);
     t.xs4 = (double4*)take(n * 32);
     t.p = (float4*)take(n * 16 * capR);

@@ -15,7 +15,7 @@
 // fp64 geometry of neighbour `slot` of atom i: minimum-image r_ij from the fp64 positions, and Eq. 19's weight
 struct Nbr64 { double x, y, z, r, om; };
 __device__ __forceinline__ Nbr64 nbr64(const SysDev& d, const Box& b, const double4& pi, const double* zrow, int slot, int N, int i) {
-    const int j = (int)(d.jrev[(size_t)slot * N + i] & kJMask);
+    const int j = (int)(__float_as_uint(d.rec[rix(slot, i, N)].w) & kJMask);
     const double4 pj = d.xs4[j];
     Nbr64 o;
     o.x = min_image(pj.x - pi.x, b.L[0], b.invL[0]);

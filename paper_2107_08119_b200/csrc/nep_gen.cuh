@@ -147,7 +147,7 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
         auto nbr = [&](int k, TD& x, TD& y, TD& z, TD& r, TD& om) {
             const int slot = gen_slot(k, nA, capR);
             if (F64) {
-                const int j = (int)(d.jrev[(size_t)slot * N + i] & kJMask);
+                const int j = (int)(__float_as_uint(d.rec[rix(slot, i, N)].w) & kJMask);
                 const double4 pj = d.xs4[j];
                 const double dx = min_image(pj.x - pi.x, bL[0], bI[0]);
                 const double dy = min_image(pj.y - pi.y, bL[1], bI[1]);
@@ -156,11 +156,11 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
                 x = (TD)(dx * ri); y = (TD)(dy * ri); z = (TD)(dz * ri); r = (TD)rr;
                 om = (TD)P.zz64[ti * kMaxTypes + ((int)__double_as_longlong(pj.w) & (kMaxTypes - 1))];
             } else {
-                const float4 e = d.rec[(size_t)slot * N + i];
+                const float4 e = d.rec[rix(slot, i, N)];
                 const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
                 const float ri = inv_norm(r2);
                 x = (TD)(e.x * ri); y = (TD)(e.y * ri); z = (TD)(e.z * ri); r = (TD)(r2 * ri);
-                om = (TD)P.zz[ti * kMaxTypes + (__float_as_int(e.w) & (kMaxTypes - 1))];
+                om = (TD)P.zz[ti * kMaxTypes + d.type_s[__float_as_uint(e.w) & kJMask]];
             }
         };
 
@@ -408,12 +408,12 @@ __global__ void __launch_bounds__(32 * kGenWarps) k_gen(SysDev d, const __grid_c
             const int k = c * kGenLanes + gl;
             const bool on = k < nR;
             const int slot = gen_slot(on ? k : 0, nA, capR);
-            float4 e = make_float4(1.f, 0.f, 0.f, 0.f);
-            if (on) e = d.rec[(size_t)slot * N + i];
+            float4 e = make_float4(1.f, 0.f, 0.f, __uint_as_float((unsigned)i));
+            if (on) e = d.rec[rix(slot, i, N)];
             const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
             const float rinv = inv_norm(r2), r = r2 * rinv;
             const float x = e.x * rinv, y = e.y * rinv, z = e.z * rinv;
-            const float om = P.zz[ti * kMaxTypes + (__float_as_int(e.w) & (kMaxTypes - 1))];
+            const float om = P.zz[ti * kMaxTypes + d.type_s[__float_as_uint(e.w) & kJMask]];
             // radial family, Eq. 24
             float gR[NMAX], dR[NMAX];
             radial_gd<NMAX>(r, P.rcR_inv, om, 1.f, gR, dR);

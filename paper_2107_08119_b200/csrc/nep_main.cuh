@@ -266,9 +266,10 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
     const int i = active ? i_ord : 0;
     const int nR = active ? d.nnR[i] : 0, nA = active ? d.nnA[i] : 0;
     const int nO = nR - nA;
-    const float4* grec = d.rec + i;                  // record of slot s: grec[(size_t)s * N]
+    const float4* grec = d.rec + 2 * (size_t)i;      // record of slot s: grec[goff(s)] (pair-major rows, see rix())
+    auto goff = [&](int s) { return ((size_t)(s >> 1) * N << 1) | (size_t)(s & 1); };
     const float* zrow = Z.zz + (MULTI ? d.type_s[i] * kMaxTypes : 0);
-    auto omega_of = [&](const float4& e) { return MULTI ? zrow[__float_as_int(e.w) & (kMaxTypes - 1)] : 1.f; };
+    auto omega_of = [&](const float4& e) { return MULTI ? zrow[d.type_s[__float_as_uint(e.w) & kJMask]] : 1.f; };
 
     // ---- P0: every neighbour record of the atom in flight at once (cp.async); the weights arrive as ONE bulk copy ----
     {
@@ -280,8 +281,8 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
             bulk_g2s(sm, params, (unsigned)wfl * 4u, wbar);
         }
         const int ka = min(nA, kRowsS), ko = min(nO, kRowsO);
-        for (int k = 0; k < ka; ++k) cp_async16(&srec[k * 32 + lane], &grec[(size_t)k * N]);
-        for (int o = 0; o < ko; ++o) cp_async16(&praw[o * 32 + lane], &grec[(size_t)(P.capR - 1 - o) * N]);
+        for (int k = 0; k < ka; ++k) cp_async16(&srec[k * 32 + lane], &grec[goff(k)]);
+        for (int o = 0; o < ko; ++o) cp_async16(&praw[o * 32 + lane], &grec[goff(P.capR - 1 - o)]);
         cp_async_wait_all();
         mbar_wait(wbar, 0);
         __syncwarp();
@@ -294,7 +295,7 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
             x = e.x; y = e.y; z = e.z; r = e.w;
             om = MULTI ? som[k * 32 + lane] : 1.f;
         } else {
-            const float4 e = grec[(size_t)k * N];
+            const float4 e = grec[goff(k)];
             const float r2 = e.x * e.x + e.y * e.y + e.z * e.z;
             const float rinv = inv_norm(r2);
             x = e.x * rinv; y = e.y * rinv; z = e.z * rinv; r = r2 * rinv;
@@ -320,8 +321,8 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
     //  first descriptor pass below, which touches them anyway)
     for (int k = 0; MULTI && k < nA; k += 2) {       // two neighbours per iteration: independent chains
         const int k1 = min(k + 1, nA - 1);
-        const float4 e0 = k < kRowsS ? srec[k * 32 + lane] : grec[(size_t)k * N];
-        const float4 e1 = k1 < kRowsS ? srec[k1 * 32 + lane] : grec[(size_t)k1 * N];
+        const float4 e0 = k < kRowsS ? srec[k * 32 + lane] : grec[goff(k)];
+        const float4 e1 = k1 < kRowsS ? srec[k1 * 32 + lane] : grec[goff(k1)];
         float ri0, r0, om0, ri1, r1, om1;
         radial_acc(e0, true, ri0, r0, om0);
         radial_acc(e1, k + 1 < nA, ri1, r1, om1);
@@ -336,7 +337,7 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
     }
     // radial-only record o: one generic load from the staged row or, past kRowsO rows, from global memory (no branch)
     auto raw_only = [&](int o) {
-        const float4* src = o < kRowsO ? &praw[o * 32 + lane] : &grec[(size_t)(P.capR - 1 - o) * N];
+        const float4* src = o < kRowsO ? &praw[o * 32 + lane] : &grec[goff(P.capR - 1 - o)];
         return *src;
     };
     for (int o = 0; o < nO; o += 4) {                // four independent chains per iteration
@@ -379,7 +380,7 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
     if (!MULTI) {
         // first touch of an angular neighbour: raw record -> Eq. 12's share, then {r^, r} back into its row
         auto load_first = [&](int k, float& x, float& y, float& z, float& r, float& om) {
-            const float4 e = k < kRowsS ? srec[k * 32 + lane] : grec[(size_t)k * N];
+            const float4 e = k < kRowsS ? srec[k * 32 + lane] : grec[goff(k)];
             float rinv;
             radial_acc(e, true, rinv, r, om);
             x = e.x * rinv; y = e.y * rinv; z = e.z * rinv;

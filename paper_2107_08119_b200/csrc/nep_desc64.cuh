@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(64) k_desc64(SysDev d, Box b, const __grid_con
     constexpr int LOF[kNumLM] = {NEP_LOF_LIST};
     const size_t gcol = (size_t)blockIdx.x * 64 + threadIdx.x;
     const size_t npad = (size_t)gridDim.x * 64;
-    const int i = d.order[gcol];
+    const int i = d.order[gcol].x;
     if (i < 0) return;
     const int N = P.N;
     const int nR = d.nnR[i], nA = d.nnA[i];

@@ -71,13 +71,15 @@ __global__ void __launch_bounds__(kOrderThreads) k_order(SysDev d, int N) {
     const int t = threadIdx.x;
     for (int b = t; b < kOrderBins; b += kOrderThreads) hist[b] = 0;
     __syncthreads();
-    int bin[kOrderItems];
+    int bin[kOrderItems], cnts[kOrderItems];
 #pragma unroll
     for (int u = 0; u < kOrderItems; ++u) {
         const int i = blockIdx.x * kWin + u * kOrderThreads + t;
         bin[u] = kOrderBins - 1;                      // past N: sorts last
+        cnts[u] = 0;
         if (i < N) {
-            const int nA = d.nnA[i], nO = d.nnR[i] - nA;
+            const int nA = d.nnA[i], nR = d.nnR[i], nO = nR - nA;
+            cnts[u] = nA | (nR << 8);
             bin[u] = max(0, kOrderBins - 2 - (min(nA, 127) * 32 + min(max(nO, 0), 31)));     // descending key
         }
         atomicAdd(&hist[bin[u]], 1);
@@ -102,7 +104,7 @@ __global__ void __launch_bounds__(kOrderThreads) k_order(SysDev d, int N) {
     for (int u = 0; u < kOrderItems; ++u) {
         const int i = blockIdx.x * kWin + u * kOrderThreads + t;
         const int rank = atomicAdd(&hist[bin[u]], 1);  // order inside a bin is arbitrary (equal keys)
-        d.order[blockIdx.x * kWin + rank] = i < N ? i : -1;
+        d.order[blockIdx.x * kWin + rank] = make_int2(i < N ? i : -1, cnts[u]);
     }
 }
 
@@ -261,10 +263,10 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
     float* som = wsm + (kRowsS + kRowsO) * 32 * 4;                     // [kRowsS][32] omega_ij (MULTI only)
 
     const int N = P.N;
-    const int i_ord = d.order[(blockIdx.x * kMainWarps + warp) * 32 + lane];
-    const bool active = i_ord >= 0;
-    const int i = active ? i_ord : 0;
-    const int nR = active ? d.nnR[i] : 0, nA = active ? d.nnA[i] : 0;
+    const int2 oe = d.order[(blockIdx.x * kMainWarps + warp) * 32 + lane];
+    const bool active = oe.x >= 0;
+    const int i = active ? oe.x : 0;
+    const int nR = active ? oe.y >> 8 : 0, nA = active ? oe.y & 255 : 0;
     const int nO = nR - nA;
     const float4* grec = d.rec + 2 * (size_t)i;      // record of slot s: grec[goff(s)] (pair-major rows, see rix())
     auto goff = [&](int s) { return ((size_t)(s >> 1) * N << 1) | (size_t)(s & 1); };

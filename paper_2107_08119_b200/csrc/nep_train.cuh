@@ -47,7 +47,7 @@ __global__ void k_build_batch(SysDev d, int N, const double* __restrict__ pos, c
         const double dy = min_image(pos[N + j] - yi, bx[1], bx[4]);
         const double dz = min_image(pos[2 * (size_t)N + j] - zi, bx[2], bx[5]);
         if (dx * dx + dy * dy + dz * dz < rc2) {
-            if (cnt < capMD) d.md_idx[(size_t)cnt * N + i] = (unsigned)j;
+            if (cnt < capMD) d.md_idx[mix(cnt, i, N)] = (unsigned)j;
             ++cnt;
         }
     }

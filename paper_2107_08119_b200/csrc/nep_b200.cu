@@ -28,7 +28,7 @@ constexpr int kMaxCapMD = 124;                // Verlet slots per atom: the acce
 constexpr double kAmuConv = 103.642697;       // 1 amu A^2/fs^2 in eV
 
 // device status / counter words (int32 each)
-enum { F_STATUS = 0, F_REBUILD = 1, F_STEP = 2, F_NREBUILD = 3, F_MAXR = 4, F_MAXA = 5, F_MAXMD = 6, F_BUILT = 7,
+enum { F_STATUS = 0, F_REBUILD = 1, F_STEP = 2, F_NREBUILD = 3, F_MAXR = 4, F_MAXA = 5, F_MAXMD = 6, F_BUILT = 7, F_NSTEPS = 8,
        F_COUNT = 16 };
 enum { ST_OVERFLOW = 1, ST_STALE = 2, ST_BADTYPE = 4 };
 
@@ -256,7 +256,9 @@ __device__ __forceinline__ void ph_gather_b(const SysDev& d, int N, int have_v, 
     }
 }
 
+// gated == 2: the chain opens an MD step -- its first kernel also advances the step counter (nothing else runs then)
 __global__ void k_clear_cells(SysDev d, int ncell, int gated) {
+    if (gated == 2 && blockIdx.x == 0 && threadIdx.x == 0) d.flags[F_STEP] += 1;
     if (gate_closed(d.flags, gated)) return;
     ph_clear(d, ncell, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
@@ -423,6 +425,7 @@ __device__ __forceinline__ void cluster_barrier() {
 __global__ void __cluster_dims__(kClusterCTAs, 1, 1) __launch_bounds__(1024, 1)
 k_build_cluster(SysDev d, const double* xin, const double* vin, int N, Box b, double rc2,
                 int capMD, int first, int n_types, int gated) {
+    if (gated == 2 && blockIdx.x == 0 && threadIdx.x == 0) d.flags[F_STEP] += 1;
     if (gate_closed(d.flags, gated)) return;               // uniform over the cluster: nobody reaches a barrier
     __shared__ int part[1024];
     const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
@@ -546,8 +549,8 @@ __global__ void __launch_bounds__(128, 4) k_filter(SysDev d, int N, const __grid
         d.nnA[i] = over ? 0 : nA;          // an overflowing atom is dropped (and reported), never truncated
         d.nnR[i] = over ? 0 : nR;
         if (over) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
-        d.masks[2 * (size_t)i] = make_uint4(mR[0], mR[1], mR[2], mR[3]);
-        d.masks[2 * (size_t)i + 1] = make_uint4(mA[0], mA[1], mA[2], mA[3]);
+        const unsigned mm[8] = {mR[0], mR[1], mR[2], mR[3], mA[0], mA[1], mA[2], mA[3]};
+        st_octet(reinterpret_cast<unsigned*>(&d.masks[2 * (size_t)i]), mm);        // both masks: one full sector
     }
     // warp-aggregated statistics
     int xR = nR, xA = nA;
@@ -671,6 +674,7 @@ struct AsmParams {
     int N, capR, capMD;
     int md;                       // 0: nep_compute; 1: MD step (kick, J from vs, thermo); 2: F(t0) of nep_md_step
     double half_dt;               // dt/2
+    double dt, half_skin2;        // MD step: the NEXT step's half-kick + drift happen here too (not after the call's last step)
     double inv_mass[kMaxTypes];   // 1 / (m * 103.642697)
     double ke_mass[kMaxTypes];    // 0.5 * m * 103.642697
     const double* vel_in;         // nep_compute: caller-order velocities (nullable)
@@ -781,10 +785,20 @@ __global__ void __launch_bounds__(128, 4) k_assemble(SysDev d, AsmParams P) {
             const int ty = d.type_s[i];
             const double im = P.md == 1 ? P.inv_mass[ty] * P.half_dt : 0.0;   // md == 2: F(t0) only, no kick
             vx = d.vs[i] + im * (double)fx; vy = d.vs[N + i] + im * (double)fy; vz = d.vs[2 * N + i] + im * (double)fz;
-            d.vs[i] = vx; d.vs[N + i] = vy; d.vs[2 * N + i] = vz;
             tK = P.ke_mass[ty] * (vx * vx + vy * vy + vz * vz);
             tU = (double)u;
             have_v = true;
+            if (P.md == 1 && d.flags[F_STEP] < d.flags[F_NSTEPS]) {
+                // not the call's last step: the next step's first half-kick and drift, while v and F are in registers
+                // (nothing in this kernel reads positions; K, J and K(t) below use the velocity at t + dt)
+                const double wx = vx + im * (double)fx, wy = vy + im * (double)fy, wz = vz + im * (double)fz;
+                const double xn = d.xs[i] + P.dt * wx, yn = d.xs[N + i] + P.dt * wy, zn = d.xs[2 * N + i] + P.dt * wz;
+                d.vs[i] = wx; d.vs[N + i] = wy; d.vs[2 * N + i] = wz;
+                d.xs[i] = xn; d.xs[N + i] = yn; d.xs[2 * N + i] = zn;
+                d.xs4[i] = make_double4(xn, yn, zn, __longlong_as_double((long long)ty));
+                const double ax = xn - d.xref[i], ay = yn - d.xref[N + i], az = zn - d.xref[2 * N + i];
+                if (ax * ax + ay * ay + az * az > P.half_skin2) d.flags[F_REBUILD] = 1;
+            } else { d.vs[i] = vx; d.vs[N + i] = vy; d.vs[2 * N + i] = vz; }
         } else if (P.vel_in) {
             vx = P.vel_in[row]; vy = P.vel_in[N + row]; vz = P.vel_in[2 * N + row];
             have_v = true;
@@ -829,7 +843,6 @@ __global__ void __launch_bounds__(128, 4) k_assemble(SysDev d, AsmParams P) {
 // v += dt/2 F/m;  r += dt v;  raise the rebuild flag when an atom has moved > skin/2 since the build
 __global__ void k_kick_drift(SysDev d, int N, double dt, double half_skin2, AsmParams P) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i == 0) d.flags[F_STEP] += 1;
     if (i >= N) return;
     const int ty = d.type_s[i];
     const double im = P.inv_mass[ty] * P.half_dt;
@@ -851,9 +864,9 @@ __global__ void k_kick_drift(SysDev d, int N, double dt, double half_skin2, AsmP
 // caller arrays -> sorted state.  mode 0 (nep_compute): a displacement > skin/2 is an error (stale
 // list); mode 1 (nep_md_step): it requests a rebuild.
 __global__ void k_load_state(SysDev d, int N, const double* __restrict__ pos, const double* __restrict__ vel,
-                             double half_skin2, int mode) {
+                             double half_skin2, int mode, int n_steps) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k == 0 && mode == 1) d.flags[F_STEP] = 0;
+    if (k == 0 && mode == 1) { d.flags[F_STEP] = 0; d.flags[F_NSTEPS] = n_steps; }
     if (k >= N) return;
     const int src = d.perm[k];
     double disp2 = 0.0, xn[3];
@@ -1135,19 +1148,16 @@ bool device_ok() {
 }
 
 // one velocity-Verlet step: half-kick + drift, device-gated rebuild, filter, k_main, assembly + second half-kick
-void launch_step(nep_system* s, const AsmParams& P, double dt_fs, double hs2, cudaStream_t st) {
-    const int N = (int)s->N;
-    phase(s, PH_KICK, st);
-    k_kick_drift<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, dt_fs, hs2, P);
+// (the half-kick + drift of every step but the call's first happen inside the previous step's assembly)
+void launch_step(nep_system* s, const AsmParams& P, cudaStream_t st) {
     phase(s, PH_BUILD, st);
-    launch_build(s, s->d.xs, s->d.vs, 0, 1, st);
+    launch_build(s, s->d.xs, s->d.vs, 0, 2, st);
     phase(s, PH_FILTER, st);
     launch_filter(s, st);
     phase(s, PH_MAIN, st);
     launch_main(s, st);
     phase(s, PH_ASSEMBLE, st);
     launch_assemble(s, P, st);
-    s->launches += 1;
 }
 
 // The step as a CUDA graph, captured on a library-owned stream (the caller's may be the legacy default
@@ -1164,7 +1174,7 @@ int ensure_step_graph(nep_system* s, const AsmParams& P, double dt_fs, double hs
     cudaGraph_t g = nullptr;
     NEP_CUDA_OK(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
     const int64_t l0 = s->launches;
-    launch_step(s, P, dt_fs, hs2, s->cap_stream);
+    launch_step(s, P, s->cap_stream);
     s->g_launches = s->launches - l0;
     s->launches = l0;
     NEP_CUDA_OK(cudaStreamEndCapture(s->cap_stream, &g));
@@ -1416,7 +1426,7 @@ int nep_compute(nep_system* s, const double* pos_dev, const double* vel_dev, flo
     const int N = (int)s->N;
     const double hs = 0.5 * s->skin;
     phase(s, PH_STATE, st);
-    k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, nullptr, hs * hs * (1.0 + 1e-12) + 1e-24, 0);
+    k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, nullptr, hs * hs * (1.0 + 1e-12) + 1e-24, 0, 0);
     phase(s, PH_FILTER, st);
     launch_filter(s, st);
     phase(s, PH_MAIN, st);
@@ -1443,7 +1453,7 @@ int nep_compute_internals(nep_system* s, const double* pos_dev, float* q_dev, fl
     s->last_stream = st;
     const int N = (int)s->N;
     const double hs = 0.5 * s->skin;
-    k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, nullptr, hs * hs * (1.0 + 1e-12) + 1e-24, 0);
+    k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, nullptr, hs * hs * (1.0 + 1e-12) + 1e-24, 0, 0);
     launch_filter(s, st);
     s->dump_q = q_dev; s->dump_fp = fp_dev;
     launch_main(s, st);
@@ -1477,7 +1487,7 @@ int nep_md_step_driven(nep_system* s, double* pos_dev, double* vel_dev, const do
     AsmParams P;
     memset(&P, 0, sizeof(P));
     P.N = N; P.capR = s->capR; P.capMD = s->capMD;
-    P.half_dt = 0.5 * dt_fs;
+    P.half_dt = 0.5 * dt_fs; P.dt = dt_fs; P.half_skin2 = hs2;
     fill_masses(&P, s->model, mass_by_type);
     P.energy = energy_dev; P.force = force_dev; P.virial = virial_dev; P.heat = heat_dev;
     P.heat_sum = heat_sum_dev; P.thermo = thermo_dev;
@@ -1493,7 +1503,7 @@ int nep_md_step_driven(nep_system* s, double* pos_dev, double* vel_dev, const do
     if (kt_dev && n_steps > 0) NEP_CUDA_OK(cudaMemsetAsync(kt_dev, 0, (size_t)n_steps * 3 * sizeof(double), st));
     // caller arrays -> sorted state
     phase(s, PH_STATE, st);
-    k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, vel_dev, hs2, 1);
+    k_load_state<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, pos_dev, vel_dev, hs2, 1, n_steps);
     s->launches += 1;
     if (!s->have_forces) {       // F(t0); a call that directly follows nep_md_step continues from its forces
         phase(s, PH_BUILD, st);
@@ -1507,8 +1517,13 @@ int nep_md_step_driven(nep_system* s, double* pos_dev, double* vel_dev, const do
         launch_assemble(s, P, st);
     }
     P.md = 1;
+    if (n_steps > 0) {           // the first step's half-kick + drift; the later ones are fused into the assembly before them
+        phase(s, PH_KICK, st);
+        k_kick_drift<<<grid_for(N, 256), 256, 0, st>>>(s->d, N, dt_fs, hs2, P);
+        s->launches += 1;
+    }
     if (s->prof_on || n_steps < 2) {
-        for (int step = 0; step < n_steps; ++step) launch_step(s, P, dt_fs, hs2, st);
+        for (int step = 0; step < n_steps; ++step) launch_step(s, P, st);
     } else {
         // the step's launch sequence is fixed (rebuilds are device-gated): capture it once, replay it
         const int rc = ensure_step_graph(s, P, dt_fs, hs2);

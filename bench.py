@@ -137,7 +137,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4_1048576")
-    ap.add_argument("--skin", type=float, default=1.0)
+    ap.add_argument("--skin", type=float, default=None, help="Verlet skin in A (default 1.0; 0.4 for c0, whose box must exceed 2 (r_c^R + skin))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -166,6 +166,8 @@ def main():
     w = make_workload(args.workload)
     N = w.n_atoms
     cap_r, cap_a = caps_for(args.workload, w)
+    if args.skin is None:
+        args.skin = 0.4 if args.workload == "c0" else 1.0
     model, system, pos, vel = api.from_workload(w, cap_r, cap_a, args.skin, dev)
     out = system.alloc_outputs()
     heat_sum = torch.zeros((3, N), dtype=torch.float64, device=dev)

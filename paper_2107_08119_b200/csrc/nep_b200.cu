@@ -519,16 +519,15 @@ __global__ void __launch_bounds__(128, 4) k_filter(SysDev d, int N, const __grid
                 const bool ang = r2 < F.rcA2;
                 if (nA + nO < capR) {
                     const float4 rv = make_float4((float)dx, (float)dy, (float)dz, __uint_as_float(e));
-                    if (ang) {                                   // slots ascend: an even slot waits for its odd partner
-                        if (nA & 1) stg256(&d.rec[rix(nA - 1, i, N)], hA, rv); else hA = rv;
-                        kA = nA + 1;
-                    } else {                                     // slots descend: an odd slot waits for the even one below it
-                        const int slot = capR - 1 - nO;
-                        if (slot & 1) hO = rv;
-                        else if (nO > 0) stg256(&d.rec[rix(slot, i, N)], rv, hO);
-                        else d.rec[rix(slot, i, N)] = rv;
-                        kO = nO + 1;
-                    }
+                    // angular slots ascend: an even slot waits for its odd partner; radial-only slots descend: an odd
+                    // slot waits for the even one below it.  One store site, selects instead of branches.
+                    const int slot = ang ? nA : capR - 1 - nO;
+                    const bool odd = slot & 1;
+                    const bool pair = ang ? odd : (!odd && nO > 0);
+                    const float4 lo = ang ? hA : rv, hi = ang ? rv : hO;
+                    if (pair) stg256(&d.rec[rix(slot & ~1, i, N)], lo, hi);
+                    else if (!ang && !odd) d.rec[rix(slot, i, N)] = rv;      // the top slot of an odd capacity has no partner
+                    if (ang) { hA = rv; kA = nA + 1; } else { hO = rv; kO = nO + 1; }
                 }
                 bR |= 1u << u;
                 if (ang) bA |= 1u << u;

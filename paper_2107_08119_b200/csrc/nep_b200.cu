@@ -90,9 +90,10 @@ struct Desc64Params {
 };
 
 // element (slot, i) of the octet-major Verlet array
-__host__ __device__ __forceinline__ size_t mix(int slot, int i, int N) { return ((((size_t)(slot >> 3)) * N + i) << 3) | (size_t)(slot & 7); }
+// (N < 2^24 and at most 128 slots: the element index fits 32 bits)
+__host__ __device__ __forceinline__ unsigned mix(int slot, int i, int N) { return ((((unsigned)(slot >> 3)) * (unsigned)N + (unsigned)i) << 3) | (unsigned)(slot & 7); }
 // element (slot, i) of the pair-major record array
-__host__ __device__ __forceinline__ size_t rix(int slot, int i, int N) { return ((((size_t)(slot >> 1)) * N + i) << 1) | (size_t)(slot & 1); }
+__host__ __device__ __forceinline__ unsigned rix(int slot, int i, int N) { return ((((unsigned)(slot >> 1)) * (unsigned)N + (unsigned)i) << 1) | (unsigned)(slot & 1); }
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -524,9 +525,10 @@ __global__ void __launch_bounds__(128, 4) k_filter(SysDev d, int N, const __grid
                     const int slot = ang ? nA : capR - 1 - nO;
                     const bool odd = slot & 1;
                     const bool pair = ang ? odd : (!odd && nO > 0);
-                    const float4 lo = ang ? hA : rv, hi = ang ? rv : hO;
-                    if (pair) stg256(&d.rec[rix(slot & ~1, i, N)], lo, hi);
-                    else if (!ang && !odd) d.rec[rix(slot, i, N)] = rv;      // the top slot of an odd capacity has no partner
+                    const float4 lo = ang ? hA : rv, hi = ang ? rv : hO;     // (two store sites instead of the selects: 0.36 -> 0.39 ms)
+                    float4* dst = &d.rec[rix(slot & ~1, i, N)];
+                    if (pair) stg256(dst, lo, hi);
+                    else if (!ang && !odd) *dst = rv;                        // the top slot of an odd capacity has no partner
                     if (ang) { hA = rv; kA = nA + 1; } else { hO = rv; kO = nO + 1; }
                 }
                 bR |= 1u << u;

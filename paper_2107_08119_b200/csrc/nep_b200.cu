@@ -428,7 +428,7 @@ __global__ void __launch_bounds__(128) k_rev(SysDev d, int N, int gated) {
 // The whole build in ONE launch for small systems: a cluster of 8 CTAs x 1024 threads, phases separated by
 // cluster barriers (hardware barrier across the cluster's SMs, release/acquire at cluster scope).  A step
 // without rebuild then costs one early-exit launch instead of ten.
-constexpr int kClusterCTAs = 8;
+constexpr int kClusterCTAs = 16;               // non-portable cluster size (opt-in attribute, set at the first launch)
 constexpr int64_t kClusterBuildMaxAtoms = 16384;
 __device__ __forceinline__ void cluster_barrier() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
@@ -439,7 +439,10 @@ k_build_cluster(SysDev d, const double* xin, const double* vin, int N, Box b, do
     if (gated == 2 && blockIdx.x == 0 && threadIdx.x == 0) d.flags[F_STEP] += 1;
     if (gate_closed(d.flags, gated)) return;               // uniform over the cluster: nobody reaches a barrier
     __shared__ int part[1024];
-    const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
+    // warps are dealt round-robin over the CTAs: with tid = blockIdx * 1024 + threadIdx a 4096-atom system would keep
+    // 4 of the 16 SMs busy (measured: its Verlet build was bound by the FP64 pipes of those four SMs, 107 of 185 us)
+    const int nth = gridDim.x * blockDim.x;
+    const int tid = ((threadIdx.x >> 5) * gridDim.x + blockIdx.x) * 32 + (threadIdx.x & 31);
     ph_clear(d, b.ncell, tid, nth);
     cluster_barrier();
     ph_bin(d, xin, N, b, tid, nth);
@@ -984,6 +987,13 @@ void launch_build(nep_system* s, const double* xin, const double* vin, int first
     const Box& b = s->box;
     const double rc = s->model->h.rc_radial + s->skin;
     if (s->N <= kClusterBuildMaxAtoms) {
+        static bool np_done[64] = {};
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (dev < 0 || dev >= 64 || !np_done[dev]) {
+            if (cudaFuncSetAttribute(k_build_cluster, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess && dev >= 0 && dev < 64)
+                np_done[dev] = true;
+        }
         k_build_cluster<<<kClusterCTAs, 1024, 0, st>>>(d, xin, vin, N, b, rc * rc, s->capMD, first, s->model->h.n_types, gated);
         s->launches += 1;
         return;

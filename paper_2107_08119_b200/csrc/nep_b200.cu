@@ -59,6 +59,7 @@ struct SysDev {                 // device pointers into the caller's workspace
     int* md_cnt;                // [N]
     unsigned* md_idx;           // [ceil(cap_md/8)][N][8]  j | rev << 24   (rev: slot of i in j's Verlet row, < 128): eight
                                 //   consecutive slots of an atom are one 32-byte sector, written and read as such; element (slot, i) at mix()
+    int capMD;                  // slots per Verlet row
     int* nnR;                   // [N]
     int* nnA;                   // [N]
     float4* rec;                // [ceil(cap_R/2)][N][2]  {dx, dy, dz, bits(j | rev << 24)}: slots 2k and 2k+1 of an atom share one
@@ -323,54 +324,101 @@ __device__ __forceinline__ double min_image(double t, double L, double invL) { r
 // Verlet list: all j != i with |r_ij|^2 < (r_c^R + skin)^2, rows ascending in the sorted index j
 // (neighbour cells are visited in ascending cell id; a cell's atoms are contiguous and ascending).
 // NC: read positions through the non-coherent path (valid when an earlier KERNEL wrote them).
-template <bool NC>
+// the wrapped coordinates {c-1, c, c+1} of one axis in ascending order (one value when the axis has a single cell)
+__device__ __forceinline__ int sorted_axis(int c, int nc, int (&a)[3]) {
+    if (nc == 1) { a[0] = a[1] = a[2] = 0; return 1; }
+    const int m = c == 0 ? nc - 1 : c - 1, p = c == nc - 1 ? 0 : c + 1;     // nc >= 3: three distinct values
+    if (m > c) { a[0] = c; a[1] = p; a[2] = m; }          // c == 0:      {0, 1, nc-1}
+    else if (p < c) { a[0] = p; a[1] = m; a[2] = c; }     // c == nc-1:   {0, nc-2, nc-1}
+    else { a[0] = m; a[1] = c; a[2] = p; }
+    return 3;
+}
+
+// LANES (1, 2 or 4 adjacent lanes of a warp) share an atom: each lane takes a contiguous part of the sorted cell
+// list, keeps the neighbours it accepts in a small local buffer, and the parts are concatenated through a shuffle
+// prefix -- the row stays ascending.  Small systems use it to spread one atom's ~310 candidate tests (a serial
+// chain of FP64 latencies) over the otherwise idle threads of the cluster.
+constexpr int kBuildBuf = 48;       // accepted neighbours a lane can buffer (a whole row when LANES = 1: else it re-scans)
+template <bool NC, int LANES>
 __device__ __forceinline__ void ph_build_md(const SysDev& d, int N, const Box& b, double rc2, int capMD, int tid, int nth) {
-    for (int i = tid; i < N; i += nth) {
+    const int l = tid % LANES;
+    const int natoms_pad = ((N + 31) / 32) * 32;                     // whole warps stay in the loop (shuffles below)
+    for (int i0 = tid / LANES; i0 < natoms_pad; i0 += nth / LANES) {
+        const bool valid = i0 < N;
+        const int i = valid ? i0 : N - 1;
         const double xi = d.xs[i], yi = d.xs[N + i], zi = d.xs[2 * N + i];
         const int cx = cell_coord(xi, b.L[0], b.invL[0], b.nc[0]);
         const int cy = cell_coord(yi, b.L[1], b.invL[1], b.nc[1]);
         const int cz = cell_coord(zi, b.L[2], b.invL[2], b.nc[2]);
-        int cells[27];
-        int ncells = 0;
-        const int wx = b.nc[0] > 1 ? 1 : 0, wy = b.nc[1] > 1 ? 1 : 0, wz = b.nc[2] > 1 ? 1 : 0;   // nc is 1 or >= 3
-        for (int ox = -wx; ox <= wx; ++ox)
-            for (int oy = -wy; oy <= wy; ++oy)
-                for (int oz = -wz; oz <= wz; ++oz) {
-                    const int c = (((cx + ox + b.nc[0]) % b.nc[0]) * b.nc[1] + (cy + oy + b.nc[1]) % b.nc[1]) * b.nc[2] +
-                                  (cz + oz + b.nc[2]) % b.nc[2];
-                    int k = ncells++;
-                    while (k > 0 && cells[k - 1] > c) { cells[k] = cells[k - 1]; --k; }
-                    cells[k] = c;
-                }
+        // The 27 neighbour cells in ascending cell id = lexicographic order of (X, Y, Z) with each axis' three wrapped
+        // coordinates sorted; a (X, Y) column's Z cells are adjacent in memory, so an unwrapped column is ONE index range.
+        int ax[3], ay[3], az[3];
+        const int nx = sorted_axis(cx, b.nc[0], ax), ny = sorted_axis(cy, b.nc[1], ay), nz = sorted_axis(cz, b.nc[2], az);
+        const bool zrun = nz == 1 || (az[2] - az[0] == 2);               // the column's Z cells are contiguous
+        const int ncols = nx * ny;
+        const int q0 = valid ? (l * ncols) / LANES : 0, q1 = valid ? ((l + 1) * ncols) / LANES : 0;
+        int base = 0;                // slot of this lane's first neighbour (known after the first sweep when LANES > 1)
         int cnt = 0;
-        for (int q = 0; q < ncells; ++q) {
-            const int lo = d.cell_start[cells[q]], hi = d.cell_start[cells[q] + 1];
-            for (int j0 = lo; j0 < hi; j0 += 4) {                // four candidates in flight (the loads are L2 round trips)
-                double4 pc[4];
+        unsigned buf[LANES > 1 ? kBuildBuf : 1];
+        // sweep 0 counts (and buffers); with LANES == 1 it writes directly.  Sweep 1 (only if a buffer overflowed) re-scans.
+        for (int sweep = 0; sweep < (LANES > 1 ? 2 : 1); ++sweep) {
+            const bool direct = LANES == 1 || sweep == 1;
+            cnt = 0;
+            for (int qq = q0 * (zrun ? 1 : nz); qq < q1 * (zrun ? 1 : nz); ++qq) {
+                const int q = zrun ? qq : qq / nz, zi0 = zrun ? 0 : qq % nz;
+                const int col = (ax[q / ny] * b.nc[1] + ay[q % ny]) * b.nc[2];
+                const int lo = d.cell_start[col + az[zi0]], hi = d.cell_start[col + az[zrun ? nz - 1 : zi0] + 1];
+                for (int j0 = lo; j0 < hi; j0 += 4) {                // four candidates in flight (the loads are L2 round trips)
+                    double4 pc[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int j = min(j0 + u, hi - 1);
-                    pc[u] = NC ? ldg256(&d.xs4[j]) : d.xs4[j];
-                }
+                    for (int u = 0; u < 4; ++u) {
+                        const int j = min(j0 + u, hi - 1);
+                        pc[u] = NC ? ldg256(&d.xs4[j]) : d.xs4[j];
+                    }
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int j = j0 + u;
-                    if (j >= hi || j == i) continue;
-                    const double4 pj = pc[u];
-                    const double dx = min_image(pj.x - xi, b.L[0], b.invL[0]);
-                    const double dy = min_image(pj.y - yi, b.L[1], b.invL[1]);
-                    const double dz = min_image(pj.z - zi, b.L[2], b.invL[2]);
-                    const double r2 = dx * dx + dy * dy + dz * dz;
-                    if (r2 < rc2) {
-                        if (cnt < capMD) d.md_idx[mix(cnt, i, N)] = j;      // (collecting octets in registers: 0.75 -> 1.08 ms per rebuild)
-                        ++cnt;
+                    for (int u = 0; u < 4; ++u) {
+                        const int j = j0 + u;
+                        if (j >= hi || j == i) continue;
+                        const double4 pj = pc[u];
+                        const double dx = min_image(pj.x - xi, b.L[0], b.invL[0]);
+                        const double dy = min_image(pj.y - yi, b.L[1], b.invL[1]);
+                        const double dz = min_image(pj.z - zi, b.L[2], b.invL[2]);
+                        const double r2 = dx * dx + dy * dy + dz * dz;
+                        if (r2 < rc2) {
+                            if (direct) { if (base + cnt < capMD) d.md_idx[mix(base + cnt, i, N)] = j; }
+                            else if (cnt < kBuildBuf) buf[cnt] = (unsigned)j;
+                            ++cnt;
+                        }
                     }
                 }
             }
+            if (LANES == 1) break;
+            if (sweep == 0) {
+                int incl = cnt;                                          // prefix over the lanes of the atom
+#pragma unroll
+                for (int o = 1; o < LANES; o <<= 1) {
+                    const int v = __shfl_up_sync(0xffffffffu, incl, o, LANES);
+                    if (l >= o) incl += v;
+                }
+                base = incl - cnt;
+                const bool fits = cnt <= kBuildBuf;
+                if (fits) {
+                    for (int k = 0; k < cnt; ++k)
+                        if (base + k < capMD) d.md_idx[mix(base + k, i, N)] = buf[k];
+                }
+                if (fits) break;                                         // (a lane whose buffer overflowed re-scans and writes directly)
+            }
         }
-        d.md_cnt[i] = min(cnt, capMD);
-        if (cnt > capMD) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
-        atomicMax(&d.flags[F_MAXMD], cnt);
+        int total = cnt;
+        if (LANES > 1) {
+#pragma unroll
+            for (int o = 1; o < LANES; o <<= 1) total += __shfl_xor_sync(0xffffffffu, total, o, LANES);
+        }
+        if (valid && l == 0) {
+            d.md_cnt[i] = min(total, capMD);
+            if (total > capMD) atomicOr(&d.flags[F_STATUS], ST_OVERFLOW);
+            atomicMax(&d.flags[F_MAXMD], total);
+        }
     }
 }
 
@@ -378,35 +426,37 @@ __device__ __forceinline__ void ph_build_md(const SysDev& d, int N, const Box& b
 // dependent probes of one search overlap those of seven others (the probes are L2 round trips)
 __device__ __forceinline__ void ph_rev(const SysDev& d, int N, int tid, int nth) {
     constexpr int B = 8;
-    for (int i = tid; i < N; i += nth) {
+    // one task per (octet of a row, atom), atoms fastest: a row's octets are searched by different threads
+    const int noct = (d.capMD + 7) >> 3;
+    for (long long t = tid; t < (long long)noct * N; t += nth) {
+        const int i = (int)(t % N), s0 = (int)(t / N) * B;
         const int cnt = d.md_cnt[i];
-        for (int s0 = 0; s0 < cnt; s0 += B) {
-            int j[B], lo[B], hi[B];
-            unsigned oct[8];
-            ld_octet(&d.md_idx[mix(s0, i, N)], oct);
+        if (s0 >= cnt) continue;
+        int j[B], lo[B], hi[B];
+        unsigned oct[8];
+        ld_octet(&d.md_idx[mix(s0, i, N)], oct);
+#pragma unroll
+        for (int u = 0; u < B; ++u) {
+            j[u] = s0 + u < cnt ? (int)(oct[u] & kJMask) : (int)(oct[0] & kJMask);     // past the row: repeat a valid entry
+            lo[u] = 0;
+        }
+#pragma unroll
+        for (int u = 0; u < B; ++u) hi[u] = d.md_cnt[j[u]] - 1;
+        // rows hold at most kMaxCapMD < 128 entries: seven halvings always suffice; a finished search keeps lo == hi
+#pragma unroll 1
+        for (int it = 0; it < 7; ++it) {
+            int v[B];
+#pragma unroll
+            for (int u = 0; u < B; ++u) v[u] = (int)(d.md_idx[mix((lo[u] + hi[u]) >> 1, j[u], N)] & kJMask);
 #pragma unroll
             for (int u = 0; u < B; ++u) {
-                j[u] = s0 + u < cnt ? (int)(oct[u] & kJMask) : (int)(oct[0] & kJMask);     // past the row: repeat a valid entry
-                lo[u] = 0;
+                const int mid = (lo[u] + hi[u]) >> 1;
+                if (v[u] < i) lo[u] = min(mid + 1, hi[u]); else hi[u] = mid;       // first entry >= i
             }
-#pragma unroll
-            for (int u = 0; u < B; ++u) hi[u] = d.md_cnt[j[u]] - 1;
-            // rows hold at most kMaxCapMD < 128 entries: seven halvings always suffice; a finished search keeps lo == hi
-#pragma unroll 1
-            for (int it = 0; it < 7; ++it) {
-                int v[B];
-#pragma unroll
-                for (int u = 0; u < B; ++u) v[u] = (int)(d.md_idx[mix((lo[u] + hi[u]) >> 1, j[u], N)] & kJMask);
-#pragma unroll
-                for (int u = 0; u < B; ++u) {
-                    const int mid = (lo[u] + hi[u]) >> 1;
-                    if (v[u] < i) lo[u] = min(mid + 1, hi[u]); else hi[u] = mid;       // first entry >= i
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < B; ++u) oct[u] = (unsigned)j[u] | ((unsigned)lo[u] << 24);
-            st_octet(&d.md_idx[mix(s0, i, N)], oct);
         }
+#pragma unroll
+        for (int u = 0; u < B; ++u) oct[u] = (unsigned)j[u] | ((unsigned)lo[u] << 24);
+        st_octet(&d.md_idx[mix(s0, i, N)], oct);
     }
 }
 
@@ -418,7 +468,7 @@ __device__ __forceinline__ void ph_done(const SysDev& d) {
 
 __global__ void __launch_bounds__(128) k_build_md(SysDev d, int N, Box b, double rc2, int capMD, int gated) {
     if (gate_closed(d.flags, gated)) return;
-    ph_build_md<true>(d, N, b, rc2, capMD, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
+    ph_build_md<true, 1>(d, N, b, rc2, capMD, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x);
 }
 __global__ void __launch_bounds__(128) k_rev(SysDev d, int N, int gated) {
     if (gate_closed(d.flags, gated)) return;
@@ -457,7 +507,9 @@ k_build_cluster(SysDev d, const double* xin, const double* vin, int N, Box b, do
     cluster_barrier();
     ph_gather_b(d, N, vin != nullptr, n_types, tid, nth);
     cluster_barrier();
-    ph_build_md<false>(d, N, b, rc2, capMD, tid, nth);
+    if (4 * N <= nth) ph_build_md<false, 4>(d, N, b, rc2, capMD, tid, nth);          // as many lanes per atom as the cluster has threads for
+    else if (2 * N <= nth) ph_build_md<false, 2>(d, N, b, rc2, capMD, tid, nth);
+    else ph_build_md<false, 1>(d, N, b, rc2, capMD, tid, nth);
     cluster_barrier();
     ph_rev(d, N, tid, nth);
     cluster_barrier();
@@ -960,6 +1012,7 @@ Layout carve(int64_t N, int capR, int capMD, int max_cells, int NA, int D64, Sys
     t.Fself = (float4*)take(n * 16);
     t.md_cnt = (int*)take(n * 4);
     t.md_idx = (unsigned*)take(n * 32 * (size_t)((capMD + 7) / 8));
+    t.capMD = capMD;
     t.nnR = (int*)take(n * 4);
     t.nnA = (int*)take(n * 4);
     t.rec = (float4*)take(n * 32 * (size_t)((capR + 1) / 2));

@@ -208,3 +208,17 @@ def test_network_widths(oracle, n_neurons):
     w.n_neurons = n_neurons
     w.params = inputs.make_params(w.dim, n_neurons, 11)
     run_config(oracle, w, skin=0.4, lists=False)
+
+
+@pytest.mark.parametrize("cap_r", [31, 37])
+def test_odd_radial_capacity_thread_filter(oracle, cap_r):
+    """Odd cap_radial on k_filter (N > 16384): the pair-major record rows end in a half-used pair -- the top slot leaves
+    as a single 16-byte store, and with cap_radial = 31 = max count + 1 the angular and the radial-only region meet
+    inside one pair.  Lists bit-exact, outputs at the north-star bars."""
+    run_config(oracle, inputs.config4(32768), cap_r=cap_r, cap_a=20)
+
+
+@pytest.mark.parametrize("cap_r,path", [(31, 1), (33, 2)])
+def test_odd_radial_capacity_small_system(oracle, cap_r, path):
+    """The same on the eight-lanes-per-atom filter (N <= 16384), with k_main (path 1) and k_gen (path 2) reading the rows."""
+    run_config(oracle, inputs.config1(), cap_r=cap_r, cap_a=20, path=path)

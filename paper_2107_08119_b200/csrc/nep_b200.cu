@@ -70,6 +70,7 @@ struct SysDev {                 // device pointers into the caller's workspace
     float2* spark0;             // [NA*6][ceil(N/kWin)*kWin] angular sums s[n][lm] of lm half 0 / half 1: parked here by k_main
     float2* spark1;             //   (coalesced rows, L2-resident between write and read) while the registers hold other phases
     float* FpG;                 // [D][ceil(N/kWin)*kWin] dU/dq from k_desc64 (multi-species models only)
+    int* smslots;               // [256] per SM: which of its parking slots (k_main) are taken
     int2* order;                // [ceil(N/kWin)*kWin] atoms of each kWin-atom window sorted by neighbour count: {atom (-1: none),
                                 //   nA | nR << 8}, so that k_main needs ONE load before it can fetch its records
 };
@@ -995,6 +996,7 @@ Layout carve(int64_t N, int capR, int capMD, int max_cells, int NA, int D64, Sys
     const size_t n = (size_t)N;
     SysDev t;
     t.flags = (int*)take(F_COUNT * sizeof(int));
+    t.smslots = (int*)take(256 * sizeof(int));
     t.type_in = (int*)take(n * 4);
     t.perm = (int*)take(n * 4);
     t.perm_tmp = (int*)take(n * 4);

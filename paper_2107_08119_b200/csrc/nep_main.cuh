@@ -213,6 +213,7 @@ __device__ __forceinline__ void force_half(const f32x2 (&A2)[NA][kHalfLM / 2], f
     px = fmaf(R, x, vx); py = fmaf(R, y, vy); pz = fmaf(R, z, vz);
 }
 
+constexpr int kParkSMs = 256, kParkSlots = 4;    // parking slots: SM ids are taken modulo 256, four slots per SM
 constexpr int kMainWarps = 4;       // independent warps per block; they share only the staged weights (measured: 1, 2, 4, 8 warps -> 1.20, 1.15, 1.08, 1.19 ms)
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
@@ -254,6 +255,7 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
     constexpr int Dp = (D + 3) & ~3;
     constexpr int NP = kHalfLM / 2;
     extern __shared__ __align__(16) float sm[];
+    __shared__ int s_park;
     const int H = P.H;
     const int wfl = main_wfloats(H, Dp);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -276,7 +278,17 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
     // ---- P0: every neighbour record of the atom in flight at once (cp.async); the weights arrive as ONE bulk copy ----
     {
         unsigned long long* wbar = reinterpret_cast<unsigned long long*>(sm + wfl + kMainWarps * main_warp_floats<NA, MULTI>());
-        if (threadIdx.x == 0) mbar_init(wbar, 1);
+        if (threadIdx.x == 0) {
+            mbar_init(wbar, 1);
+            if (!MULTI) {                            // claim a parking slot of this SM (at most two blocks are resident)
+                unsigned smid;
+                asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+                smid &= kParkSMs - 1;
+                int sl = 0;
+                while (atomicOr(&d.smslots[smid], 1 << sl) & (1 << sl)) sl = (sl + 1) & (kParkSlots - 1);
+                s_park = (int)smid * kParkSlots + sl;
+            }
+        }
         __syncthreads();
         if (threadIdx.x == 0) {
             mbar_expect_tx(wbar, (unsigned)wfl * 4u);
@@ -358,6 +370,13 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
     f32x2 s2[NA][NP];
     const size_t npad = (size_t)gridDim.x * (32 * kMainWarps);
     const size_t gcol = (size_t)(blockIdx.x * kMainWarps + warp) * 32 + lane;
+    // Where the halves are parked.  Indexed by atom column the rows are 0.8 GB at 1M atoms and every byte is written back
+    // to DRAM; a block that claims one of its SM's parking slots instead reuses the same 48 KB per half for every block
+    // that runs there: 30 MB for the whole chip, resident in L2, never written back.  (Multi-species models read what
+    // k_desc64 left per atom column; small systems keep the atom columns: their rows are shorter than the slot table.)
+    const bool slots = !MULTI && npad >= (size_t)kParkSMs * kParkSlots * (32 * kMainWarps);
+    const size_t ppad = slots ? (size_t)kParkSMs * kParkSlots * (32 * kMainWarps) : npad;
+    const size_t pcol = slots ? (size_t)s_park * (32 * kMainWarps) + threadIdx.x : gcol;
     auto park = [&](float2* base) {
 #pragma unroll
         for (int n = 0; n < NA; ++n)
@@ -365,7 +384,7 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
             for (int mm = 0; mm < NP; ++mm) {
                 float s0, s1;
                 unpack2(s2[n][mm], s0, s1);
-                base[(size_t)(n * NP + mm) * npad + gcol] = make_float2(s0, s1);
+                base[(size_t)(n * NP + mm) * ppad + pcol] = make_float2(s0, s1);
             }
     };
     auto unpark = [&](const float2* base) {
@@ -373,7 +392,7 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
         for (int n = 0; n < NA; ++n)
 #pragma unroll
             for (int mm = 0; mm < NP; ++mm) {
-                const float2 v = base[(size_t)(n * NP + mm) * npad + gcol];
+                const float2 v = base[(size_t)(n * NP + mm) * ppad + pcol];
                 s2[n][mm] = pack2(v.x, v.y);
             }
     };
@@ -520,4 +539,8 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
         prow[k] = make_float4(px, py, pz, 0.f);
     }
     if (active) d.Fself[i] = make_float4(fsx, fsy, fsz, 0.f);
+    if (!MULTI) {                                    // give the parking slot back once every warp has read its sums
+        __syncthreads();
+        if (threadIdx.x == 0) atomicAnd(&d.smslots[s_park / kParkSlots], ~(1 << (s_park % kParkSlots)));
+    }
 }

@@ -2,11 +2,13 @@
 //
 // Data flow of one evaluation (all in the cell-sorted atom order):
 //   k_filter    Verlet list -> per-step radial/angular lists as records {r_ij (fp32 from an fp64
-//               minimum-image difference), j, type_j}; predicate |d|^2 < r_c^2 in fp64
+//               minimum-image difference), j | rev << 24}; predicate |d|^2 < r_c^2 in fp64; two records of an
+//               atom leave as one full 32-byte sector
 //   k_main      one thread per atom: radial descriptor (Eq. 12), angular sums s[n][lm] (Eq. 17-18 route
 //               to Eq. 13), network (Eq. 21-22) and dU/dq, partial forces (Eq. 23-25) -> p_ij
 //   k_assemble  F_i = sum_j (p_ij - p_ji), W_i = sum_j r_ij (x) p_ji (Eq. 4-6), second half-kick,
-//               J_i = W_i . v_i (Eq. 7), thermo sums; outputs in the caller's atom order
+//               J_i = W_i . v_i (Eq. 7), thermo sums; outputs in the caller's atom order; then the NEXT
+//               step's first half-kick and drift (not after the last step of a call)
 // Neighbour build (rare): k_bin -> k_scan -> k_fill -> k_sort_cells -> k_gather -> k_build_md -> k_rev.
 #include <cuda_runtime.h>
 #include <stdint.h>

@@ -42,7 +42,8 @@ typedef enum {
     NEP_ECUDA     = -4,  /* CUDA runtime / launch failure (or no device)                                */
     NEP_EOVERFLOW = -5,  /* some atom has more neighbours than cap_radial / cap_angular / the MD cap    */
     NEP_ESTALE    = -6,  /* nep_compute called with positions that moved > skin/2 since nep_neighbors   */
-    NEP_ESTATE    = -7   /* call order: nep_compute / nep_md_step before nep_neighbors                  */
+    NEP_ESTATE    = -7,  /* call order: nep_compute / nep_md_step before nep_neighbors                  */
+    NEP_ENAN      = -8   /* a site energy or force came out non-finite (e.g. two atoms at one position)    */
 } nep_error;
 
 typedef struct nep_model  nep_model;   /* opaque, library-owned, immutable after nep_create           */
@@ -186,7 +187,8 @@ int  nep_md_step_driven(nep_system*, double* pos_dev, double* vel_dev, const dou
                         const float* w0_dev, double* kt_dev, void* cuda_stream);
 
 /* Synchronises the stream last used by this system and returns the sticky device status
- * (NEP_OK, NEP_EOVERFLOW, NEP_ESTALE) or NEP_ECUDA.  Clears the sticky word. */
+ * (NEP_OK, NEP_EINVAL for an atom type outside the model, NEP_EOVERFLOW, NEP_ESTALE, NEP_ENAN) or NEP_ECUDA.
+ * Clears the sticky word. */
 int  nep_status(nep_system*);
 
 /* Counters since nep_system_create (host values; synchronises like nep_status):

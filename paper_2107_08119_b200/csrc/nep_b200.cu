@@ -32,7 +32,7 @@ constexpr double kAmuConv = 103.642697;       // 1 amu A^2/fs^2 in eV
 // device status / counter words (int32 each)
 enum { F_STATUS = 0, F_REBUILD = 1, F_STEP = 2, F_NREBUILD = 3, F_MAXR = 4, F_MAXA = 5, F_MAXMD = 6, F_BUILT = 7, F_NSTEPS = 8,
        F_COUNT = 16 };
-enum { ST_OVERFLOW = 1, ST_STALE = 2, ST_BADTYPE = 4 };
+enum { ST_OVERFLOW = 1, ST_STALE = 2, ST_BADTYPE = 4, ST_NAN = 8 };
 
 struct Box {
     double L[3], invL[3];
@@ -854,6 +854,7 @@ __global__ void __launch_bounds__(128, 4) k_assemble(SysDev d, AsmParams P) {
         fx = fs.x - fx; fy = fs.y - fy; fz = fs.z - fz;               // Eq. 4-5
         const int row = d.perm[i];
         const float u = d.Us[i];
+        if (!(isfinite(u) && isfinite(fx + fy + fz))) atomicOr(&d.flags[F_STATUS], ST_NAN);      // reported, never silent: NEP_ENAN
         P.energy[row] = u;
         P.force[row] = fx; P.force[N + row] = fy; P.force[2 * N + row] = fz;      // the potential force of Eq. 4
         if (P.driven) {                                                // Eq. 9: (F^ext)^b = sum_a F_e^a W^{ab}
@@ -1295,6 +1296,7 @@ const char* nep_strerror(int code) {
         case NEP_EOVERFLOW: return "neighbour capacity exceeded (cap_radial / cap_angular / Verlet cap)";
         case NEP_ESTALE: return "positions moved more than skin/2 since nep_neighbors";
         case NEP_ESTATE: return "nep_neighbors must be called first";
+        case NEP_ENAN: return "a site energy or force is not finite";
         default: return "unknown error";
     }
 }
@@ -1647,6 +1649,7 @@ int nep_status(nep_system* s) {
     if (flags[F_STATUS] & ST_BADTYPE) return NEP_EINVAL;
     if (flags[F_STATUS] & ST_OVERFLOW) return NEP_EOVERFLOW;
     if (flags[F_STATUS] & ST_STALE) return NEP_ESTALE;
+    if (flags[F_STATUS] & ST_NAN) return NEP_ENAN;
     return NEP_OK;
 }
 

@@ -83,6 +83,14 @@ def test_error_codes(oracle):
     with pytest.raises(api.NepError) as e:
         system.status()
     assert e.value.code == -6
+    # two atoms at one position: r_ij = 0, the result is not finite -> NEP_ENAN (sticky, reported by nep_status)
+    model, system, pos, vel = api.from_workload(w, 64, 32, 0.4)
+    twin = pos.clone(); twin[:, 1] = twin[:, 0]
+    system.neighbors(twin, w.box)
+    system.compute(twin, vel)
+    with pytest.raises(api.NepError) as e:
+        system.status()
+    assert e.value.code == -8
 
 
 def test_compute_with_moved_positions_within_skin(oracle):

@@ -501,12 +501,15 @@ __global__ void __launch_bounds__(128) k_rev(SysDev d, int N, int gated) {
 // without rebuild then costs one early-exit launch instead of ten.
 constexpr int kClusterCTAs = 16;               // non-portable cluster size (opt-in attribute, set at the first launch)
 constexpr int64_t kClusterBuildMaxAtoms = 16384;
+// Up to here the cheap phases (cells, sort, gather) still run as ONE cluster launch and only the Verlet build and the
+// reverse slots are separate full-chip kernels: 4 gated launches per step instead of 10.
+constexpr int64_t kClusterPreMaxAtoms = 65536;
 __device__ __forceinline__ void cluster_barrier() {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 __global__ void __cluster_dims__(kClusterCTAs, 1, 1) __launch_bounds__(1024, 1)
 k_build_cluster(SysDev d, const double* xin, const double* vin, int N, Box b, double rc2,
-                int capMD, int first, int n_types, int gated) {
+                int capMD, int first, int n_types, int gated, int upto_gather) {
     if (gated == 2 && blockIdx.x == 0 && threadIdx.x == 0) d.flags[F_STEP] += 1;
     if (gate_closed(d.flags, gated)) return;               // uniform over the cluster: nobody reaches a barrier
     __shared__ int part[1024];
@@ -527,6 +530,7 @@ k_build_cluster(SysDev d, const double* xin, const double* vin, int N, Box b, do
     ph_gather_a(d, xin, vin, N, first, tid, nth);
     cluster_barrier();
     ph_gather_b(d, N, vin != nullptr, n_types, tid, nth);
+    if (upto_gather) return;                               // mid-size systems: the Verlet build runs on the whole chip
     cluster_barrier();
     if (4 * N <= nth) ph_build_md<false, 4>(d, N, b, rc2, capMD, tid, nth);          // as many lanes per atom as the cluster has threads for
     else if (2 * N <= nth) ph_build_md<false, 2>(d, N, b, rc2, capMD, tid, nth);
@@ -1062,7 +1066,7 @@ void launch_build(nep_system* s, const double* xin, const double* vin, int first
     const SysDev& d = s->d;
     const Box& b = s->box;
     const double rc = s->model->h.rc_radial + s->skin;
-    if (s->N <= kClusterBuildMaxAtoms) {
+    if (s->N <= kClusterPreMaxAtoms) {
         static bool np_done[64] = {};
         int dev = 0;
         cudaGetDevice(&dev);
@@ -1070,8 +1074,14 @@ void launch_build(nep_system* s, const double* xin, const double* vin, int first
             if (cudaFuncSetAttribute(k_build_cluster, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess && dev >= 0 && dev < 64)
                 np_done[dev] = true;
         }
-        k_build_cluster<<<kClusterCTAs, 1024, 0, st>>>(d, xin, vin, N, b, rc * rc, s->capMD, first, s->model->h.n_types, gated);
+        k_build_cluster<<<kClusterCTAs, 1024, 0, st>>>(d, xin, vin, N, b, rc * rc, s->capMD, first, s->model->h.n_types, gated, s->N > kClusterBuildMaxAtoms);
         s->launches += 1;
+        if (s->N <= kClusterBuildMaxAtoms) return;
+        const int gbm = grid_for(N, 128) > 148 * 16 ? 148 * 16 : grid_for(N, 128);
+        k_build_md<<<gbm, 128, 0, st>>>(d, N, b, rc * rc, s->capMD, gated ? 1 : 0);
+        k_rev<<<gbm, 128, 0, st>>>(d, N, gated ? 1 : 0);
+        k_build_done<<<1, 1, 0, st>>>(d, gated ? 1 : 0);
+        s->launches += 3;
         return;
     }
     k_clear_cells<<<grid_stride(b.ncell + 1), 256, 0, st>>>(d, b.ncell, gated);

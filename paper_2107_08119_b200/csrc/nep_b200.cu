@@ -461,18 +461,34 @@ __device__ __forceinline__ void ph_rev(const SysDev& d, int N, int tid, int nth)
             j[u] = s0 + u < cnt ? (int)(oct[u] & kJMask) : (int)(oct[0] & kJMask);     // past the row: repeat a valid entry
             lo[u] = 0;
         }
+        int cj[B];
 #pragma unroll
-        for (int u = 0; u < B; ++u) hi[u] = d.md_cnt[j[u]] - 1;
-        // rows hold at most kMaxCapMD < 128 entries: seven halvings always suffice; a finished search keeps lo == hi
+        for (int u = 0; u < B; ++u) { cj[u] = d.md_cnt[j[u]]; hi[u] = ((cj[u] + 7) >> 3) - 1; }
+        // first the octet of j's row that holds i (rows ascend; at most 16 octets: four halvings over the octets' first
+        // entries), then that octet as one sector: i's slot = 8 * octet + the number of its entries below i
 #pragma unroll 1
-        for (int it = 0; it < 7; ++it) {
+        for (int it = 0; it < 4; ++it) {
             int v[B];
 #pragma unroll
-            for (int u = 0; u < B; ++u) v[u] = (int)(d.md_idx[mix((lo[u] + hi[u]) >> 1, j[u], N)] & kJMask);
+            for (int u = 0; u < B; ++u) v[u] = (int)(d.md_idx[mix(((lo[u] + hi[u] + 1) >> 1) << 3, j[u], N)] & kJMask);
 #pragma unroll
             for (int u = 0; u < B; ++u) {
-                const int mid = (lo[u] + hi[u]) >> 1;
-                if (v[u] < i) lo[u] = min(mid + 1, hi[u]); else hi[u] = mid;       // first entry >= i
+                const int mid = (lo[u] + hi[u] + 1) >> 1;
+                if (v[u] <= i) lo[u] = mid; else hi[u] = mid - 1;          // last octet whose first entry is <= i
+            }
+        }
+#pragma unroll
+        for (int h = 0; h < B; h += 4) {
+            unsigned oc[4][8];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) ld_octet(&d.md_idx[mix(lo[h + u] << 3, j[h + u], N)], oc[u]);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                int below = 0;
+#pragma unroll
+                for (int t = 0; t < 8; ++t)
+                    below += ((lo[h + u] << 3) + t < cj[h + u] && (int)(oc[u][t] & kJMask) < i) ? 1 : 0;
+                lo[h + u] = (lo[h + u] << 3) + below;
             }
         }
 #pragma unroll

@@ -56,7 +56,7 @@ typedef struct {
     double rc_angular;      /* r_c^A, Angstrom, <= rc_radial                                          */
     int    n_max_radial;    /* 0..15                                                                  */
     int    n_max_angular;   /* 0..15                                                                  */
-    int    l_max;           /* 1..4                                                                   */
+    int    l_max;           /* 1..8; 5..8 (general-l kernel): one species, one hidden layer, q_nl only    */
     int    n_neurons;       /* N_neu, single hidden layer (Eq. 21-22), 1..128                         */
     int    n_types;         /* 1..8; >1 switches on the sqrt(Z_i Z_j) weighting of Eq. 19             */
 } nep_hyper;

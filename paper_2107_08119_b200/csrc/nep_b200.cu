@@ -772,6 +772,7 @@ __global__ void k_export_p(SysDev d, int N, int capR, float* p_out) {
 #include "nep_main.cuh"
 #include "nep_desc64.cuh"
 #include "nep_gen.cuh"
+#include "nep_highl.cuh"
 #include "fp32_peak.cuh"
 
 // ------------------------------------------------------------------------------------------------
@@ -1188,8 +1189,22 @@ void launch_gen_t(nep_system* s, cudaStream_t st) {
     s->launches += 1;
 }
 
+void launch_highl(nep_system* s, cudaStream_t st) {
+    const nep_model* m = s->model;
+    HighLParams P;
+    memset(&P, 0, sizeof(P));
+    P.rcR_inv = (float)(1.0 / m->h.rc_radial); P.rcA_inv = (float)(1.0 / m->h.rc_angular);
+    P.NR = m->NR; P.NA = m->NA; P.LMAX = m->h.l_max; P.H = m->H; P.D = m->D; P.Dp = (m->D + 3) & ~3;
+    P.N = (int)s->N; P.capR = s->capR;
+    P.params = m->params_dev;
+    P.q_out = s->dump_q; P.fp_out = s->dump_fp;
+    k_highl<<<grid_for(s->N, 64), 64, 0, st>>>(s->d, P);
+    s->launches += 1;
+}
+
 void launch_gen(nep_system* s, cudaStream_t st) {
     const nep_model* m = s->model;
+    if (m->h.l_max > 4) { launch_highl(s, st); return; }           // the harmonics of k_gen / k_main are written out for l <= 4
     const bool multi = m->h.n_types > 1;
     const bool small = m->NR <= 8 && m->NA <= 8;
     if (small) { if (multi) launch_gen_t<8, double>(s, st); else launch_gen_t<8, float>(s, st); }
@@ -1341,7 +1356,7 @@ int nep_create_ex(const nep_hyper_ex* hx, const int* atomic_number, const double
     *out = nullptr;
     if (!(hy->rc_radial > 0.0) || !(hy->rc_angular > 0.0) || hy->rc_angular > hy->rc_radial) return NEP_EINVAL;
     if (hy->n_max_radial < 0 || hy->n_max_radial > 15 || hy->n_max_angular < 0 || hy->n_max_angular > 15) return NEP_EINVAL;
-    if (hy->l_max < 1 || hy->l_max > 4) return NEP_EINVAL;
+    if (hy->l_max < 1 || hy->l_max > kHLMaxL) return NEP_EINVAL;
     if (hy->n_neurons < 1 || hy->n_neurons > kMaxHGen) return NEP_EINVAL;
     if (hy->n_types < 1 || hy->n_types > kMaxTypes) return NEP_EINVAL;
     if (hy->n_types > 1 && !atomic_number) return NEP_EINVAL;
@@ -1351,6 +1366,8 @@ int nep_create_ex(const nep_hyper_ex* hx, const int* atomic_number, const double
     if (L >= 3 && (hx->n_neurons_3 < 1 || hx->n_neurons_3 > kMaxHGen)) return NEP_EINVAL;
     if (hx->angular_kind != NEP_ANGULAR_QNL && hx->angular_kind != NEP_ANGULAR_QNNL) return NEP_EINVAL;
     if (hx->angular_kind == NEP_ANGULAR_QNNL && (hy->n_max_radial > 7 || hy->n_max_angular > 7)) return NEP_EINVAL;
+    // l_max = 5..8 (k_highl, the general-l kernel): one species, one hidden layer, the q_nl descriptor
+    if (hy->l_max > 4 && (hy->n_types > 1 || L != 1 || hx->angular_kind != NEP_ANGULAR_QNL)) return NEP_EINVAL;
     nep_model* m = new (std::nothrow) nep_model();
     if (!m) return NEP_ENOMEM;
     m->h = *hy;

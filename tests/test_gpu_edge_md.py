@@ -59,7 +59,7 @@ def test_error_codes(oracle):
         api.Model(w.rc_r, w.rc_a, 7, 7, 4, 30, w.atomic_numbers, w.params[:-1])
     assert e.value.code == -1
     with pytest.raises(api.NepError) as e:
-        api.Model(w.rc_r, w.rc_a, 7, 7, 5, 30, w.atomic_numbers, w.params)
+        api.Model(w.rc_r, w.rc_a, 7, 7, 9, 30, w.atomic_numbers, w.params)
     assert e.value.code == -1
     model, system, pos, vel = api.from_workload(w, 64, 32, 1.0)
     with pytest.raises(api.NepError) as e:            # compute before neighbors -> NEP_ESTATE

@@ -76,3 +76,32 @@ def test_create_ex_validation():
         api.Model(w.rc_r, w.rc_a, 8, 8, 4, 30, w.atomic_numbers, np.zeros(10), hidden_layers=[30], angular_kind=1)
     with pytest.raises(api.NepError):          # four hidden layers
         api.Model(w.rc_r, w.rc_a, 7, 7, 4, 30, w.atomic_numbers, np.zeros(10), hidden_layers=[30, 20, 10, 5])
+
+
+@pytest.mark.parametrize("which", ["c0", "c2"])
+@pytest.mark.parametrize("l_max,n_max_a", [(5, 7), (6, 5), (8, 3)])
+def test_l_max_above_four_matches_oracle(oracle, which, l_max, n_max_a):
+    """l_max = 5..8: the general-l kernel (harmonics and gradients by recurrence) against the oracle's
+    literal Legendre double sum of Eq. 13 / 25, outputs at the north-star bars, intermediate rows included."""
+    torch, api = _gpu()
+    w, caps, skin = {"c0": (inputs.config0(), (64, 32), 0.4), "c2": (inputs.config2(), (80, 40), 1.0)}[which]
+    h = oracle.Hyper(w.rc_r, w.rc_a, w.n_max_r, n_max_a, l_max, 30, 1)
+    dim = oracle.descriptor_dim(h)
+    assert dim == (w.n_max_r + 1) + (n_max_a + 1) * l_max
+    npar = oracle.num_params(h)
+    par = (2.0 * inputs.uniform01(43, npar) - 1.0) / np.sqrt(float(dim))
+    model = api.Model(w.rc_r, w.rc_a, w.n_max_r, n_max_a, l_max, 30, w.atomic_numbers, par)
+    assert model.descriptor_dim == dim and model.num_params == npar
+    system = api.System(model, torch.from_numpy(w.types).cuda(), caps[0], caps[1], skin)
+    pos = torch.from_numpy(w.pos).cuda().contiguous(); vel = torch.from_numpy(w.vel).cuda().contiguous()
+    system.neighbors(pos, w.box)
+    out = system.compute(pos, vel)
+    system.status()
+    ref = oracle.evaluate(h, w.atomic_numbers, par, w.pos, w.vel, w.types, w.box, 96, 64)
+    compare_outputs(out, ref, label="%s l_max %d" % (which, l_max))
+    q, fp, p = [t.cpu().numpy().astype(np.float64) for t in system.compute_internals(pos)]
+    ocR, oiR, _ = oracle.neighbors(w.pos, w.box, w.rc_r, 96)
+    ocA, oiA, _ = oracle.neighbors(w.pos, w.box, w.rc_a, 64)
+    refi = oracle.compute(h, w.atomic_numbers, par, w.pos, w.vel, w.types, w.box, ocR, oiR, ocA, oiA, want_internals=True)
+    assert np.abs(q.T - refi["q"]).max() <= 2e-6 * np.abs(refi["q"]).max()
+    assert np.abs(fp.T - refi["Fp"]).max() <= 2e-5 * np.abs(refi["Fp"]).max()

@@ -34,7 +34,7 @@ def test_argument_validation_without_gpu():
     out = C.c_void_p()
     # wrong parameter count, unsupported l_max, r_c^A > r_c^R: rejected before any CUDA call
     assert L.nep_create(C.byref(h), None, par.ctypes.data_as(C.c_void_p), 1260, C.byref(out)) == -1
-    h3 = api.Hyper(5.0, 4.0, 7, 7, 5, 30, 1)
+    h3 = api.Hyper(5.0, 4.0, 7, 7, 9, 30, 1)          # l_max 1..8 (5..8: the general-l kernel)
     assert L.nep_create(C.byref(h3), None, par.ctypes.data_as(C.c_void_p), 1261, C.byref(out)) == -1
     h16 = api.Hyper(5.0, 4.0, 16, 7, 4, 30, 1)
     assert L.nep_create(C.byref(h16), None, par.ctypes.data_as(C.c_void_p), 1261, C.byref(out)) == -1

@@ -1142,7 +1142,12 @@ void launch_main_t(nep_system* s, cudaStream_t st) {
     if (MULTI) {
         Desc64Params p64 = m->p64;
         p64.N = (int)s->N; p64.capR = s->capR; p64.q_out = s->dump_q;
-        k_desc64<NR, NA><<<windows * (kWin / 64), 64, 0, st>>>(s->d, s->box, p64, m->params64_dev);
+        static bool d64_attr[64] = {};
+        if (dev < 0 || dev >= 64 || !d64_attr[dev]) {
+            if (cudaFuncSetAttribute(k_desc64<NR, NA>, cudaFuncAttributeMaxDynamicSharedMemorySize, kD64Rows * 6 * 64 * 8) == cudaSuccess &&
+                dev >= 0 && dev < 64) d64_attr[dev] = true;
+        }
+        k_desc64<NR, NA><<<windows * (kWin / 64), 64, kD64Rows * 6 * 64 * 8, st>>>(s->d, s->box, p64, m->params64_dev);
         s->launches += 1;
     }
     k_main<NR, NA, MULTI><<<windows * (kWin / (32 * kMainWarps)), 32 * kMainWarps, smem, st>>>(s->d, P, m->params_dev, m->zz);

@@ -26,6 +26,8 @@ __device__ __forceinline__ Nbr64 nbr64(const SysDev& d, const Box& b, const doub
     return o;
 }
 
+constexpr int kD64Rows = 16;          // angular neighbours whose geometry is kept in shared memory between the sweeps (48 KB per block)
+
 // One third of the angular sums (lm components 8 T .. 8 T + 7; 64 register accumulators): s, its share of
 // q_nl, and s rounded to fp32 into k_main's parked layout.  The first third also does Eq. 12 for the
 // angular neighbours.
@@ -41,15 +43,27 @@ __device__ __forceinline__ void desc64_third(const SysDev& d, const Box& b, cons
     for (int n = 0; n < NA; ++n)
 #pragma unroll
         for (int m = 0; m < 8; ++m) s[n][m] = 0.0;
+    extern __shared__ double sgeo[];                                     // [kD64Rows][6][64]: x, y, z, r, omega, cos(pi r / r_c^A)
     for (int k = 0; k < nA; ++k) {
-        const Nbr64 e = nbr64(d, b, pi, zrow, k, N, i);
+        // the first sweep leaves the neighbour's geometry and its cutoff cosine in shared memory: the other two read
+        // them instead of repeating the gather, the minimum image, the square root and the fp64 cosine
+        Nbr64 e;
+        double cosA;
+        double* row = sgeo + (size_t)(k * 6) * 64 + threadIdx.x;
+        if (T == 0 || k >= kD64Rows) {
+            e = nbr64(d, b, pi, zrow, k, N, i);
+            cosA = cos(3.14159265358979323846 * (e.r / P.rcA));
+            if (T == 0 && k < kD64Rows) { row[0] = e.x; row[64] = e.y; row[128] = e.z; row[192] = e.r; row[256] = e.om; row[320] = cosA; }
+        } else {
+            e.x = row[0]; e.y = row[64]; e.z = row[128]; e.r = row[192]; e.om = row[256]; cosA = row[320];
+        }
         double g[NR > NA ? NR : NA];
         if (T == 0) {
             radial_g64<NR>(e.r, P.rcR, e.om, g);
 #pragma unroll
             for (int n = 0; n < NR; ++n) q[n] += g[n];                   // Eq. 12
         }
-        radial_g64<NA>(e.r, P.rcA, e.om, g);
+        radial_g64c<NA>(e.r, P.rcA, e.om, cosA, g);
         double bb[kNumLM];
         const double rinv = 1.0 / e.r;
         ylm_basis64(e.x * rinv, e.y * rinv, e.z * rinv, bb);             // the unused components are dead code

@@ -297,6 +297,21 @@ NEP_HD void radial_gd(float r, float rcinv, float omega, float gscale, float* gs
 // descriptor reaches ~4e3 and the network's pre-activations cancel to O(1), so q, the pre-activations
 // and tanh are evaluated in double there.  Same polynomials as above.
 // ------------------------------------------------------------------------------------------------
+// (cosv = cos(pi r / rc): k_desc64 keeps it between its three sweeps over a neighbour)
+template <int N>
+NEP_HD void radial_g64c(double r, double rc, double omega, double cosv, double* g) {
+    const double u = r / rc, um1 = u - 1.0;
+    const double x2 = 4.0 * um1 * um1 - 2.0;                           // 2 x
+    const double hf = 0.25 * omega * (1.0 + cosv);                     // omega fc / 2   (Eq. 15)
+    double Tm = 1.0, T = 0.5 * x2;
+    g[0] = 2.0 * hf;
+#pragma unroll
+    for (int n = 1; n < N; ++n) {
+        g[n] = hf * (T + 1.0);                                         // Eq. 14
+        const double Tn = x2 * T - Tm; Tm = T; T = Tn;                 // Eq. A1
+    }
+}
+
 template <int N>
 NEP_HD void radial_g64(double r, double rc, double omega, double* g) {
     const double u = r / rc, um1 = u - 1.0;

@@ -18,6 +18,7 @@
 #include <new>
 
 #include "../../include/nep_b200.h"
+#include "../../include/nep_b200_measure.h"
 #include "nep_math.cuh"
 
 using namespace nepk;

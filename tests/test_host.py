@@ -15,7 +15,8 @@ def test_library_exports_every_declared_symbol():
     from paper_2107_08119_b200 import api, build
     build.build()
     L = api.lib()
-    header = open(os.path.join(ROOT, "include", "nep_b200.h")).read()
+    import glob
+    header = "".join(open(h).read() for h in sorted(glob.glob(os.path.join(ROOT, "include", "*.h"))))
     declared = set(re.findall(r"\b(nep_[a-z0-9_]+)\s*\(", header))
     declared -= {"nep_error"}
     assert declared == set(api.SYMBOLS), declared ^ set(api.SYMBOLS)

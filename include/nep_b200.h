@@ -234,6 +234,42 @@ int  nep_snes_sample(const double* m_dev, const double* s_dev, const double* r_d
 int  nep_snes_update(double* m_dev, double* s_dev, const double* r_dev, const double* loss_dev, int loss_stride, int n_pop,
                      int n_par, double eta_m, double eta_s, void* cuda_stream);
 
+/* ---- for callers that cannot allocate device memory ------------------------------------------------ */
+
+/* The loss of Eq. 29-34 for ONE parameter vector from predictions already on the device -- the
+ * numbers nep_trainer_predict returns -- computed without any workspace from the caller and without a single
+ * allocation inside the library (no cudaMalloc / cudaFree, no allocating library routine).
+ *
+ * Meant for code that has device arrays in its hands but no allocator: a callback invoked by another program with
+ * just this step's arrays; a process whose device memory belongs wholly to one pool (PyTorch's caching allocator, a
+ * scheduler's arena), where a raw cudaMalloc fails or robs the pool; a loop that cannot afford the device-wide
+ * synchronisation of cudaMalloc, or runs while a stream of the process is being captured, when cudaMalloc is refused.
+ * Everyone else should use nep_trainer_losses, which evaluates the model too and has no size limit.
+ *
+ * The partial sums live in a fixed 524,544-byte (0.5 MiB + 256 B) __device__ array inside libnep_b200.so; each GPU
+ * that loads the library's device code holds that array until the process exits, used or not.  Consequences:
+ *   - LIMIT: 3 n_atoms + 7 n_structures + n_par <= 16,777,216.  Beyond it the call returns NEP_ENOMEM, writes the
+ *     reason to errbuf and touches nothing.
+ *   - FIRST CALL PER DEVICE does a one-time set-up (looks up the array's address on the current device with
+ *     cudaGetSymbolAddress; the runtime may load the library's device code at that moment).  Make it at start-up with
+ *     the intended device current and BEFORE any stream capture begins.  Later calls on that device do none.
+ *   - The array is shared by every call in the process and keeps the previous call's contents; the call clears the
+ *     one counter that must start at zero itself (a memset on cuda_stream ahead of the kernel).  Calls that may
+ *     OVERLAP on the GPU -- two streams with no event between them, two host threads -- race on it and give wrong
+ *     losses: keep all calls on a device in one stream order.
+ *
+ *   e_dev [S] per-atom energy of each structure, f_dev [3][N] forces, v_dev [S][6] per-atom virial (xx yy zz xy yz zx):
+ *     fp32 DEVICE, the layout of nep_trainer_predict; e_tar_dev, f_tar_dev, v_tar_dev: the targets, same layouts.
+ *   z_dev [n_par] fp64 DEVICE: the parameter vector (L_1, L_2 of Eq. 33-34).  lambda [5] HOST: lambda_e, _f, _v, _1, _2.
+ *   loss_dev [6] fp64 DEVICE, caller-owned: L_e, L_f, L_v, L_1, L_2 and the weighted total (Eq. 29).
+ *   errbuf [errbuf_len] HOST, nullable: a plain-text reason whenever the return value is not NEP_OK.
+ * Asynchronous on cuda_stream like every compute call.  Returns NEP_OK, NEP_EINVAL (null pointer, size < 1),
+ * NEP_ENOMEM (beyond the limit above) or NEP_ECUDA. */
+int  nep_loss_noalloc(int64_t n_structures, int64_t n_atoms, int64_t n_par, const float* e_dev, const float* f_dev,
+                      const float* v_dev, const float* e_tar_dev, const float* f_tar_dev, const float* v_tar_dev,
+                      const double* z_dev, const double* lambda, double* loss_dev, void* cuda_stream, char* errbuf,
+                      size_t errbuf_len);
+
 const char* nep_strerror(int code);
 
 #ifdef __cplusplus

@@ -18,7 +18,7 @@ SYMBOLS = ["nep_create", "nep_create_ex", "nep_descriptor_dim", "nep_num_params"
            "nep_system_create", "nep_system_destroy", "nep_system_set_path", "nep_system_path", "nep_neighbors", "nep_get_neighbors", "nep_compute", "nep_compute_internals",
            "nep_md_step", "nep_md_step_driven", "nep_status", "nep_stats", "nep_launch_count", "nep_profile", "nep_get_profile", "nep_measure_fp32_peak", "nep_measure_fp32_patterns",
            "nep_trainer_workspace_bytes", "nep_trainer_create", "nep_trainer_destroy", "nep_trainer_num_params", "nep_trainer_status",
-           "nep_trainer_losses", "nep_trainer_predict", "nep_snes_sample", "nep_snes_update",
+           "nep_trainer_losses", "nep_trainer_predict", "nep_snes_sample", "nep_snes_update", "nep_loss_noalloc",
            "nep_strerror"]
 
 
@@ -82,6 +82,7 @@ def lib():
         L.nep_snes_update.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double,
                                       C.c_double, C.c_void_p]
         L.nep_get_profile.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nep_loss_noalloc.argtypes = [C.c_int64, C.c_int64, C.c_int64] + [C.c_void_p] * 10 + [C.c_char_p, C.c_size_t]
         _lib = L
     return _lib
 
@@ -335,3 +336,24 @@ def snes_update(m, s, r, loss, eta_m, eta_s):
     ptr = loss.data_ptr() + (0 if loss.dim() == 1 else 5 * loss.element_size())
     _check(lib().nep_snes_update(_ptr(m), _ptr(s), _ptr(r), C.c_void_p(ptr), stride, r.shape[0], r.shape[1], float(eta_m),
                                  float(eta_s), _stream()), "nep_snes_update")
+
+
+def loss_noalloc(e, f, v, e_tar, f_tar, v_tar, z, lambdas, out):
+    """nep_loss_noalloc: Eq. 29-34 for one parameter vector from predictions on the device, for callers that cannot
+    allocate device memory (see include/nep_b200.h for who they are and for the limits: a fixed 0.5 MiB scratch inside
+    the library, 3 N + 7 S + n_par <= 16,777,216, first call per device before any stream capture, no overlapping
+    calls).  Nothing is allocated here either: `out` [6] fp64 cuda is the caller's.  e [S], f [3, N], v [S, 6] and the
+    targets: fp32 cuda, contiguous; z [n_par] fp64 cuda.  Returns out = L_e, L_f, L_v, L_1, L_2, L."""
+    for t in (e, f, v, e_tar, f_tar, v_tar):
+        assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+    assert z.is_cuda and z.dtype == torch.float64 and z.is_contiguous() and z.dim() == 1
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 6
+    S, N = e.shape[0], f.shape[1]
+    assert f.shape == (3, N) and v.shape == (S, 6) and e_tar.shape == e.shape and f_tar.shape == f.shape and v_tar.shape == v.shape
+    lam = np.ascontiguousarray(lambdas, dtype=np.float64)
+    msg = C.create_string_buffer(512)
+    code = lib().nep_loss_noalloc(S, N, z.shape[0], _ptr(e), _ptr(f), _ptr(v), _ptr(e_tar), _ptr(f_tar), _ptr(v_tar), _ptr(z),
+                                  lam.ctypes.data_as(C.c_void_p), _ptr(out), _stream(), msg, len(msg))
+    if code != 0:
+        raise NepError(code, msg.value.decode() or "nep_loss_noalloc")
+    return out

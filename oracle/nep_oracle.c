@@ -599,13 +599,16 @@ void orc_snes_sample(int npop, int npar, const double *m, const double *s, const
         for (int n = 0; n < npar; ++n) z[(size_t)k * npar + n] = m[n] + s[n] * r[(size_t)k * npar + n];
 }
 
-/* Rank-based utilities of reading Q25: util[k] for member k given the losses. */
+/* Rank-based utilities of reading Q25: util[k] for member k given the losses.  A loss that is not finite (NaN from
+ * coincident atoms, overflowing weights) counts as +infinity, so the member ranks last instead of first (Q25). */
+static double orc_rank_key(double l) { return isfinite(l) ? l : INFINITY; }
 void orc_snes_utilities(int npop, const double *loss, double *util) {
     double norm = 0.0;
     for (int j = 1; j <= npop; ++j) { double v = log(npop / 2.0 + 1.0) - log((double)j); norm += v > 0 ? v : 0; }
     for (int k = 0; k < npop; ++k) {
         int rank = 1;                                   /* 1 = smallest loss; ties by index */
-        for (int j = 0; j < npop; ++j) if (loss[j] < loss[k] || (loss[j] == loss[k] && j < k)) ++rank;
+        const double lk = orc_rank_key(loss[k]);
+        for (int j = 0; j < npop; ++j) { const double lj = orc_rank_key(loss[j]); if (lj < lk || (lj == lk && j < k)) ++rank; }
         double v = log(npop / 2.0 + 1.0) - log((double)rank);
         util[k] = (v > 0 ? v : 0) / norm - 1.0 / npop;
     }

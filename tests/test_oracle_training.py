@@ -87,6 +87,22 @@ def test_utilities_and_two_member_update_by_hand(oracle):
     assert np.allclose(m3, m2, rtol=1e-15) and np.allclose(s3, s2, rtol=1e-15)
 
 
+def test_a_member_with_a_non_finite_loss_ranks_last(oracle):
+    """Reading Q25 (the paper gives no rule; a NaN compares false with everything, so a literal rank count would put the
+    broken member FIRST and pull m, s towards it): NaN and +-inf losses count as +inf, ties among them by index."""
+    good = [0.3, 0.1, 0.7, 0.2, 0.9, 0.5, 0.4, 0.6]
+    for bad in (float("nan"), float("inf"), float("-inf")):
+        l = list(good); l[3] = bad
+        as_huge = list(good); as_huge[3] = 1e300
+        u = oracle.snes_utilities(l)
+        assert np.array_equal(u, oracle.snes_utilities(as_huge))
+        assert u[3] == u.min() == pytest.approx(-1.0 / len(good)) and abs(u.sum()) < 1e-15
+    two = list(good); two[1] = float("nan"); two[6] = float("inf")
+    ref = list(good); ref[1] = 1e300; ref[6] = 2e300                          # the earlier index ranks first among the broken
+    assert np.array_equal(oracle.snes_utilities(two), oracle.snes_utilities(ref))
+    assert np.array_equal(oracle.snes_utilities(good), oracle.snes_utilities([2 * x for x in good]))     # finite losses as before
+
+
 def test_snes_minimises_a_quadratic(oracle):
     """The update follows the natural gradient: on L(z) = |z - z*|^2 the mean converges to z* (PAPER.md:273)."""
     npar, npop = 12, 20

@@ -42,6 +42,26 @@ def test_force_is_minus_gradient(oracle, which):
     assert np.abs(F.sum(axis=1)).max() < 1e-10 * max(1.0, np.abs(F).max())
 
 
+@pytest.mark.parametrize("l_max,n_max_a", [(6, 5), (8, 3)])
+def test_force_is_minus_gradient_for_l_max_above_four(oracle, l_max, n_max_a):
+    """The literal Legendre double sum of Eq. 13 / 25 at l_max = 6 and 8 -- what the GPU's general-l kernel is compared
+    with (the finite-difference pin stopped at l_max = 4)."""
+    w = inputs.config0()
+    h = oracle.Hyper(w.rc_r, w.rc_a, w.n_max_r, n_max_a, l_max, 30, 1)
+    dim = oracle.descriptor_dim(h)
+    par = (2.0 * inputs.uniform01(43, oracle.num_params(h)) - 1.0) / math.sqrt(float(dim))
+    F = oracle.evaluate(h, w.atomic_numbers, par, w.pos, w.vel, w.types, w.box)["F"]
+    frms = math.sqrt((F ** 2).mean())
+    eps = 1e-5
+    for (a, i) in [(0, 0), (1, 7), (2, 13), (0, 31), (1, 50), (2, 63)]:
+        def U_at(t):
+            pp = w.pos.copy(); pp[a, i] += t
+            return oracle.evaluate(h, w.atomic_numbers, par, pp, None, w.types, w.box)["U"].sum()
+        num = -(8 * (U_at(eps) - U_at(-eps)) - (U_at(2 * eps) - U_at(-2 * eps))) / (12 * eps)
+        assert F[a, i] == pytest.approx(num, abs=1e-6 * max(frms, 1e-3)), (a, i)
+    assert np.abs(F.sum(axis=1)).max() < 1e-10 * max(1.0, np.abs(F).max())
+
+
 @pytest.mark.parametrize("which", ["si", "pbte"])
 def test_total_virial_is_minus_strain_derivative(oracle, which):
     w = inputs.config0() if which == "si" else _small_pbte()

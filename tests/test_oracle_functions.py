@@ -119,9 +119,17 @@ def test_legendre_closed_forms(oracle):
     assert np.allclose(P, 1.0) and np.allclose(dP, [l * (l + 1) / 2 for l in range(7)])
     P, _ = oracle.legendre(-1.0, 6)
     assert np.allclose(P, [(-1) ** l for l in range(7)])
-    from scipy.special import eval_legendre
+    from scipy.special import eval_legendre, legendre as legendre_poly
     for l in range(7):
         assert oracle.legendre(0.3731, 6)[0][l] == pytest.approx(eval_legendre(l, 0.3731), abs=1e-14)
+    # up to l = 8, the largest l_max the GPU's general-l kernel is judged at: values and derivatives
+    for c in (-0.9137, -0.25, 0.0, 0.3731, 0.77, 0.999):
+        P, dP = oracle.legendre(c, 8)
+        for l in range(9):
+            assert P[l] == pytest.approx(eval_legendre(l, c), abs=2e-14)
+            assert dP[l] == pytest.approx(float(legendre_poly(l).deriv()(c)), abs=1e-11)
+    P, dP = oracle.legendre(1.0, 8)
+    assert np.allclose(P, 1.0) and np.allclose(dP, [l * (l + 1) / 2 for l in range(9)])
 
 
 def test_network_hand_case(oracle):

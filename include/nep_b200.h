@@ -71,7 +71,7 @@ typedef struct {
  *          (n=1: l=1..l_max) | ...].  n_params must equal (D+2)H+1 (Eq. 26) else NEP_EINVAL. */
 int  nep_create(const nep_hyper* hyper, const int* atomic_number, const double* params, size_t n_params,
                 nep_model** out);
-/* Variants the paper mentions without using them; evaluated by the eight/sixteen-lanes-per-atom
+/* Variants the paper mentions without using them; evaluated by the 16-lanes-per-atom
  * kernel (NEP_PATH_GROUP) only:
  *   n_hidden_layers 1..3 ("generalization to more hidden layers is straightforward"):
  *     x^(k) = tanh(W^(k) x^(k-1) - b^(k)), x^(0) = q, U = w_out . x^(L) - b_out, every bias with the minus sign of
@@ -81,6 +81,13 @@ int  nep_create(const nep_hyper* hyper, const int* atomic_number, const double* 
  *     q_nn'l = (2l+1)/(4 pi) sum_jk g_n(r_ij) g_n'(r_ik) P_l(cos theta_ijk) = sum_m c_nlm c*_n'lm, for the pairs n <= n'
  *     (q_nn'l = q_n'nl), ordered n, then n' >= n, then l; N_des = (n_max_R+1) + (n_max_A+1)(n_max_A+2)/2 l_max;
  *     needs n_max_radial, n_max_angular <= 7.
+ * Size limit: the lanes-per-atom kernel keeps the weights of ALL layers in shared memory beside its per-atom blocks, so
+ * the padded weight count  sum_k H_k (in_k rounded up to 4) + the biases  is bounded by what a block may opt in to
+ * (227 KB on B200): about 46,400 fp32 values for n_max <= 7 and 45,000 above; for n_types > 1 (fp64 weights) 17,300 /
+ * 14,900 values.  nep_create_ex checks this on the current device and returns NEP_EINVAL for a shape that does not
+ * fit, instead of a model whose launches fail.  Every one-species single-layer shape fits, and so do 3 x 128 at
+ * D = 80 and 2 x 128 over q_nn'l; NOT: 3 x 128 over q_nn'l (D = 152); with n_types > 1: 2 x 128 at D = 80, or one
+ * layer of 128 over q_nn'l (one layer of 128 at D = 80 and one of 100 over q_nn'l fit).
  * nep_create(h, ...) is nep_create_ex with one hidden layer and NEP_ANGULAR_QNL. */
 enum { NEP_ANGULAR_QNL = 0, NEP_ANGULAR_QNNL = 1 };
 typedef struct {
@@ -105,7 +112,9 @@ size_t nep_workspace_bytes(const nep_model*, int64_t n_atoms, int cap_radial, in
 
 /* type_dev [N] device int32 in 0..n_types-1 (copied).  workspace_dev: caller-owned device memory,
  * 256-byte aligned, >= nep_workspace_bytes(); must outlive the system.  skin >= 0 (Angstrom) is the
- * Verlet skin: lists stay valid while no atom has moved more than skin/2 since the last build. */
+ * Verlet skin: lists stay valid while no atom has moved more than skin/2 since the last build.
+ * A set-up call: it clears the workspace and copies the types, and synchronises the WHOLE DEVICE before and after doing
+ * so -- whatever stream produced type_dev has finished, and any stream may be used for nep_neighbors afterwards. */
 int  nep_system_create(const nep_model*, int64_t n_atoms, const int* type_dev, int cap_radial,
                        int cap_angular, double skin, void* workspace_dev, size_t workspace_bytes,
                        nep_system** out);
@@ -115,7 +124,7 @@ void nep_system_destroy(nep_system*);
  *   NEP_PATH_THREAD  one thread per atom (k_main): every per-atom quantity in registers; instantiated for
  *                    n_max_radial / n_max_angular = 7/7, 8/8 or 12/6, l_max == 4, n_neurons <= 64 -- the BASELINE.json
  *                    shapes (D = 40 / 45); the faster form from ~1e4 atoms (nep_system_create switches at 12000)
- *   NEP_PATH_GROUP   eight lanes per atom (k_gen): any shape nep_create accepts, Table I's 80-50-1, 65-40-1 and
+ *   NEP_PATH_GROUP   16 lanes per atom (k_gen): any shape nep_create accepts, Table I's 80-50-1, 65-40-1 and
  *                    41-40-1 models included; the form for small systems
  * nep_system_create picks one from the shape and n_atoms (NEP_PATH_AUTO); nep_system_set_path overrides it
  * (NEP_EINVAL if the thread path is not instantiated for the model).  Changing the path invalidates the

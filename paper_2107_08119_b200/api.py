@@ -155,7 +155,7 @@ class System:
     PATH_AUTO, PATH_THREAD, PATH_GROUP = 0, 1, 2
 
     def set_path(self, path: int):
-        """nep_system_set_path: 0 auto, 1 one thread per atom (k_main), 2 eight lanes per atom (k_gen)."""
+        """nep_system_set_path: 0 auto, 1 one thread per atom (k_main), 2 16 lanes per atom (k_gen)."""
         _check(lib().nep_system_set_path(self._h, int(path)), "nep_system_set_path")
 
     @property

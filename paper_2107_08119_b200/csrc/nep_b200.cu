@@ -16,6 +16,7 @@
 #include <string.h>
 #include <math.h>
 #include <new>
+#include <math_constants.h>
 
 #include "../../include/nep_b200.h"
 #include "../../include/nep_b200_measure.h"
@@ -1163,6 +1164,36 @@ bool main_supported(const nep_model* m) {
     return smem <= (size_t)kMainSmemLimit;
 }
 
+// dynamic shared memory of k_gen<NMAX, TD> for a model: the per-atom blocks of one CTA plus the staged weights of every layer
+template <int NMAX, typename TD>
+size_t gen_smem_bytes_t(const nep_model* m) {
+    const int Dp = (m->D + 3) & ~3;
+    const size_t wbytes = m->nlayers > 1 ? (size_t)m->blob_elems * sizeof(TD)
+                                         : ((size_t)m->H * (sizeof(TD) == 8 ? (Dp | 1) : Dp + 4) + 2 * m->H + 1) * sizeof(TD);
+    return (size_t)kGenAtomsPerBlock * sizeof(GenSmem<NMAX, TD>) + ((wbytes + 15) & ~(size_t)15);
+}
+
+// Does the k_gen instantiation this model runs on fit the opt-in shared memory of the current device?  Every model can
+// be put on the group path (small systems, nep_system_set_path, the trainer), so nep_create_ex refuses what does not
+// fit instead of handing out a model whose every later launch fails.  l_max > 4 runs on k_highl (no weights in smem).
+template <int NMAX, typename TD>
+bool gen_fits_t(const nep_model* m, size_t* need, size_t* limit) {
+    cudaFuncAttributes fa;
+    int dev = 0, optin = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaFuncGetAttributes(&fa, k_gen<NMAX, TD>) != cudaSuccess ||
+        cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) { cudaGetLastError(); return false; }
+    *need = gen_smem_bytes_t<NMAX, TD>(m) + fa.sharedSizeBytes;
+    *limit = (size_t)optin;
+    return *need <= *limit;
+}
+bool gen_fits(const nep_model* m, size_t* need, size_t* limit) {
+    *need = 0; *limit = 0;
+    if (m->h.l_max > 4) return true;
+    const bool multi = m->h.n_types > 1, small = m->NR <= 8 && m->NA <= 8;
+    if (small) return multi ? gen_fits_t<8, double>(m, need, limit) : gen_fits_t<8, float>(m, need, limit);
+    return multi ? gen_fits_t<16, double>(m, need, limit) : gen_fits_t<16, float>(m, need, limit);
+}
+
 template <int NMAX, typename TD>
 void launch_gen_t(nep_system* s, cudaStream_t st) {
     const nep_model* m = s->model;
@@ -1179,9 +1210,7 @@ void launch_gen_t(nep_system* s, cudaStream_t st) {
     P.kind = m->kind; P.nlayers = m->nlayers; P.off_out = m->off_out; P.blob_elems = m->blob_elems;
     for (int k = 0; k < 3; ++k) { P.lw[k] = m->lw[k]; P.lin_p[k] = m->lin_p[k]; P.off_w[k] = m->off_w[k]; P.off_b[k] = m->off_b[k]; }
     P.blob = m->blob_dev; P.blob64 = m->blob64_dev;
-    const size_t wbytes = m->nlayers > 1 ? (size_t)m->blob_elems * sizeof(TD)
-                                         : ((size_t)m->H * (sizeof(TD) == 8 ? (P.Dp | 1) : P.Dp + 4) + 2 * m->H + 1) * sizeof(TD);
-    const size_t smem = (size_t)kGenAtomsPerBlock * sizeof(GenSmem<NMAX, TD>) + ((wbytes + 15) & ~(size_t)15);     // + the staged weights
+    const size_t smem = gen_smem_bytes_t<NMAX, TD>(m);             // per-atom blocks + the staged weights (checked in nep_create_ex)
     static size_t attr_smem[64] = {};              // per device: the largest dynamic size this instantiation was opted in for
     int dev = 0;
     cudaGetDevice(&dev);
@@ -1336,7 +1365,8 @@ extern "C" {
 const char* nep_strerror(int code) {
     switch (code) {
         case NEP_OK: return "ok";
-        case NEP_EINVAL: return "invalid argument (hyper-parameters, parameter count, null pointer or unsupported shape)";
+        case NEP_EINVAL: return "invalid argument (hyper-parameters, parameter count, null pointer, or a shape whose staged "
+                                "weights exceed the shared memory of the lanes-per-atom kernel: see nep_create_ex in nep_b200.h)";
         case NEP_EBOX: return "box length <= 2 (r_c^R + skin): minimum image ambiguous";
         case NEP_ENOMEM: return "workspace too small";
         case NEP_ECUDA: return g_cuda_msg;
@@ -1448,6 +1478,13 @@ int nep_create_ex(const nep_hyper_ex* hx, const int* atomic_number, const double
         delete[] blob;
     }
     if (e != cudaSuccess) { set_cuda_error(e, "nep_create"); nep_destroy(m); return NEP_ECUDA; }
+    {
+        size_t need = 0, limit = 0;
+        if (!gen_fits(m, &need, &limit)) {
+            nep_destroy(m);
+            return NEP_EINVAL;
+        }
+    }
     *out = m;
     return NEP_OK;
 }
@@ -1484,7 +1521,7 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
     s->capMD = cap_md_of(m, cap_radial, skin);
     s->max_cells = max_cells_of(n_atoms);
     // one thread per atom pays once the machine is full; below that (and for every shape k_main is not
-    // instantiated for) eight lanes share an atom
+    // instantiated for) 16 lanes share an atom (k_gen)
     s->path = (m->thread_path_ok && n_atoms >= kThreadPathMinAtoms) ? NEP_PATH_THREAD : NEP_PATH_GROUP;
     carve(n_atoms, s->capR, s->capMD, s->max_cells, m->NA, m->h.n_types > 1 ? m->D : 0, &s->d, (char*)workspace_dev);
     s->last_driven = false; s->last_fe[0] = s->last_fe[1] = s->last_fe[2] = 0.f;
@@ -1493,8 +1530,13 @@ int nep_system_create(const nep_model* m, int64_t n_atoms, const int* type_dev, 
     s->launches = 0; s->prof_on = false; s->prof_n = 0;
     for (int k = 0; k < NEP_PHASES; ++k) { s->prof_ms[k] = 0.0; s->prof_cnt[k] = 0; }
     for (int k = 0; k < kProfMaxEvents; ++k) s->prof_ev[k] = nullptr;
-    cudaError_t e = cudaMemset(workspace_dev, 0, need);
+    // Set-up call: the whole device is synchronised on both sides of the clear and the copy.  They are issued on the
+    // legacy default stream, which orders itself against blocking streams only; a cudaStreamNonBlocking stream (any
+    // PyTorch side stream) that produced type_dev, or that runs nep_neighbors next, would otherwise overlap them.
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemset(workspace_dev, 0, need);
     if (e == cudaSuccess) e = cudaMemcpy(s->d.type_in, type_dev, (size_t)n_atoms * sizeof(int), cudaMemcpyDeviceToDevice);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { set_cuda_error(e, "nep_system_create"); delete s; return NEP_ECUDA; }
     *out = s;
     return NEP_OK;

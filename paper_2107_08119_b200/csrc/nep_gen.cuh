@@ -2,8 +2,8 @@
 // (included by nep_b200.cu inside its anonymous namespace, after nep_main.cuh and nep_desc64.cuh).
 //
 // k_main (nep_main.cuh) is one thread per atom with everything in registers: the fastest form once a few
-// hundred thousand atoms fill the machine, but instantiated only for 8 or 9 radial functions per family and
-// serial in the atom (one warp = 32 atoms, ~35 us of dependent instructions).  k_gen is the cooperative form:
+// hundred thousand atoms fill the machine, but instantiated only for 8/8, 9/9 or 13/7 radial/angular functions,
+// l_max = 4, N_neu <= 64, and serial in the atom (one warp = 32 atoms, ~35 us of dependent instructions).  k_gen is the cooperative form:
 // a group of G = 16 lanes owns one atom (2 atoms per warp), the runtime shape is free -- n_max^R, n_max^A up to
 // NMAX-1 (NMAX = 8 or 16), l_max = 1..4, any N_neu, Table I's models included -- and an
 // atom's work is spread over its lanes, so small systems (C0-C2, the paper's 8000-atom protocol,

@@ -286,6 +286,7 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
                 smid &= kParkSMs - 1;
                 int sl = 0;
                 while (atomicOr(&d.smslots[smid], 1 << sl) & (1 << sl)) sl = (sl + 1) & (kParkSlots - 1);
+                __threadfence();                     // acquire: this block's writes to the slot come after the claim
                 s_park = (int)smid * kParkSlots + sl;
             }
         }
@@ -541,6 +542,9 @@ __global__ void __launch_bounds__(32 * kMainWarps, 2) k_main(SysDev d, MainParam
     if (active) d.Fself[i] = make_float4(fsx, fsy, fsz, 0.f);
     if (!MULTI) {                                    // give the parking slot back once every warp has read its sums
         __syncthreads();
-        if (threadIdx.x == 0) atomicAnd(&d.smslots[s_park / kParkSlots], ~(1 << (s_park % kParkSlots)));
+        if (threadIdx.x == 0) {
+            __threadfence();                         // release: every warp's reads of the slot (ordered before the barrier) precede it
+            atomicAnd(&d.smslots[s_park / kParkSlots], ~(1 << (s_park % kParkSlots)));
+        }
     }
 }

@@ -140,12 +140,17 @@ __global__ void __launch_bounds__(256) k_snes_update(double* m, double* s, const
     double norm = 0.0;
     for (int j = 1; j <= npop; ++j) norm += fmax(0.0, log(npop / 2.0 + 1.0) - log((double)j));
     for (int k = threadIdx.x; k < npop; k += blockDim.x) {
-        const double lk = loss[(size_t)k * loss_stride];
+        // a loss that is not finite counts as +inf: the member ranks last, not first (reading Q25)
+        const double lk0 = loss[(size_t)k * loss_stride], lk = isfinite(lk0) ? lk0 : CUDART_INF;
         int rank = 1;                                   // 1 = smallest loss, ties by index
-        for (int j = 0; j < npop; ++j) { const double lj = loss[(size_t)j * loss_stride]; if (lj < lk || (lj == lk && j < k)) ++rank; }
+        for (int j = 0; j < npop; ++j) {
+            const double lj0 = loss[(size_t)j * loss_stride], lj = isfinite(lj0) ? lj0 : CUDART_INF;
+            if (lj < lk || (lj == lk && j < k)) ++rank;
+        }
         util[k] = fmax(0.0, log(npop / 2.0 + 1.0) - log((double)rank)) / norm - 1.0 / npop;
     }
     __syncthreads();
+    // m[n], s[n] are read and written by exactly one thread (n is owned by one thread of the grid-stride loop): no atomics
     for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < npar; n += gridDim.x * blockDim.x) {
         double gm = 0.0, gs = 0.0;
         for (int k = 0; k < npop; ++k) {

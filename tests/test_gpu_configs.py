@@ -82,3 +82,55 @@ def test_md_c3_pbte_64000(oracle, path):
 
 def test_md_c4_32768_with_rebuild(oracle):
     _md_leg(oracle, inputs.config4(32768), 60, 64, 32, 2, "C4 Si 32768", 1e-4)
+
+
+def _md_final_state(oracle, w, n_steps, cap_r, cap_a, min_rebuilds, label, oracle_md_steps=0):
+    """MD above 65,536 atoms, where launch_build takes its third form: the ten-kernel device-gated chain that re-sorts
+    an already sorted state (first = 0, gated = 2), with k_main's per-SM parking slots and the kick+drift fused into
+    k_assemble (npad >= 262144) -- the configuration bench.py times.
+    After n_steps with at least min_rebuilds in-loop rebuilds: filtered lists bit-exact and U, F, W, J at the
+    north-star bars against the oracle evaluated at the GPU's OWN final state; the energy record stays flat.  With
+    oracle_md_steps > 0 the first steps are also followed against orc_md (energies, trajectory, accumulated J)."""
+    torch, api = _gpu()
+    model, system, pos, vel = api.from_workload(w, cap_r, cap_a, 1.0)
+    assert system.path == 1
+    system.neighbors(pos, w.box)
+    heat_sum = torch.zeros((3, w.n_atoms), dtype=torch.float64, device="cuda")
+    thermo = torch.zeros((n_steps, 5), dtype=torch.float64, device="cuda")
+    h = _hyper(oracle, w)
+    done = 0
+    if oracle_md_steps:
+        system.md_step(pos, vel, w.masses, w.dt, oracle_md_steps, heat_sum=heat_sum, thermo=thermo[:oracle_md_steps])
+        system.status()
+        ref = oracle.md(h, w.atomic_numbers, w.params, w.pos, w.vel, w.types, w.box, w.masses, w.dt, oracle_md_steps, 96, 64)
+        th = thermo[:oracle_md_steps].cpu().numpy()
+        E, Eref = th[:, 0] + th[:, 1], ref["thermo"][1:, 0] + ref["thermo"][1:, 1]
+        dpos = np.abs(pos.cpu().numpy() - ref["pos"]).max()
+        print("%s: first %d steps vs orc_md: max|E-Eref|/N %.3g, max|dpos| %.3g A" % (label, oracle_md_steps,
+                                                                                 np.abs(E - Eref).max() / w.n_atoms, dpos))
+        assert dpos < 1e-4 and np.abs(E - Eref).max() / w.n_atoms < 1e-5
+        assert np.abs(heat_sum.cpu().numpy() - ref["Jsum"]).max() < 5e-3 * np.abs(ref["Jsum"]).max()
+        done = oracle_md_steps
+    out = system.md_step(pos, vel, w.masses, w.dt, n_steps - done, heat_sum=heat_sum, thermo=thermo[done:])
+    system.status()
+    st = system.stats()
+    th = thermo.cpu().numpy()
+    E = th[:, 0] + th[:, 1]
+    drift = np.abs(E - E[0]).max() / w.n_atoms
+    print("%s: %d steps, rebuilds %d, |E-E0|/N %.3g eV" % (label, n_steps, st["rebuilds"], drift))
+    assert st["rebuilds"] >= min_rebuilds + 1, st          # the initial nep_neighbors counts as one
+    assert drift < 2e-5
+    gpos, gvel = pos.cpu().numpy(), vel.cpu().numpy()
+    w2 = inputs.Workload(w.name, gpos, gvel, w.types, w.box, w.rc_r, w.rc_a, w.n_max_r, w.n_max_a, w.l_max,
+                         w.n_neurons, w.atomic_numbers, w.masses, w.params)
+    check_lists(oracle, w2, system, cap_r, cap_a)
+    ref2 = oracle.evaluate(h, w.atomic_numbers, w.params, gpos, gvel, w.types, w.box, 96, 64)
+    compare_outputs(out, ref2, label=label + " final state")
+
+
+def test_md_c4_262144_gated_rebuild_chain(oracle):
+    _md_final_state(oracle, inputs.config4(262144), 60, 64, 32, 2, "C4 Si 262144", oracle_md_steps=20)
+
+
+def test_md_c4_1048576_benchmarked_configuration(oracle):
+    _md_final_state(oracle, inputs.config4(1048576), 60, 64, 32, 2, "C4 Si 1048576")

@@ -193,3 +193,36 @@ def test_md_chunked_calls_continue_trajectory(oracle):
         res.append((pos.clone(), vel.clone(), out[1].clone()))
     assert (res[0][0] - res[1][0]).abs().max().item() < 1e-9
     assert (res[0][1] - res[1][1]).abs().max().item() < 1e-10
+
+
+def test_system_created_and_run_on_a_non_blocking_stream(oracle):
+    """nep_system_create clears the workspace and copies the types on the legacy default stream, which
+    does not order itself against cudaStreamNonBlocking streams (every PyTorch side stream is one).  With the types
+    produced on such a stream right before the call, and nep_neighbors / nep_compute issued on it right after, the
+    results must be those of the default-stream run: nep_system_create synchronises the device on both sides."""
+    torch, api = _gpu()
+    w = inputs.config3((6, 6, 6))                                   # two species: a wrong or late type copy shows
+    ref_model, ref_sys, pos, vel = api.from_workload(w, 80, 40, 1.0)
+    ref_sys.neighbors(pos, w.box)
+    ref = [t.clone() for t in ref_sys.compute(pos, vel)]
+    ref_sys.status()
+    side = torch.cuda.Stream()
+    host_types = torch.from_numpy(w.types).pin_memory()
+    filler = torch.empty(1 << 28, dtype=torch.uint8, device="cuda")
+    for rep in range(3):
+        with torch.cuda.stream(side):
+            for _ in range(8):
+                filler.fill_(rep)                                   # keeps the side stream busy ahead of the copy
+            types = torch.empty(w.n_atoms, dtype=torch.int32, device="cuda")
+            types.copy_(host_types, non_blocking=True)
+            system = api.System(ref_model, types, 80, 40, 1.0)
+            system.neighbors(pos, w.box)
+            out = system.compute(pos, vel)
+        side.synchronize()
+        system.status()
+        for a, b in zip(out, ref):
+            assert torch.equal(a, b)
+        for which in (0, 1):
+            ca, ia = system.get_neighbors(which); cb, ib = ref_sys.get_neighbors(which)
+            torch.cuda.synchronize()
+            assert torch.equal(ca, cb)

@@ -60,19 +60,20 @@ def compare_outputs(out_gpu, ref, tol_u=TOL_U, tol_rel=TOL_REL, label=""):
         # the total heat current of a thermal crystal nearly cancels; compare it on the scale
         # sqrt(N) * rms(J_i) of a sum of N terms
         rep["dJtot"] = np.linalg.norm(J.sum(1) - ref["J"].sum(1)) / (jrms * np.sqrt(J.shape[1]))
-        # the literal reading of "within 1e-4 relative of its norm", printed beside it (not asserted:
-        # |sum J| is a cancelling sum ~ sqrt(N) rms(J_i); reading Q18)
-        rep["dJtot_plain"] = np.linalg.norm(J.sum(1) - ref["J"].sum(1)) / max(np.linalg.norm(ref["J"].sum(1)), 1e-300)
+        # the literal reading of "within 1e-4 relative of its norm" (|sum J| is a cancelling sum ~ sqrt(N) rms(J_i);
+        # DESIGN.md reading Q18), asserted as well wherever the reference total is not identically zero
+        jt = np.linalg.norm(ref["J"].sum(1))
+        rep["dJtot_plain"] = np.linalg.norm(J.sum(1) - ref["J"].sum(1)) / jt if jt > 0 else 0.0
     print(label, {k: float("%.3g" % v) for k, v in rep.items()})
     assert rep["dU"] <= tol_u, rep
     for k, v in rep.items():
-        if k not in ("dU", "dJtot_plain"):
+        if k != "dU":
             assert v <= tol_rel, rep
     return rep
 
 
 def run_config(oracle, w, cap_r=64, cap_a=32, skin=1.0, tol_u=TOL_U, tol_rel=TOL_REL, lists=True, path=1):
-    """path = 1: one thread per atom (k_main), whatever the size -- the eight-lanes-per-atom path on the same
+    """path = 1: one thread per atom (k_main), whatever the size -- the 16-lanes-per-atom path (k_gen) on the same
     configs is tests/test_gpu_shapes.py."""
     torch, api = _gpu()
     model, system, pos, vel = api.from_workload(w, cap_r, cap_a, skin, path=path)

@@ -1,4 +1,4 @@
-"""GPU parity of the eight-lanes-per-atom path (k_gen, NEP_PATH_GROUP) and of the model shapes only it covers:
+"""GPU parity of the 16-lanes-per-atom path (k_gen, NEP_PATH_GROUP) and of the model shapes only it covers:
 the paper's three Table I models (80-50-1, 65-40-1, 41-40-1), n_max^R != n_max^A,
 l_max < 4 -- all against the fp64 oracle at the north-star bars (tests/test_gpu_parity.py)."""
 import numpy as np
@@ -44,7 +44,7 @@ def test_group_path_on_baseline_configs(oracle, which):
 
 
 def test_auto_path_switches_with_size(oracle):
-    """nep_system_create picks eight lanes per atom for small systems and one thread per atom for large ones;
+    """nep_system_create picks 16 lanes per atom (k_gen) for small systems and one thread per atom for large ones;
     sizes on either side of the switch (12000 atoms) give the same results as the oracle (C2 with 8000 atoms in
     test_group_path_on_baseline_configs, C4-262144 here)."""
     torch, api = _gpu()

@@ -74,8 +74,25 @@ def test_snes_generation_matches_oracle(oracle):
     assert np.allclose(dm.cpu().numpy(), m2, rtol=1e-13, atol=1e-15) and np.allclose(ds.cpu().numpy(), s2, rtol=1e-13)
 
 
+def test_snes_update_ranks_a_nan_member_last(oracle):
+    """ADVICE round 2 / reading Q25: one member with a NaN loss and one with +inf; the update equals the oracle's, in
+    which both rank last, and stays finite."""
+    torch, api = _gpu()
+    npop, npar = 12, 300
+    m = 0.5 * (2 * inputs.uniform01(83, npar) - 1); s = np.full(npar, 0.1)
+    r = inputs.normal(84, npop * npar).reshape(npop, npar)
+    loss = inputs.uniform01(85, npop); loss[2] = float("nan"); loss[9] = float("inf")
+    dm, ds, dr = [torch.from_numpy(a).cuda() for a in (m, s, r)]
+    api.snes_update(dm, ds, dr, torch.from_numpy(loss).cuda(), 1.0, 0.3)
+    m2, s2 = oracle.snes_update(m, s, r, loss, 1.0, 0.3)
+    assert np.all(np.isfinite(m2)) and np.all(np.isfinite(s2))
+    assert np.allclose(dm.cpu().numpy(), m2, rtol=1e-13, atol=1e-15) and np.allclose(ds.cpu().numpy(), s2, rtol=1e-13)
+
+
 def test_training_loop_reduces_the_loss():
-    """A few SNES generations on synthetic targets (a teacher network evaluated by the library itself): the best loss falls."""
+    """A few SNES generations on synthetic targets (a teacher network evaluated by the library itself): the best loss falls.
+    NOT a parity test: the targets are the library's own predictions, so this checks the sample -> losses -> update loop
+    only; the comparisons with the oracle are the tests above and below."""
     torch, api = _gpu()
     ts = inputs.training_set(16, seed=90)
     dev = "cuda"

@@ -105,3 +105,54 @@ def test_l_max_above_four_matches_oracle(oracle, which, l_max, n_max_a):
     refi = oracle.compute(h, w.atomic_numbers, par, w.pos, w.vel, w.types, w.box, ocR, oiR, ocA, oiA, want_internals=True)
     assert np.abs(q.T - refi["q"]).max() <= 2e-6 * np.abs(refi["q"]).max()
     assert np.abs(fp.T - refi["Fp"]).max() <= 2e-5 * np.abs(refi["Fp"]).max()
+
+
+def _make(api, w, n_max, layers, kind, npar):
+    par = (2.0 * inputs.uniform01(47, npar) - 1.0) / np.sqrt(128.0)
+    return par, api.Model(w.rc_r, w.rc_a, n_max, n_max, 4, layers[0], w.atomic_numbers, par, hidden_layers=list(layers),
+                          angular_kind=kind)
+
+
+def _npar(dim, layers):
+    n, fan = 0, dim
+    for wd in layers:
+        n += (fan + 1) * wd; fan = wd
+    return n + fan + 1
+
+
+def test_shapes_beyond_the_shared_memory_of_k_gen_are_refused():
+    """k_gen stages every layer's weights in shared memory beside its eight per-atom blocks.  Shapes that
+    need more than the device's opt-in limit (227 KB per block on B200) used to be accepted by nep_create_ex and then
+    failed at every launch; they are NEP_EINVAL now (include/nep_b200.h states the budgets)."""
+    torch, api = _gpu()
+    si, pbte = inputs.config0(), inputs.config3(cells=(4, 4, 4))
+    for w, n_max, layers, kind in ((si, 7, (128, 128, 128), 1),        # 3 x 128 over q_nn'l (D = 152), fp32: ~257 KB
+                                   (pbte, 15, (128, 128), 0),          # two species (fp64), 2 x 128 at D = 80: ~328 KB
+                                   (pbte, 7, (128,), 1)):              # two species, one layer of 128 over q_nn'l: ~251 KB
+        dim = (n_max + 1) + ((n_max + 1) * (n_max + 2) // 2 if kind else (n_max + 1)) * 4
+        with pytest.raises(api.NepError) as err:
+            _make(api, w, n_max, layers, kind, _npar(dim, layers))
+        assert err.value.code == -1
+
+
+@pytest.mark.parametrize("which,n_max,layers,kind", [("c0", 15, (128, 128, 128), 0), ("c0", 7, (128, 128), 1),
+                                                       ("c3_replica", 15, (128,), 0), ("c3_replica", 7, (100,), 1)])
+def test_widest_shapes_that_fit_match_oracle(oracle, which, n_max, layers, kind):
+    """The widest networks nep_create_ex still accepts per kernel instantiation (fp32 / fp64, n_max <= 7 / > 7): each is
+    within a few KB of the shared-memory limit, runs, and meets the north-star bars against the oracle."""
+    torch, api = _gpu()
+    w, caps, skin = {"c0": (inputs.config0(), (64, 32), 0.4), "c3_replica": (inputs.config3(cells=(4, 4, 4)), (80, 40), 1.0)}[which]
+    h = oracle.Hyper(w.rc_r, w.rc_a, n_max, n_max, 4, layers[0], len(w.atomic_numbers))
+    h.nlayers = len(layers); h.nneu2 = layers[1] if len(layers) > 1 else 0; h.nneu3 = layers[2] if len(layers) > 2 else 0
+    h.kind = kind
+    npar = oracle.num_params(h)
+    assert npar == _npar(oracle.descriptor_dim(h), layers)
+    par, model = _make(api, w, n_max, layers, kind, npar)
+    system = api.System(model, torch.from_numpy(w.types).cuda(), caps[0], caps[1], skin)
+    assert system.path == 2
+    pos = torch.from_numpy(w.pos).cuda().contiguous(); vel = torch.from_numpy(w.vel).cuda().contiguous()
+    system.neighbors(pos, w.box)
+    out = system.compute(pos, vel)
+    system.status()
+    ref = oracle.evaluate(h, w.atomic_numbers, par, w.pos, w.vel, w.types, w.box, 96, 64)
+    compare_outputs(out, ref, label="%s n_max %d layers %s kind %d" % (which, n_max, layers, kind))

@@ -130,6 +130,105 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def run_train(args):
+    """--workload train[_<S>]: the training side.  A "step" is one SNES generation
+    over a set of S small periodic structures combined into one system (default 24; the paper's sets hold hundreds to
+    thousands): Eq. 35 sample of N_pop = 50 parameter vectors -> nep_trainer_losses (every member evaluates all atoms:
+    stage weights, k_gen, k_assemble, per-structure reduction, Eq. 29-34) -> Eq. 36-39 update.  The metric here is
+    structure-evaluations/s, NOT BASELINE.json's atom-steps/s: this line measures a "next" row, beside the default."""
+    import math
+    import torch
+    from paper_2107_08119_b200 import api, inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    S = int(args.workload.split("_")[1]) if "_" in args.workload else 24
+    n_pop, K, Wm = 50, max(1, min(args.steps, 50)), max(min(args.warmup, 10), 3)
+    dev = "cuda:0"
+    ts = inputs.training_set(S, seed=50)
+    pos = torch.from_numpy(ts.pos).to(dev)
+    shape = (5.0, 4.0, 7, 7, 4, (30,))
+    probe = api.Trainer(*shape, ts.first, ts.boxes, pos)
+    npar = probe.num_params
+    teacher = torch.from_numpy((2 * inputs.uniform01(51, npar) - 1) / math.sqrt(30.0)).to(dev)
+    e_t, f_t, v_t = probe.predict(teacher)                     # synthetic targets: a teacher network (no dataset here)
+    tr = api.Trainer(*shape, ts.first, ts.boxes, pos, e_t, f_t, v_t)
+    m = torch.from_numpy(0.3 * (2 * inputs.uniform01(52, npar) - 1) / math.sqrt(30.0)).to(dev)
+    sd = torch.full((npar,), 0.02, dtype=torch.float64, device=dev)
+    r = torch.from_numpy(inputs.normal(53, n_pop * npar).reshape(n_pop, npar)).to(dev)   # the normals are inputs (Eq. 35)
+    lam = [1.0, 1.0, 0.1, 0.05, 0.05]
+    eta_s = (3 + math.log(npar)) / (5 * math.sqrt(npar))
+
+    def generation():
+        z = api.snes_sample(m, sd, r)
+        L = tr.losses(z, lam)
+        api.snes_update(m, sd, r, L, 1.0, eta_s)
+        return L
+
+    for _ in range(Wm):
+        generation()
+    tr.status()
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(K):
+        L = generation()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    tr.status()
+    # end to end: the generation's normals come from pinned host memory and its losses go back to the host
+    h_r = r.cpu().pin_memory(); h_L = torch.empty((n_pop, 6), dtype=torch.float64).pin_memory()
+    ke = min(K, 10)
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for _ in range(ke):
+        r.copy_(h_r, non_blocking=True)
+        h_L.copy_(generation(), non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+    t1.record()
+    torch.cuda.synchronize()
+    e2e_ms = t0.elapsed_time(t1)
+    # the oracle's loss for a few members, timed on the host cores
+    import oracle
+    h = oracle.Hyper(5.0, 4.0, 7, 7, 4, 30, 1)
+    z_host = api.snes_sample(m, sd, r).cpu().numpy()
+    tgt = [t.cpu().numpy() for t in (e_t, f_t, v_t)]
+    c0 = time.perf_counter(); reps = 0
+    while reps < 1 or (time.perf_counter() - c0 < 10.0 and reps < n_pop):
+        oracle.loss(h, [14], z_host[reps], ts.first, ts.pos, ts.types, ts.boxes, tgt[0], tgt[1], tgt[2], lam)
+        reps += 1
+    cdt = time.perf_counter() - c0
+    flops_atom = algorithmic_flops_per_atom(8, 8, 40, 30, 28.0, 14.0) + 25 * 28.0
+    line = {
+        "metric": "NEP training structure-evaluations/s", "value": n_pop * S * K / (ms * 1e-3), "unit": "structure-evaluations/s",
+        "n_gpus": 1, "steps": K, "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "%s: one SNES generation, N_pop = %d members x %d Si structures (%d atoms, 63-64 per structure), "
+                               "D=40 NN 40-30-1, targets from a teacher network" % (args.workload, n_pop, S, ts.n_atoms),
+                   "n_structures": S, "n_atoms": ts.n_atoms, "n_pop": n_pop, "n_par": npar,
+                   "l2": "working set far below L2 by nature of the workload (small structures): L2-resident, stated, not flushed",
+                   "best_loss_last_generation": float(L[:, 5].min())},
+        "clocks": clocks,
+        "e2e": {"value": n_pop * S * ke / (e2e_ms * 1e-3), "unit": "structure-evaluations/s",
+                "h2d_bytes_per_step": n_pop * npar * 8, "d2h_bytes_per_step": n_pop * 6 * 8, "steps": ke,
+                "what": "per generation: pinned-host normals -> device, sample + losses + update, losses -> pinned host"},
+        "gpu_launches": K * (n_pop * 6 + 2),
+        "launches_per_generation": n_pop * 6 + 2,
+        "roofline": {"bound": "alu", "kernel": "k_gen inside the member loop (whole generation time as the denominator)",
+                     "achieved": flops_atom * ts.n_atoms * n_pop / (ms / K * 1e-3) / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                     "frac": flops_atom * ts.n_atoms * n_pop / (ms / K * 1e-3) / 1e12 / FP32_PEAK_TFLOPS, "traffic": None,
+                     "what": "useful FP32 flops of all members' evaluations / generation time: launch- and latency-bound "
+                             "(members run one after another, each a fraction of one wave)"},
+        "cpu_baseline": {"value": S * reps / cdt, "unit": "structure-evaluations/s", "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": "orc_loss for %d of the %d members over the same %d structures, %.1f s" % (reps, n_pop, S, cdt)},
+    }
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -140,6 +239,10 @@ def main():
     ap.add_argument("--skin", type=float, default=None, help="Verlet skin in A (default 1.0; 0.4 for c0, whose box must exceed 2 (r_c^R + skin))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.workload.startswith("train"):
+        if args.impl == "reference":
+            raise SystemExit("--impl reference times the MD workloads; the train line carries its own cpu_baseline")
+        return run_train(args)
     if args.impl == "reference":
         return run_reference(args)
 
@@ -218,21 +321,40 @@ def main():
     phase_ms = {k: v["ms"] / kp for k, v in prof.items()}
     tot_phase = sum(phase_ms.values())
 
-    # ---- end to end through the C ABI with HOST buffers: per step H2D(pos, vel) + one MD step + D2H ----
+    # ---- end to end through the C ABI with HOST buffers: per step H2D(pos, vel) + one MD step + D2H of everything ----
+    # The trajectory runs THROUGH the host: step n+1's positions and velocities are the ones step n brought back, so
+    # H2D -> step -> D2H(pos, vel) is a true dependency chain.  Only the 67 MB of U, F, W, J are off that chain: they go
+    # back on a second stream from one of two output sets while the next step's H2D and compute run, and the host
+    # reads them one step late.  Every byte of every step is copied inside the timed region.
     ke = min(K, 50)
     h_pos = pos.cpu().pin_memory(); h_vel = vel.cpu().pin_memory()
-    h_out = [torch.empty_like(t, device="cpu").pin_memory() for t in out]
+    outs = [out, system.alloc_outputs()]
+    h_outs = [[torch.empty_like(t, device="cpu").pin_memory() for t in out] for _ in range(2)]
+    s_main = torch.cuda.current_stream()
+    s_out = torch.cuda.Stream()
+    ev_state = [torch.cuda.Event() for _ in range(2)]          # pos, vel of step n are on their way to the host
+    ev_out = [torch.cuda.Event() for _ in range(2)]            # output set n % 2 has reached the host
     system.md_step(pos, vel, w.masses, w.dt, 1, out)          # warm the 1-step path
     barrier()
     t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
     t0.record()
-    for _ in range(ke):
+    for n in range(ke):
+        b = n & 1
         pos.copy_(h_pos, non_blocking=True); vel.copy_(h_vel, non_blocking=True)
-        system.md_step(pos, vel, w.masses, w.dt, 1, out)
+        if n >= 2:
+            s_main.wait_event(ev_out[b])                       # the step overwrites output set b: its last copy must be done
+        system.md_step(pos, vel, w.masses, w.dt, 1, outs[b])
         h_pos.copy_(pos, non_blocking=True); h_vel.copy_(vel, non_blocking=True)
-        for hd, dd in zip(h_out, out):
-            hd.copy_(dd, non_blocking=True)
-        torch.cuda.current_stream().synchronize()              # the host reads the step's result
+        ev_state[b].record(s_main)
+        s_out.wait_event(ev_state[b])                          # after pos, vel: the two D2H transfers do not share the link
+        with torch.cuda.stream(s_out):
+            for hd, dd in zip(h_outs[b], outs[b]):
+                hd.copy_(dd, non_blocking=True)
+            ev_out[b].record(s_out)
+        s_main.synchronize()                                   # the host has step n's positions and velocities ...
+        if n >= 1:
+            ev_out[1 - b].synchronize()                        # ... and reads step n-1's U, F, W, J
+    s_out.synchronize()
     t1.record()
     barrier()
     e2e_ms = t0.elapsed_time(t1)
@@ -262,13 +384,13 @@ def main():
         hbm_phases[name] = {"bound": "hbm", "bytes_per_atom": nbytes, "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
                             "frac": gbs / hbm_peak}
     # Counters of the dominant kernel from the committed ncu --set full capture of this same command
-    # (profiles/r2_k_main_counters.json; 1M-atom workload, one thread per atom): DRAM bytes per launch and the
+    # (profiles/r3_k_main_counters.json; 1M-atom workload, one thread per atom): DRAM bytes per launch and the
     # EXECUTED FP32 flops per launch (FFMA = 2, FFMA2 = 4, FMUL/FADD = 1, summed over the SASS of one launch).
     traffic = executed = None
     counters_src = None
     try:
         if args.workload == "c4_1048576" and system.path == 1:
-            cj = json.load(open(os.path.join(ROOT, "profiles", "r2_k_main_counters.json")))
+            cj = json.load(open(os.path.join(ROOT, "profiles", "r3_k_main_counters.json")))
             traffic = cj["k_main_dram_bytes_per_launch"]
             executed = cj["k_main_executed_fp32_flops_per_launch"]
             counters_src = cj["capture"]
@@ -296,7 +418,9 @@ def main():
             "clocks": clocks,
             "e2e": {"value": world * N * ke / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "steps": ke,
-                    "what": "per step: pinned-host pos+vel -> device, nep_md_step(1), pos+vel+U+F+W+J -> pinned host"},
+                    "what": "per step: pinned-host pos+vel -> device, nep_md_step(1), pos+vel -> pinned host (the next step's input: a true "
+                            "dependency through the host), U+F+W+J -> pinned host on a second stream from double-buffered output "
+                            "sets, overlapping the next step; the host reads them one step late"},
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "kernel": ("k_main, one thread per atom" if system.path == 1 else "k_gen, 16 lanes per atom") +
                                                   " (descriptor + network + partial forces)",

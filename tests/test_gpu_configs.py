@@ -84,7 +84,7 @@ def test_md_c4_32768_with_rebuild(oracle):
     _md_leg(oracle, inputs.config4(32768), 60, 64, 32, 2, "C4 Si 32768", 1e-4)
 
 
-def _md_final_state(oracle, w, n_steps, cap_r, cap_a, min_rebuilds, label, oracle_md_steps=0):
+def _md_final_state(oracle, w, n_steps, cap_r, cap_a, min_rebuilds, label, oracle_md_steps=0, max_drift=2e-5, ocaps=(96, 64)):
     """MD above 65,536 atoms, where launch_build takes its third form: the ten-kernel device-gated chain that re-sorts
     an already sorted state (first = 0, gated = 2), with k_main's per-SM parking slots and the kick+drift fused into
     k_assemble (npad >= 262144) -- the configuration bench.py times.
@@ -119,13 +119,30 @@ def _md_final_state(oracle, w, n_steps, cap_r, cap_a, min_rebuilds, label, oracl
     drift = np.abs(E - E[0]).max() / w.n_atoms
     print("%s: %d steps, rebuilds %d, |E-E0|/N %.3g eV" % (label, n_steps, st["rebuilds"], drift))
     assert st["rebuilds"] >= min_rebuilds + 1, st          # the initial nep_neighbors counts as one
-    assert drift < 2e-5
+    assert max_drift is None or drift < max_drift
     gpos, gvel = pos.cpu().numpy(), vel.cpu().numpy()
     w2 = inputs.Workload(w.name, gpos, gvel, w.types, w.box, w.rc_r, w.rc_a, w.n_max_r, w.n_max_a, w.l_max,
                          w.n_neurons, w.atomic_numbers, w.masses, w.params)
     check_lists(oracle, w2, system, cap_r, cap_a)
-    ref2 = oracle.evaluate(h, w.atomic_numbers, w.params, gpos, gvel, w.types, w.box, 96, 64)
+    ref2 = oracle.evaluate(h, w.atomic_numbers, w.params, gpos, gvel, w.types, w.box, ocaps[0], ocaps[1])
     compare_outputs(out, ref2, label=label + " final state")
+
+
+def test_md_c3_pbte_all_1000_steps_final_state(oracle):
+    """BASELINE.json configs[3] in full: 1000 NVE steps of the 64,000-atom PbTe cell (the MD legs above follow orc_md for
+    20).  A chaotic trajectory cannot be compared step by step that far, and the random-weight PbTe surface heats in the
+    oracle too (section 3 of DESIGN.md), so what is checked is the state the GPU arrives at after ~50 in-loop rebuilds
+    (permutations composed rebuild after rebuild, velocities carried): lists bit-exact, U, F, W, J at the bars.
+    Measured: the seeded random-weight model is not a stable potential at dt = 1 fs -- E/N rises by 12.4 eV over the
+    1000 steps (2.6e-4 after 20 steps on the GPU and in orc_md alike, 3.6e-2 after 200), the lists are rebuilt 420
+    times -- and the hot, disordered end state still meets every bar: the comparison is about the arithmetic, not the
+    physics of a random network."""
+    _md_final_state(oracle, inputs.config3(), 1000, 80, 40, 20, "C3 PbTe 64000, 1000 steps", max_drift=None, ocaps=(124, 64))
+
+
+def test_md_c4_32768_all_1000_steps_final_state(oracle):
+    """BASELINE.json configs[4], smallest size, all 1000 steps: energy flat to 2e-5 eV/atom, final state at the bars."""
+    _md_final_state(oracle, inputs.config4(32768), 1000, 64, 32, 20, "C4 Si 32768, 1000 steps")
 
 
 def test_md_c4_262144_gated_rebuild_chain(oracle):

@@ -89,6 +89,42 @@ def test_snes_update_ranks_a_nan_member_last(oracle):
     assert np.allclose(dm.cpu().numpy(), m2, rtol=1e-13, atol=1e-15) and np.allclose(ds.cpu().numpy(), s2, rtol=1e-13)
 
 
+def test_a_broken_member_is_reported_and_ranked_last(oracle):
+    """One member of the population has NaN weights: its losses come out non-finite, nep_trainer_status reports
+    NEP_ENAN for the generation (sticky bit set in k_assemble), the other members' losses are untouched, and the SNES
+    update that follows ranks the broken member last (reading Q25) -- m and s stay finite and equal the oracle's."""
+    torch, api = _gpu()
+    ts = inputs.training_set(6, seed=93)
+    dev = "cuda"
+    pos = torch.from_numpy(ts.pos).to(dev)
+    probe = api.Trainer(5.0, 4.0, 3, 3, 2, (8,), ts.first, ts.boxes, pos)
+    npar = probe.num_params
+    teacher = torch.from_numpy((2 * inputs.uniform01(94, npar) - 1) * 0.5).to(dev)
+    e_t, f_t, v_t = probe.predict(teacher)
+    tr = api.Trainer(5.0, 4.0, 3, 3, 2, (8,), ts.first, ts.boxes, pos, e_t, f_t, v_t)
+    npop = 8
+    m = 0.5 * (2 * inputs.uniform01(95, npar) - 1); s = np.full(npar, 0.1)
+    r = inputs.normal(96, npop * npar).reshape(npop, npar)
+    dm, ds, dr = [torch.from_numpy(a).to(dev) for a in (m, s, r)]
+    z = api.snes_sample(dm, ds, dr)
+    lam = [1.0, 1.0, 1.0, 0.0, 0.0]
+    good = tr.losses(z, lam).cpu().numpy()
+    tr.status()                                                   # a healthy generation: no error
+    z[3] = float("nan")
+    L = tr.losses(z, lam)
+    with pytest.raises(api.NepError) as err:
+        tr.status()
+    assert err.value.code == -8                                   # NEP_ENAN
+    Lh = L.cpu().numpy()
+    # the others as before (to rounding: k_train_reduce adds its per-structure squared errors with fp64 atomics)
+    assert not np.isfinite(Lh[3, 5]) and np.allclose(np.delete(Lh, 3, axis=0), np.delete(good, 3, axis=0), rtol=1e-12, atol=0)
+    api.snes_update(dm, ds, dr, L, 1.0, 0.3)
+    m2, s2 = oracle.snes_update(m, s, r, Lh[:, 5], 1.0, 0.3)
+    assert np.all(np.isfinite(m2)) and np.all(np.isfinite(s2))
+    assert np.allclose(dm.cpu().numpy(), m2, rtol=1e-13, atol=1e-15) and np.allclose(ds.cpu().numpy(), s2, rtol=1e-13)
+    tr.status()                                                   # the sticky bit was cleared by the read above
+
+
 def test_training_loop_reduces_the_loss():
     """A few SNES generations on synthetic targets (a teacher network evaluated by the library itself): the best loss falls.
     NOT a parity test: the targets are the library's own predictions, so this checks the sample -> losses -> update loop
